@@ -1,0 +1,162 @@
+/*
+ * hea.h -- C ABI of libhea_b200: the data-parallel hot path of PyHEA (arxiv 2411.18906) on NVIDIA B200 (sm_100a).
+ *
+ * The path (citations "P:<n>" = PAPER.md line; "D<n>/A<n>" = DESIGN.md section 3):
+ *   hea_create        lattice supercell S = A*L^3, species concentrations, coordination shells,
+ *                     shell weights w_k and target alpha; builds the shell neighbour tables on the host (D1-D3)
+ *   hea_init_random   seeded exact-composition random start (D8)
+ *   hea_sro_full      full Warren-Cowley recount: ordered pair counts N_ij^(k), alpha_ij^(k) = 1 - P_ij^(k)/c_j (Eq. 2,
+ *                     P:256-262) and J = F^2 = sum_k w_k sum_ij (alpha - alpha_target)^2 (Eq. 3)  (D4-D6)
+ *   hea_mc_run        chain-parallel Monte Carlo local search (Alg. 3): per step K candidate swaps, each
+ *                     evaluated by the incremental pair-count update (Eq. 4; Eq. 5), the
+ *                     lowest-index improving candidate applied (D9; Eq. 6 P:313 is the "best-of-K" variant, not built)
+ *
+ * Conventions for every call
+ *   - All functions return HEA_OK (0) or an error code; hea_last_error() gives a thread-local message.
+ *   - Pointers named *_dev are DEVICE pointers on the context's device, owned by the caller (e.g. torch tensors);
+ *     pointers named *_host are HOST pointers owned by the caller.  The library owns only hea_ctx and its tables.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device entry points are
+ *     asynchronous on that stream: argument errors are reported synchronously before any launch; device faults
+ *     surface at the caller's next synchronisation.  *_host entry points are synchronous.
+ *   - Layouts are dense, row-major, little-endian: occ [C][N] uint8 (species id < n_species; larger values are
+ *     undefined behaviour, not validated on the hot path), counts [C][S][M][M] int32, alpha [C][S][M][M] double.
+ *   - Site order (D1): site = ((x*Ly + y)*Lz + z)*A + b with basis fcc A=4 (0,0,0),(0,1,1),(1,0,1),(1,1,0),
+ *     bcc A=2 (0,0,0),(1,1,1) in units of a/2.  Shells (D2): fcc |o|^2 = 2,4,6 (z = 12,6,24), bcc 3,4,8 (z = 8,6,12),
+ *     offsets in lexicographic order, periodic; tiny cells keep exactly z_s table entries (multi-edge semantics).
+ *   - There is no CPU fallback: without a CUDA device every compute call returns HEA_ECUDA.
+ */
+#ifndef HEA_H
+#define HEA_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hea_ctx hea_ctx;                 /* opaque; created by hea_create, freed by hea_destroy */
+
+enum { HEA_FCC = 0, HEA_BCC = 1 };
+enum { HEA_OK = 0, HEA_EINVAL = 1, HEA_EUNSUPPORTED = 2, HEA_ENOMEM = 3, HEA_ECUDA = 4 };
+
+#define HEA_MAX_SPECIES 8
+#define HEA_MAX_SHELLS  3
+#define HEA_MAX_K       1024
+#define HEA_HASH_INIT   0xcbf29ce484222325ULL   /* initial value of hea_mc_stats.hash (D9.4) */
+#define HEA_NO_STEP     0xffffffffffffffffULL   /* initial value of hea_mc_stats.last_accept_step */
+
+/* Per-chain running statistics of hea_mc_run (in/out: counters and hash continue across calls; J is output). */
+typedef struct {
+    uint64_t n_accept;           /* accepted moves */
+    uint64_t n_null;             /* candidate slots that stayed like-species after the one redraw (D9.1) */
+    uint64_t hash;               /* FNV-1a style hash over (step lo, step hi, k, a, b) of every accepted move */
+    uint64_t last_accept_step;   /* absolute step of the last accepted move, HEA_NO_STEP if none */
+    double   J;                  /* objective J = F^2 of the current configuration (D6) */
+} hea_mc_stats;
+
+/* One accepted move. */
+typedef struct { uint64_t step; uint32_t k, a, b; } hea_move;
+
+/* Library version string (static storage). */
+const char* hea_version(void);
+
+/* Thread-local message of the last error returned on this thread (static storage, never NULL). */
+const char* hea_last_error(void);
+
+/*
+ * hea_create -- problem statement of the paper: P:105 (lattice, supercell), P:35/P:142 (species, concentrations),
+ * P:271 (shells, weights w_k, target alpha).
+ *   lattice          HEA_FCC | HEA_BCC;  Lx,Ly,Lz >= 1 conventional cells;  N = A*Lx*Ly*Lz < 2^31
+ *   conc             [n_species] host, > 0, sums to 1 within 1e-9; species counts N_i by D3 (round if integral,
+ *                    else floor + largest remainder, ties to the lower index); any N_i == 0 -> HEA_EINVAL
+ *   shell_w          [n_shells] host;  alpha_target [n_shells][n_species][n_species] host, row-major
+ *   n_species in [1, 8], n_shells in [1, 3] (else HEA_EUNSUPPORTED)
+ *   device           CUDA device ordinal.  Builds both device copies of the neighbour table
+ *                    (site-major for the MC kernel, slot-major for the recount kernel).
+ * All host arrays are copied.  Errors: HEA_EINVAL, HEA_EUNSUPPORTED, HEA_ENOMEM, HEA_ECUDA (no device / alloc failed).
+ */
+int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz,
+               int n_species, const double* conc,
+               int n_shells, const double* shell_w, const double* alpha_target,
+               int device);
+
+/* Frees the context and its device tables.  NULL is allowed. */
+int hea_destroy(hea_ctx* ctx);
+
+/* n_sites, z[n_shells], n_per_species[n_species] (any output pointer may be NULL). */
+int hea_info(const hea_ctx* ctx, int64_t* n_sites, int* z, int64_t* n_per_species);
+
+/* Host copy of the shell's neighbour table, [N][z_shell] int32, entry k = site at offset o_k (D2).  For tests. */
+int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host);
+
+/*
+ * Tuning knobs (never change results).  name:
+ *   "mc_lanes"        lanes cooperating on one candidate: 0 = auto, else 1,2,4,8,16,32
+ *   "mc_occ_mode"     0 = auto, 1 = shared uint8, 2 = shared 4-bit packed, 3 = global memory (through L2)
+ *   "mc_threads"      threads per chain block: 0 = auto, else a multiple of 32 in [32, 1024]
+ *   "mc_cluster"      CTAs per chain (thread-block cluster, replicated occupancy): 0 = auto, 1, 2, 4, 8
+ *   "mc_neighbors"    0 = auto, 1 = neighbour table, 2 = computed from the lattice stencil
+ *   "sro_variant"     0 = auto, 1 = direct table gather, 2 = shared-memory staged table tiles
+ * Unknown name or value -> HEA_EINVAL.
+ */
+int hea_set_option(hea_ctx* ctx, const char* name, int64_t value);
+int hea_get_option(const hea_ctx* ctx, const char* name, int64_t* value);
+
+/*
+ * hea_init_random -- D8 ("generated entirely randomly"): occ[c] = species blocks in ascending order, then
+ * Fisher-Yates for n = N-1..1 with j = (Philox4x32-10(ctr=(n,0,0xFFFFFFFF,chain0+c), key=seed)[0] * (n+1)) >> 32.
+ *   occ_dev [C][N] uint8 out;  chain0 + C <= 2^32.
+ */
+int hea_init_random(hea_ctx* ctx, uint8_t* occ_dev, int64_t C, uint64_t seed, uint64_t chain0, void* cuda_stream);
+
+/*
+ * hea_sro_full -- D4-D6 (Eq. 2, Eq. 3): for each of B configurations
+ *   counts[s][i][j] = #{(a, k < z_s) : occ[a] = i and occ[nbr_s[a][k]] = j}      (ordered pairs, int32)
+ *   alpha[s][i][j]  = 1 - counts * g,  g = N / (z_s N_i N_j)                       (optional, may be NULL)
+ *   obj[b]          = J = sum_s w_s sum_i sum_j (alpha - alpha_target)^2           (optional, may be NULL)
+ * evaluated in fp64 in the fixed order of D6 (no FMA contraction).  counts_dev is overwritten.
+ */
+int hea_sro_full(hea_ctx* ctx, const uint8_t* occ_dev, int64_t B,
+                 int32_t* counts_dev, double* alpha_dev, double* obj_dev, void* cuda_stream);
+
+/* Sets stats_dev[0..C) to {0, 0, HEA_HASH_INIT, HEA_NO_STEP, 0.0}. */
+int hea_mc_stats_reset(hea_ctx* ctx, hea_mc_stats* stats_dev, int64_t C, void* cuda_stream);
+
+/*
+ * hea_mc_run -- D9 (Alg. 3 P:242-250 with Eq. 4-5): advances C independent chains by n_steps steps.
+ * Per chain c (global id chain0 + c < 2^32) and absolute step t = step0 + 0..n_steps-1:
+ *   for k = 0..K-1: (r0..r3) = Philox4x32-10(ctr=(t lo, t hi, k, chain), key=seed); a = (r0*N)>>32,
+ *   b = (r1*(N-1))>>32, b += (b >= a); if occ[a] == occ[b] redraw once from (r2, r3); still alike -> null candidate.
+ *   Every non-null candidate's J_k is computed from counts + delta (neighbours of a and b except a, b themselves)
+ *   in the D6 order; the lowest k with J_k < J_cur (strict) is applied: occ swapped, counts updated, stats updated.
+ *   occ_dev    [C][N] in/out
+ *   counts_dev [C][S][M][M] in/out; MUST equal the recount of occ_dev on entry (get it from hea_sro_full)
+ *   stats_dev  [C] in/out (see hea_mc_stats; initialise with hea_mc_stats_reset for a fresh chain)
+ *   log_dev    [C][log_cap] accepted moves of THIS call in order (first log_cap of them), or NULL with log_cap 0
+ *   K in [1, HEA_MAX_K].  Results depend only on (seed, chain id, step), never on C, batching or tuning options:
+ *   run(S1) followed by run(S2, step0 = S1) equals run(S1 + S2).
+ */
+int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, uint64_t n_steps, int K,
+               uint64_t seed, uint64_t chain0, uint64_t step0,
+               hea_mc_stats* stats_dev, hea_move* log_dev, int64_t log_cap, void* cuda_stream);
+
+/*
+ * Host-buffer (end-to-end) forms: the same kernels, with host<->device copies done by the library on an internal
+ * stream, synchronous.  Host buffers may be pageable or pinned.
+ *   hea_sro_full_host: occ_host [B][N] -> counts_host (required), alpha_host / obj_host (optional).
+ *   hea_mc_run_host:   occ_host [C][N] in/out; the library recounts occ on the device first (so no counts input),
+ *                      runs hea_mc_run, and returns occ, counts_host [C][S][M][M] (optional) and stats_host [C]
+ *                      (in/out, required).
+ */
+int hea_sro_full_host(hea_ctx* ctx, const uint8_t* occ_host, int64_t B,
+                      int32_t* counts_host, double* alpha_host, double* obj_host);
+int hea_mc_run_host(hea_ctx* ctx, uint8_t* occ_host, int32_t* counts_host, int64_t C, uint64_t n_steps, int K,
+                    uint64_t seed, uint64_t chain0, uint64_t step0, hea_mc_stats* stats_host);
+
+/* Number of kernel launches issued by this context since creation (for bench.py's gpu_launches). */
+int hea_launch_count(const hea_ctx* ctx, int64_t* n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HEA_H */

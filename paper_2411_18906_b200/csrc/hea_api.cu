@@ -1,0 +1,429 @@
+// hea_api.cu -- the C ABI of libhea_b200 (include/hea.h): context, validation, launches.  No torch types.
+#include "../../include/hea.h"
+
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "hea_device.cuh"
+#include "hea_lattice.hpp"
+
+namespace hea {
+// launchers (hea_sro.cu / hea_mc.cu)
+cudaError_t launch_sro_count(const KParams& P, const uint8_t* occ, int64_t B, int32_t* counts, int n_sms,
+                             cudaStream_t st, int64_t* n_launches);
+cudaError_t launch_sro_epilogue(const KParams& P, const int32_t* counts, int64_t B, double* alpha, double* obj,
+                                cudaStream_t st, int64_t* n_launches);
+cudaError_t launch_init_random(const KParams& P, uint8_t* occ, int64_t C, uint64_t seed, uint64_t chain0,
+                               const int64_t* n_per_species_dev, cudaStream_t st, int64_t* n_launches);
+cudaError_t launch_stats_reset(void* stats, int64_t C, cudaStream_t st, int64_t* n_launches);
+cudaError_t launch_transpose_table(const int32_t* site_major, int32_t* slot_major, int N, int Npad, int Z,
+                                   cudaStream_t st, int64_t* n_launches);
+size_t mc_shared_bytes(int occ_mode, int N);
+cudaError_t launch_mc(const KParams& P, int lanes, int occ_mode, int threads, uint8_t* occ, int32_t* counts,
+                      int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0, uint64_t step0,
+                      void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches);
+}  // namespace hea
+
+struct hea_ctx {
+    hea::Lattice lat;
+    int M = 0, S = 0;
+    int64_t n_per_species[hea::kMaxSpecies] = {0};
+    int device = 0;
+    int n_sms = 0;
+    size_t smem_optin = 0;
+    int32_t* d_nbr_site = nullptr;
+    int32_t* d_nbr_slot = nullptr;
+    hea::DevTables* d_tab = nullptr;
+    int64_t* d_nps = nullptr;
+    hea::KParams P{};
+    // tuning options (0 = auto)
+    int64_t opt_lanes = 0, opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_neighbors = 0, opt_sro_variant = 0;
+    int64_t n_launches = 0;
+    // internal stream and scratch for the *_host entry points
+    cudaStream_t stream = nullptr;
+    void* scratch[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    size_t scratch_cap[5] = {0, 0, 0, 0, 0};
+};
+
+namespace {
+
+thread_local std::string g_err = "";
+
+int fail(int code, const std::string& msg)
+{
+    g_err = msg;
+    return code;
+}
+
+int fail_cuda(cudaError_t e, const char* what)
+{
+    g_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return HEA_ECUDA;
+}
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; prev = -1; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+int ensure_scratch(hea_ctx* ctx, int slot, size_t bytes)
+{
+    if (ctx->scratch_cap[slot] >= bytes) return HEA_OK;
+    if (ctx->scratch[slot]) cudaFree(ctx->scratch[slot]);
+    ctx->scratch[slot] = nullptr;
+    ctx->scratch_cap[slot] = 0;
+    cudaError_t e = cudaMalloc(&ctx->scratch[slot], bytes);
+    if (e != cudaSuccess) return fail(HEA_ENOMEM, std::string("cudaMalloc scratch: ") + cudaGetErrorString(e));
+    ctx->scratch_cap[slot] = bytes;
+    return HEA_OK;
+}
+
+int64_t* option_slot(hea_ctx* ctx, const char* name)
+{
+    if (!name) return nullptr;
+    if (!strcmp(name, "mc_lanes")) return &ctx->opt_lanes;
+    if (!strcmp(name, "mc_occ_mode")) return &ctx->opt_occ_mode;
+    if (!strcmp(name, "mc_threads")) return &ctx->opt_threads;
+    if (!strcmp(name, "mc_cluster")) return &ctx->opt_cluster;
+    if (!strcmp(name, "mc_neighbors")) return &ctx->opt_neighbors;
+    if (!strcmp(name, "sro_variant")) return &ctx->opt_sro_variant;
+    return nullptr;
+}
+
+bool option_value_ok(const char* name, int64_t v)
+{
+    if (v == 0) return true;
+    if (!strcmp(name, "mc_lanes")) return v == 1 || v == 2 || v == 4 || v == 8 || v == 16 || v == 32;
+    if (!strcmp(name, "mc_occ_mode")) return v >= 1 && v <= 3;
+    if (!strcmp(name, "mc_threads")) return v >= 32 && v <= 1024 && v % 32 == 0;
+    if (!strcmp(name, "mc_cluster")) return v == 1 || v == 2 || v == 4 || v == 8;
+    if (!strcmp(name, "mc_neighbors")) return v == 1 || v == 2;
+    if (!strcmp(name, "sro_variant")) return v == 1 || v == 2;
+    return false;
+}
+
+int floor_pow2(int64_t v)
+{
+    int p = 1;
+    while ((int64_t)p * 2 <= v) p *= 2;
+    return p;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* hea_version(void) { return "hea-b200 0.1 (sm_100a)"; }
+
+const char* hea_last_error(void) { return g_err.c_str(); }
+
+int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz, int n_species, const double* conc, int n_shells,
+               const double* shell_w, const double* alpha_target, int device)
+{
+    if (!out) return fail(HEA_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!conc || !shell_w || !alpha_target) return fail(HEA_EINVAL, "conc / shell_w / alpha_target is NULL");
+    if (n_species < 1 || n_species > HEA_MAX_SPECIES) return fail(HEA_EUNSUPPORTED, "n_species must be in [1, 8]");
+    if (n_shells < 1 || n_shells > HEA_MAX_SHELLS) return fail(HEA_EUNSUPPORTED, "n_shells must be in [1, 3]");
+    if (lattice != HEA_FCC && lattice != HEA_BCC) return fail(HEA_EINVAL, "lattice must be HEA_FCC or HEA_BCC");
+
+    hea_ctx* ctx = new (std::nothrow) hea_ctx();
+    if (!ctx) return fail(HEA_ENOMEM, "out of host memory");
+    std::string err = hea::lattice_init(ctx->lat, lattice, Lx, Ly, Lz, n_shells);
+    if (!err.empty()) { delete ctx; return fail(HEA_EINVAL, err); }
+    ctx->M = n_species;
+    ctx->S = n_shells;
+    err = hea::species_counts(ctx->lat.N, n_species, conc, ctx->n_per_species);
+    if (!err.empty()) { delete ctx; return fail(HEA_EINVAL, err); }
+
+    int n_dev = 0;
+    cudaError_t e = cudaGetDeviceCount(&n_dev);
+    if (e != cudaSuccess || n_dev <= 0) {
+        delete ctx;
+        return fail(HEA_ECUDA, std::string("no CUDA device available (this library has no CPU fallback): ") +
+                                   cudaGetErrorString(e));
+    }
+    if (device < 0 || device >= n_dev) { delete ctx; return fail(HEA_EINVAL, "device ordinal out of range"); }
+    ctx->device = device;
+    DeviceGuard guard(device);
+    if (!guard.ok) { delete ctx; return fail(HEA_ECUDA, "cudaSetDevice failed"); }
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) { delete ctx; return fail_cuda(e, "cudaGetDeviceProperties"); }
+    ctx->n_sms = prop.multiProcessorCount;
+    ctx->smem_optin = prop.sharedMemPerBlockOptin;
+
+    const hea::Lattice& lat = ctx->lat;
+    const int N = (int)lat.N, Z = lat.Z, M = n_species, S = n_shells;
+    const int Npad = (N + 3) & ~3;
+
+    // constant tables (D5-D6: den exact in fp64, one correctly rounded divide)
+    std::vector<hea::DevTables> tab(1);
+    memset(tab.data(), 0, sizeof(hea::DevTables));
+    for (int s = 0; s < S; ++s) {
+        tab[0].w[s] = shell_w[s];
+        for (int i = 0; i < M; ++i)
+            for (int j = 0; j < M; ++j) {
+                const int idx = (s * M + i) * M + j;
+                const double den = (double)((int64_t)lat.z[s] * ctx->n_per_species[i] * ctx->n_per_species[j]);
+                tab[0].g[idx] = (double)lat.N / den;
+                tab[0].t[idx] = alpha_target[idx];
+            }
+    }
+    for (int b = 0; b < lat.A; ++b)
+        for (int k = 0; k < Z; ++k) {
+            const hea::StencilEntry& st = lat.stencil[b][k];
+            int8_t* dst = tab[0].stencil + (b * Z + k) * 4;
+            dst[0] = st.nb; dst[1] = st.sx; dst[2] = st.sy; dst[3] = st.sz;
+        }
+
+    auto bail = [&](int code, const std::string& msg) {
+        hea_destroy(ctx);
+        return fail(code, msg);
+    };
+    if ((e = cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking)) != cudaSuccess)
+        return bail(HEA_ECUDA, std::string("cudaStreamCreate: ") + cudaGetErrorString(e));
+    if ((e = cudaMalloc(&ctx->d_tab, sizeof(hea::DevTables))) != cudaSuccess ||
+        (e = cudaMalloc(&ctx->d_nps, sizeof(int64_t) * hea::kMaxSpecies)) != cudaSuccess ||
+        (e = cudaMalloc(&ctx->d_nbr_site, sizeof(int32_t) * (size_t)N * Z)) != cudaSuccess ||
+        (e = cudaMalloc(&ctx->d_nbr_slot, sizeof(int32_t) * (size_t)Npad * Z)) != cudaSuccess)
+        return bail(HEA_ENOMEM, std::string("cudaMalloc tables: ") + cudaGetErrorString(e));
+    if ((e = cudaMemcpy(ctx->d_tab, tab.data(), sizeof(hea::DevTables), cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMemcpy(ctx->d_nps, ctx->n_per_species, sizeof(int64_t) * hea::kMaxSpecies, cudaMemcpyHostToDevice)) != cudaSuccess)
+        return bail(HEA_ECUDA, std::string("cudaMemcpy tables: ") + cudaGetErrorString(e));
+
+    // host table builder -> site-major device table, in chunks; slot-major copy by a device transpose
+    {
+        const int64_t chunk_sites = 1 << 20;
+        std::vector<int32_t> buf((size_t)std::min<int64_t>(chunk_sites, N) * Z);
+        for (int64_t first = 0; first < N; first += chunk_sites) {
+            const int64_t last = std::min<int64_t>(N, first + chunk_sites);
+            hea::build_site_major(lat, first, last, buf.data());
+            e = cudaMemcpy(ctx->d_nbr_site + (size_t)first * Z, buf.data(), sizeof(int32_t) * (size_t)(last - first) * Z,
+                           cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) return bail(HEA_ECUDA, std::string("cudaMemcpy table: ") + cudaGetErrorString(e));
+        }
+        e = hea::launch_transpose_table(ctx->d_nbr_site, ctx->d_nbr_slot, N, Npad, Z, ctx->stream, &ctx->n_launches);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) return bail(HEA_ECUDA, std::string("table transpose: ") + cudaGetErrorString(e));
+    }
+
+    hea::KParams& P = ctx->P;
+    P.N = N; P.Npad = Npad; P.M = M; P.S = S; P.Z = Z; P.A = lat.A;
+    for (int d = 0; d < 3; ++d) P.L[d] = lat.L[d];
+    for (int s = 0; s < 3; ++s) P.z[s] = s < S ? lat.z[s] : 0;
+    for (int s = 0; s < 4; ++s) P.zoff[s] = s <= S ? lat.zoff[s] : Z;
+    P.nbr_site = ctx->d_nbr_site;
+    P.nbr_slot = ctx->d_nbr_slot;
+    P.tab = ctx->d_tab;
+    *out = ctx;
+    return HEA_OK;
+}
+
+int hea_destroy(hea_ctx* ctx)
+{
+    if (!ctx) return HEA_OK;
+    {
+        DeviceGuard guard(ctx->device);
+        if (ctx->stream) { cudaStreamSynchronize(ctx->stream); cudaStreamDestroy(ctx->stream); }
+        cudaFree(ctx->d_tab);
+        cudaFree(ctx->d_nps);
+        cudaFree(ctx->d_nbr_site);
+        cudaFree(ctx->d_nbr_slot);
+        for (void* p : ctx->scratch) cudaFree(p);
+    }
+    delete ctx;
+    return HEA_OK;
+}
+
+int hea_info(const hea_ctx* ctx, int64_t* n_sites, int* z, int64_t* n_per_species)
+{
+    if (!ctx) return fail(HEA_EINVAL, "ctx is NULL");
+    if (n_sites) *n_sites = ctx->lat.N;
+    if (z) for (int s = 0; s < ctx->S; ++s) z[s] = ctx->lat.z[s];
+    if (n_per_species) for (int i = 0; i < ctx->M; ++i) n_per_species[i] = ctx->n_per_species[i];
+    return HEA_OK;
+}
+
+int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host)
+{
+    if (!ctx || !out_host) return fail(HEA_EINVAL, "ctx / out_host is NULL");
+    if (shell < 0 || shell >= ctx->S) return fail(HEA_EINVAL, "shell out of range");
+    hea::build_shell_table(ctx->lat, shell, out_host);
+    return HEA_OK;
+}
+
+int hea_set_option(hea_ctx* ctx, const char* name, int64_t value)
+{
+    if (!ctx) return fail(HEA_EINVAL, "ctx is NULL");
+    int64_t* slot = option_slot(ctx, name);
+    if (!slot) return fail(HEA_EINVAL, "unknown option name");
+    if (!option_value_ok(name, value)) return fail(HEA_EINVAL, "option value not allowed");
+    *slot = value;
+    return HEA_OK;
+}
+
+int hea_get_option(const hea_ctx* ctx, const char* name, int64_t* value)
+{
+    if (!ctx || !value) return fail(HEA_EINVAL, "ctx / value is NULL");
+    int64_t* slot = option_slot(const_cast<hea_ctx*>(ctx), name);
+    if (!slot) return fail(HEA_EINVAL, "unknown option name");
+    *value = *slot;
+    return HEA_OK;
+}
+
+int hea_launch_count(const hea_ctx* ctx, int64_t* n)
+{
+    if (!ctx || !n) return fail(HEA_EINVAL, "ctx / n is NULL");
+    *n = ctx->n_launches;
+    return HEA_OK;
+}
+
+int hea_init_random(hea_ctx* ctx, uint8_t* occ_dev, int64_t C, uint64_t seed, uint64_t chain0, void* cuda_stream)
+{
+    if (!ctx || !occ_dev) return fail(HEA_EINVAL, "ctx / occ_dev is NULL");
+    if (C < 0 || chain0 + (uint64_t)C > (1ull << 32)) return fail(HEA_EINVAL, "chain ids must be < 2^32");
+    if (C == 0) return HEA_OK;
+    DeviceGuard guard(ctx->device);
+    cudaError_t e = hea::launch_init_random(ctx->P, occ_dev, C, seed, chain0, ctx->d_nps, (cudaStream_t)cuda_stream,
+                                            &ctx->n_launches);
+    return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_init_random launch");
+}
+
+int hea_sro_full(hea_ctx* ctx, const uint8_t* occ_dev, int64_t B, int32_t* counts_dev, double* alpha_dev,
+                 double* obj_dev, void* cuda_stream)
+{
+    if (!ctx || !occ_dev || !counts_dev) return fail(HEA_EINVAL, "ctx / occ_dev / counts_dev is NULL");
+    if (B < 0) return fail(HEA_EINVAL, "B must be >= 0");
+    if (B == 0) return HEA_OK;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = hea::launch_sro_count(ctx->P, occ_dev, B, counts_dev, ctx->n_sms, st, &ctx->n_launches);
+    if (e != cudaSuccess) return fail_cuda(e, "hea_sro_full count launch");
+    e = hea::launch_sro_epilogue(ctx->P, counts_dev, B, alpha_dev, obj_dev, st, &ctx->n_launches);
+    return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_sro_full epilogue launch");
+}
+
+int hea_mc_stats_reset(hea_ctx* ctx, hea_mc_stats* stats_dev, int64_t C, void* cuda_stream)
+{
+    if (!ctx || !stats_dev) return fail(HEA_EINVAL, "ctx / stats_dev is NULL");
+    if (C < 0) return fail(HEA_EINVAL, "C must be >= 0");
+    if (C == 0) return HEA_OK;
+    DeviceGuard guard(ctx->device);
+    cudaError_t e = hea::launch_stats_reset(stats_dev, C, (cudaStream_t)cuda_stream, &ctx->n_launches);
+    return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_mc_stats_reset launch");
+}
+
+int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, uint64_t n_steps, int K, uint64_t seed,
+               uint64_t chain0, uint64_t step0, hea_mc_stats* stats_dev, hea_move* log_dev, int64_t log_cap,
+               void* cuda_stream)
+{
+    static_assert(sizeof(hea_mc_stats) == 40, "hea_mc_stats layout");
+    static_assert(sizeof(hea_move) == 24, "hea_move layout");
+    if (!ctx || !occ_dev || !counts_dev || !stats_dev) return fail(HEA_EINVAL, "ctx / occ_dev / counts_dev / stats_dev is NULL");
+    if (K < 1 || K > HEA_MAX_K) return fail(HEA_EINVAL, "K must be in [1, 1024]");
+    if (C < 0 || chain0 + (uint64_t)C > (1ull << 32)) return fail(HEA_EINVAL, "chain ids must be < 2^32");
+    if (log_cap < 0 || (log_cap > 0 && !log_dev)) return fail(HEA_EINVAL, "log_cap > 0 needs log_dev");
+    if (step0 + n_steps < step0) return fail(HEA_EINVAL, "step0 + n_steps overflows");
+    if (C == 0) return HEA_OK;
+    DeviceGuard guard(ctx->device);
+    const int N = ctx->P.N;
+
+    // ---- launch configuration (results never depend on it)
+    int occ_mode = (int)ctx->opt_occ_mode;
+    const size_t budget = ctx->smem_optin;
+    if (occ_mode == 0) {
+        if (hea::mc_shared_bytes(1, N) <= budget) occ_mode = 1;
+        else if (hea::mc_shared_bytes(2, N) <= budget) occ_mode = 2;
+        else occ_mode = 3;
+    } else if (hea::mc_shared_bytes(occ_mode, N) > budget) {
+        return fail(HEA_EINVAL, "mc_occ_mode does not fit in shared memory for this N");
+    }
+    int lanes = (int)ctx->opt_lanes;
+    if (lanes == 0) {
+        const int64_t total = (int64_t)C * K;
+        lanes = floor_pow2(std::max<int64_t>(1, (int64_t)ctx->n_sms * 2048 / std::max<int64_t>(1, total)));
+        lanes = std::min(lanes, 32);
+        lanes = std::min(lanes, floor_pow2(std::max(1, 1024 / K)));
+    }
+    int threads = (int)ctx->opt_threads;
+    if (threads == 0) {
+        threads = (int)std::min<int64_t>(1024, (int64_t)K * lanes);
+        threads = (threads + 31) & ~31;
+    }
+    cudaError_t e = hea::launch_mc(ctx->P, lanes, occ_mode, threads, occ_dev, counts_dev, C, n_steps, K, seed, chain0,
+                                   step0, stats_dev, log_dev, log_cap, (cudaStream_t)cuda_stream, &ctx->n_launches);
+    return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_mc_run launch");
+}
+
+int hea_sro_full_host(hea_ctx* ctx, const uint8_t* occ_host, int64_t B, int32_t* counts_host, double* alpha_host,
+                      double* obj_host)
+{
+    if (!ctx || !occ_host || !counts_host) return fail(HEA_EINVAL, "ctx / occ_host / counts_host is NULL");
+    if (B < 0) return fail(HEA_EINVAL, "B must be >= 0");
+    if (B == 0) return HEA_OK;
+    DeviceGuard guard(ctx->device);
+    const size_t N = (size_t)ctx->P.N, SMM = (size_t)ctx->S * ctx->M * ctx->M;
+    int rc;
+    if ((rc = ensure_scratch(ctx, 0, N * B)) != HEA_OK) return rc;
+    if ((rc = ensure_scratch(ctx, 1, sizeof(int32_t) * SMM * B)) != HEA_OK) return rc;
+    if (alpha_host && (rc = ensure_scratch(ctx, 2, sizeof(double) * SMM * B)) != HEA_OK) return rc;
+    if (obj_host && (rc = ensure_scratch(ctx, 3, sizeof(double) * B)) != HEA_OK) return rc;
+    cudaStream_t st = ctx->stream;
+    cudaError_t e = cudaMemcpyAsync(ctx->scratch[0], occ_host, N * B, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return fail_cuda(e, "H2D occ");
+    rc = hea_sro_full(ctx, (const uint8_t*)ctx->scratch[0], B, (int32_t*)ctx->scratch[1],
+                      alpha_host ? (double*)ctx->scratch[2] : nullptr, obj_host ? (double*)ctx->scratch[3] : nullptr, st);
+    if (rc != HEA_OK) return rc;
+    e = cudaMemcpyAsync(counts_host, ctx->scratch[1], sizeof(int32_t) * SMM * B, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && alpha_host)
+        e = cudaMemcpyAsync(alpha_host, ctx->scratch[2], sizeof(double) * SMM * B, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && obj_host)
+        e = cudaMemcpyAsync(obj_host, ctx->scratch[3], sizeof(double) * B, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_sro_full_host");
+}
+
+int hea_mc_run_host(hea_ctx* ctx, uint8_t* occ_host, int32_t* counts_host, int64_t C, uint64_t n_steps, int K,
+                    uint64_t seed, uint64_t chain0, uint64_t step0, hea_mc_stats* stats_host)
+{
+    if (!ctx || !occ_host || !stats_host) return fail(HEA_EINVAL, "ctx / occ_host / stats_host is NULL");
+    if (C < 0) return fail(HEA_EINVAL, "C must be >= 0");
+    if (C == 0) return HEA_OK;
+    DeviceGuard guard(ctx->device);
+    const size_t N = (size_t)ctx->P.N, SMM = (size_t)ctx->S * ctx->M * ctx->M;
+    int rc;
+    if ((rc = ensure_scratch(ctx, 0, N * C)) != HEA_OK) return rc;
+    if ((rc = ensure_scratch(ctx, 1, sizeof(int32_t) * SMM * C)) != HEA_OK) return rc;
+    if ((rc = ensure_scratch(ctx, 4, sizeof(hea_mc_stats) * C)) != HEA_OK) return rc;
+    cudaStream_t st = ctx->stream;
+    cudaError_t e = cudaMemcpyAsync(ctx->scratch[0], occ_host, N * C, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(ctx->scratch[4], stats_host, sizeof(hea_mc_stats) * C, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return fail_cuda(e, "H2D occ/stats");
+    rc = hea_sro_full(ctx, (const uint8_t*)ctx->scratch[0], C, (int32_t*)ctx->scratch[1], nullptr, nullptr, st);
+    if (rc != HEA_OK) return rc;
+    rc = hea_mc_run(ctx, (uint8_t*)ctx->scratch[0], (int32_t*)ctx->scratch[1], C, n_steps, K, seed, chain0, step0,
+                    (hea_mc_stats*)ctx->scratch[4], nullptr, 0, st);
+    if (rc != HEA_OK) return rc;
+    e = cudaMemcpyAsync(occ_host, ctx->scratch[0], N * C, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && counts_host)
+        e = cudaMemcpyAsync(counts_host, ctx->scratch[1], sizeof(int32_t) * SMM * C, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(stats_host, ctx->scratch[4], sizeof(hea_mc_stats) * C, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_mc_run_host");
+}
+
+}  // extern "C"

@@ -1,0 +1,61 @@
+// hea_device.cuh -- device-side parameter blocks and small helpers shared by the kernels of libhea_b200.
+// Product code (sm_100a); shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace hea {
+
+constexpr int kSMM = 3 * 8 * 8;           // max S*M*M
+
+// Constant tables of one context, resident in device global memory (copied to shared memory by the MC kernel).
+struct DevTables {
+    double g[kSMM];                       // g[s][i][j] = N / (z_s N_i N_j), compact index (s*M + i)*M + j  (D5-D6)
+    double t[kSMM];                       // alpha target, same index
+    double w[4];                          // shell weights
+    int8_t stencil[4 * 42 * 4];           // [b][e] -> (nb, sx, sy, sz), e over the concatenated shells, stride Z
+};
+
+// Scalars passed by value to every kernel.
+struct KParams {
+    int N;                                // sites
+    int Npad;                             // N rounded up to a multiple of 4 (row stride of the slot-major table)
+    int M, S, Z, A;
+    int L[3];
+    int z[3];
+    int zoff[4];
+    const int32_t* nbr_site;              // [N][Z]   site-major: the Z neighbours of one site are contiguous
+    const int32_t* nbr_slot;              // [Z][Npad] slot-major: one slot of consecutive sites is contiguous
+    const DevTables* tab;
+};
+
+// ---------------------------------------------------------------- Philox4x32-10 (Salmon et al. SC'11; D7)
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               uint32_t k0, uint32_t k1)
+{
+    constexpr uint32_t MUL_A = 0xD2511F53u, MUL_B = 0xCD9E8D57u;
+    constexpr uint32_t BUMP_A = 0x9E3779B9u, BUMP_B = 0xBB67AE85u;
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        const uint32_t a_hi = __umulhi(MUL_A, c0), a_lo = MUL_A * c0;
+        const uint32_t b_hi = __umulhi(MUL_B, c2), b_lo = MUL_B * c2;
+        c0 = b_hi ^ c1 ^ k0;
+        c1 = b_lo;
+        c2 = a_hi ^ c3 ^ k1;
+        c3 = a_lo;
+        k0 += BUMP_A;
+        k1 += BUMP_B;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// D6: one squared deviation, every operation individually rounded (no FMA contraction).
+__device__ __forceinline__ double sq_dev(int n, double g, double t)
+{
+    const double x = __dmul_rn((double)n, g);
+    const double al = __dsub_rn(1.0, x);
+    const double d = __dsub_rn(al, t);
+    return __dmul_rn(d, d);
+}
+
+}  // namespace hea

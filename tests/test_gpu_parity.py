@@ -1,0 +1,246 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Bar (BASELINE.json:north_star): pair counts, occupancies, accepted-move sequences, n_accept, n_null
+bit-exact; J within 1e-12 relative (it is expected, and asserted, to be bit-equal under D6)."""
+import numpy as np
+import pytest
+
+from oracle import hea_oracle as ho
+from paper_2411_18906_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def hb():
+    import torch
+    from paper_2411_18906_b200 import binding
+    assert torch.cuda.is_available()
+    return binding
+
+
+def pair(hb, w):
+    return hb.Hea(*w.create_args()), ho.Oracle(*w.create_args())
+
+
+def small(lattice, dims, conc, S, target_seed=None, rng=(-0.1, 0.1), **kw):
+    base = dict(name="t", lattice=lattice, dims=dims, conc=conc, n_shells=S, shell_w=[1.0, 0.5, 0.25][:S],
+                n_chains=4, n_steps=50, K=8, seed=42, target_seed=target_seed, target_range=rng)
+    base.update(kw)
+    return wl.Workload(**base)
+
+
+def assert_stats_equal(got, want):
+    for f in ("n_accept", "n_null", "hash", "last_accept_step"):
+        np.testing.assert_array_equal(got[f], want[f], err_msg=f)
+    np.testing.assert_allclose(got["J"], want["J"], rtol=1e-12, atol=0)
+    np.testing.assert_array_equal(got["J"], want["J"])            # bit-equal under the fixed D6 order
+
+
+LATTICES = [("fcc", (3, 3, 3), [0.5, 0.5], 3), ("fcc", (3, 4, 5), [0.2] * 5, 3), ("bcc", (4, 3, 5), [0.25] * 4, 3),
+            ("bcc", (3, 3, 3), [0.5, 0.25, 0.25], 2), ("fcc", (1, 1, 1), [0.5, 0.5], 3), ("bcc", (1, 2, 3), [0.5, 0.5], 3),
+            ("fcc", (2, 2, 2), [0.125] * 8, 3), ("bcc", (7, 7, 7), [1 / 7] * 7, 1), ("fcc", (6, 5, 4), [0.4, 0.4, 0.1, 0.1], 2),
+            ("bcc", (2, 2, 2), [1.0], 3), ("fcc", (4, 4, 4), [1 / 6] * 6, 3), ("bcc", (5, 5, 5), [0.2, 0.3, 0.5], 3)]
+
+
+@pytest.mark.parametrize("lattice,dims,conc,S", LATTICES)
+def test_info_and_neighbor_table(hb, lattice, dims, conc, S):
+    h, o = pair(hb, small(lattice, dims, conc, S))
+    assert (h.N, h.z, h.n_per_species) == (o.N, o.z, o.n_per_species)
+    for s in range(S):
+        np.testing.assert_array_equal(h.neighbor_table(s), o.neighbor_table(s))
+
+
+@pytest.mark.parametrize("lattice,dims,conc,S", LATTICES)
+def test_init_and_sro_full_bit_exact(hb, lattice, dims, conc, S):
+    w = small(lattice, dims, conc, S, target_seed=3)
+    h, o = pair(hb, w)
+    B = 5
+    occ = h.init_random(B, seed=w.seed, chain0=7)
+    want_occ = o.init_random(B, seed=w.seed, chain0=7)
+    np.testing.assert_array_equal(occ.cpu().numpy(), want_occ)
+    counts, alpha, obj = h.sro_full(occ)
+    wc, wa, wj = o.sro_full(want_occ)
+    np.testing.assert_array_equal(counts.cpu().numpy(), wc)
+    np.testing.assert_array_equal(alpha.cpu().numpy(), wa)
+    np.testing.assert_array_equal(obj.cpu().numpy(), wj)
+
+
+def test_sro_full_ordered_structures(hb):
+    # B2 on bcc: closed form alpha (+1/-1), through the GPU path
+    w = small("bcc", (6, 6, 6), [0.5, 0.5], 3)
+    h, o = pair(hb, w)
+    import torch
+    occ = torch.tensor(np.arange(h.N, dtype=np.int64) % 2, dtype=torch.uint8, device="cuda").reshape(1, -1)
+    counts, alpha, obj = h.sro_full(occ)
+    al = alpha.cpu().numpy()[0]
+    np.testing.assert_array_equal(al[0], [[1, -1], [-1, 1]])
+    np.testing.assert_array_equal(al[1], [[-1, 1], [1, -1]])
+    np.testing.assert_array_equal(counts.cpu().numpy()[0], o.pair_counts(occ.cpu().numpy()[0]))
+
+
+@pytest.mark.parametrize("L,B", [(10, 3), (16, 2), (23, 1)])
+def test_sro_full_multi_tile_and_ragged(hb, L, B):
+    # several blocks / grid-stride iterations, flushes of the 16-bit accumulators, N % 4 != 0 for bcc odd L
+    for lattice, conc in (("fcc", [0.2] * 5), ("bcc", None)):
+        if conc is None:
+            n = 2 * L ** 3
+            conc = [0.5, 0.25, 0.25] if n % 4 == 0 else [0.5, 0.5]
+        w = small(lattice, (L, L, L), conc, 3, target_seed=9)
+        h, o = pair(hb, w)
+        occ = h.init_random(B, seed=5)
+        counts, alpha, obj = h.sro_full(occ)
+        wc, wa, wj = o.sro_full(occ.cpu().numpy(), n_threads=4)
+        np.testing.assert_array_equal(counts.cpu().numpy(), wc)
+        np.testing.assert_array_equal(obj.cpu().numpy(), wj)
+
+
+def run_both(hb, w, n_chains, n_steps, log_cap=16, chain0=0, step0=0, opts=None, threads=8):
+    h, o = pair(hb, w)
+    for k, v in (opts or {}).items():
+        h.set_option(k, v)
+    occ = h.init_random(n_chains, seed=w.seed, chain0=chain0)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    o_occ = occ.cpu().numpy().copy()
+    o_cnt = counts.cpu().numpy().copy()
+    stats, log = h.mc_run(occ, counts, n_steps, w.K, w.seed, chain0=chain0, step0=step0, log_cap=log_cap)
+    o_stats, o_log = o.mc_run(o_occ, o_cnt, n_steps, w.K, w.seed, chain0=chain0, step0=step0, log_cap=log_cap,
+                              n_threads=threads, eval_all=False)
+    np.testing.assert_array_equal(occ.cpu().numpy(), o_occ)
+    np.testing.assert_array_equal(counts.cpu().numpy(), o_cnt)
+    assert_stats_equal(hb.stats_to_numpy(stats), o_stats)
+    if log_cap:
+        got = hb.log_to_numpy(log)
+        for c in range(n_chains):
+            n = min(int(o_stats["n_accept"][c]), log_cap)
+            for f in ("step", "k", "a", "b"):
+                np.testing.assert_array_equal(got[c][:n][f], o_log[c][:n][f])
+    # the incremental counts equal a fresh recount of the final configuration
+    recount, _, obj = h.sro_full(occ)
+    np.testing.assert_array_equal(recount.cpu().numpy(), o_cnt)
+    np.testing.assert_array_equal(obj.cpu().numpy(), o_stats["J"])
+    return o_stats
+
+
+@pytest.mark.parametrize("lanes", [1, 2, 4, 8, 16, 32])
+@pytest.mark.parametrize("occ_mode", [1, 2, 3])
+def test_mc_parity_all_launch_variants(hb, lanes, occ_mode):
+    w = small("fcc", (4, 4, 4), [0.2, 0.2, 0.2, 0.4], 3, target_seed=5, K=24, n_steps=120)
+    st = run_both(hb, w, 5, 120, opts={"mc_lanes": lanes, "mc_occ_mode": occ_mode})
+    assert st["n_accept"].sum() > 50
+
+
+@pytest.mark.parametrize("lattice,dims,conc,S", LATTICES[:9])
+def test_mc_parity_lattices_including_degenerate_cells(hb, lattice, dims, conc, S):
+    w = small(lattice, dims, conc, S, target_seed=11, K=16)
+    run_both(hb, w, 3, 80)
+
+
+@pytest.mark.parametrize("K,threads", [(1, 0), (7, 32), (33, 64), (200, 0), (1024, 0), (64, 96)])
+def test_mc_parity_candidate_counts(hb, K, threads):
+    w = small("bcc", (5, 5, 5), [0.2, 0.3, 0.5], 3, target_seed=2, K=K)
+    run_both(hb, w, 3, 40, opts={"mc_threads": threads})
+
+
+def test_mc_c1_full(hb):
+    w = wl.config(1)                                        # 64 chains x 10,000 steps x K=32, target 0
+    st = run_both(hb, w, w.n_chains, w.n_steps, log_cap=64)
+    assert int(st["n_accept"][0]) == 53 and float(st["J"][0]) == 0.0     # SURVEY cross-check values
+
+
+def test_mc_c2_prefix(hb):
+    w = wl.config(2)
+    run_both(hb, w, 32, 3000)
+
+
+def test_mc_c3_prefix(hb):
+    w = wl.config(3)
+    st = run_both(hb, w, 8, 400, log_cap=400)
+    assert (st["n_accept"] > 300).all()                    # accept regime
+
+
+def test_mc_c4_prefix(hb):
+    w = wl.config(4)
+    st = run_both(hb, w, 4, 300, log_cap=300)
+    assert (st["n_accept"] > 250).all()
+
+
+def test_mc_c4_global_occupancy_path(hb):
+    w = wl.config(4)
+    run_both(hb, w, 2, 100, opts={"mc_occ_mode": 3, "mc_lanes": 32})
+
+
+def test_mc_split_run_and_chain_offset(hb):
+    w = small("fcc", (5, 5, 5), [0.2] * 5, 2, K=32, seed=1)
+    h, o = pair(hb, w)
+    occ0 = h.init_random(6, seed=w.seed)
+    cnt0, _, _ = h.sro_full(occ0, want_alpha=False, want_obj=False)
+    occ, cnt = occ0.clone(), cnt0.clone()
+    st, _ = h.mc_run(occ, cnt, 400, w.K, w.seed)
+    occ_s, cnt_s = occ0.clone(), cnt0.clone()
+    st_s, _ = h.mc_run(occ_s, cnt_s, 150, w.K, w.seed)
+    st_s, _ = h.mc_run(occ_s, cnt_s, 250, w.K, w.seed, step0=150, stats=st_s)
+    assert (occ == occ_s).all() and (cnt == cnt_s).all() and (st == st_s).all()
+    occ_c, cnt_c = occ0[2:].clone(), cnt0[2:].clone()
+    h.set_option("mc_lanes", 4)
+    st_c, _ = h.mc_run(occ_c, cnt_c, 400, w.K, w.seed, chain0=2)
+    assert (occ[2:] == occ_c).all() and (st[2:] == st_c).all()
+
+
+def test_mc_large_step_offset(hb):
+    w = small("bcc", (4, 4, 4), [0.25] * 4, 3, target_seed=8, K=16)
+    run_both(hb, w, 2, 60, step0=(1 << 32) - 20, chain0=(1 << 32) - 2)
+
+
+def test_empty_and_zero_step_calls(hb):
+    import torch
+    w = small("bcc", (3, 3, 3), [0.5, 0.5], 2)
+    h, o = pair(hb, w)
+    occ = h.init_random(2, seed=1)
+    counts, _, obj = h.sro_full(occ)
+    before = occ.clone()
+    st, _ = h.mc_run(occ, counts, 0, 8, 1)                   # zero steps: state unchanged, J reported
+    assert (occ == before).all()
+    np.testing.assert_array_equal(hb.stats_to_numpy(st)["J"], obj.cpu().numpy())
+    empty = torch.empty((0, h.N), dtype=torch.uint8, device="cuda")
+    c0, _, _ = h.sro_full(empty)
+    assert c0.shape[0] == 0
+
+
+def test_argument_errors(hb):
+    w = small("bcc", (3, 3, 3), [0.5, 0.5], 2)
+    h, _ = pair(hb, w)
+    occ = h.init_random(1, seed=1)
+    counts, _, _ = h.sro_full(occ)
+    with pytest.raises(hb.HeaError) as e:
+        h.mc_run(occ, counts, 1, 0, 1)
+    assert e.value.code == hb.HEA_EINVAL
+    with pytest.raises(hb.HeaError):
+        h.mc_run(occ, counts, 1, 2000, 1)
+    with pytest.raises(hb.HeaError):
+        h.set_option("mc_lanes", 3)
+    with pytest.raises(hb.HeaError):
+        h.set_option("nonsense", 1)
+    with pytest.raises(hb.HeaError) as e:
+        hb.Hea("fcc", (2, 2, 2), [0.5, 0.4], [1.0], np.zeros((1, 2, 2)))
+    assert e.value.code == hb.HEA_EINVAL
+    with pytest.raises(hb.HeaError) as e:
+        hb.Hea("fcc", (2, 2, 2), [1 / 9] * 9, [1.0], np.zeros((1, 9, 9)))
+    assert e.value.code == hb.HEA_EUNSUPPORTED
+
+
+def test_host_buffer_entry_points(hb):
+    w = small("fcc", (6, 6, 6), [0.25] * 4, 2, target_seed=4, K=32)
+    h, o = pair(hb, w)
+    occ = o.init_random(6, seed=w.seed)
+    counts, alpha, obj = h.sro_full_host(occ, want_alpha=True)
+    wc, wa, wj = o.sro_full(occ)
+    np.testing.assert_array_equal(counts, wc)
+    np.testing.assert_array_equal(alpha, wa)
+    np.testing.assert_array_equal(obj, wj)
+    g_occ = occ.copy()
+    g_counts, g_stats = h.mc_run_host(g_occ, 200, w.K, w.seed)
+    o_cnt = wc.copy()
+    o_stats, _ = o.mc_run(occ, o_cnt, 200, w.K, w.seed, n_threads=4)
+    np.testing.assert_array_equal(g_occ, occ)
+    np.testing.assert_array_equal(g_counts, o_cnt)
+    assert_stats_equal(g_stats, o_stats)
