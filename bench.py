@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py -- the driver's measurement contract for libhea_b200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--mc-steps n]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+Workload (BASELINE.json:configs[3], "c4"): fcc 40x40x40 = 256,000 atoms, 4 species at 0.25, shells 1-2, non-zero
+first-shell target (seed 11), 16 chains per GPU, K = 128 candidates per MC step.  One bench "step" is one pass of the
+whole hot path over that batch: `hea_sro_full` of the 16 configurations (counts, alpha, J) followed by
+`hea_mc_run` for --mc-steps MC steps of every chain (default 50,000; the 1e7-step trajectory of the config is
+cut into such segments -- split-run invariance, D9, makes the result identical to one long call).
+`value` = swap trials/s = chains * mc-steps * K / device time of the whole step, inputs resident in HBM.
+`e2e` = the same metric through the host-buffer C-ABI call `hea_mc_run_host` (H2D of the occupancies from pinned
+memory, recount, MC, D2H of occupancies + counts + stats inside the timed region).
+Multi-GPU: chains are independent, so rank r runs chains [16 r, 16 r + 16) with no data-path collective ("weak").
+
+`roofline` is for the dominant kernel of the step (the MC kernel; ALU-issue bound, model in DESIGN.md section 6);
+`recount_roofline` is for the recount kernel on the sweep point of configs[4] where the neighbour table exceeds L2
+(fcc 100^3 = 4,000,000 atoms, 3 shells, batch 1; HBM bound, 4*Z+1 = 169 B/atom).
+`cpu_baseline` / `--impl reference`: the CPU oracle (oracle/hea_oracle.c), as it stands, on the host cores.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "delta-SRO swap trials/sec (c4: fcc 40^3, 256,000 atoms, 16 chains, K=128) incl. full-SRO recount per step"
+UNIT = "swap-trials/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+# ALU-issue model of one swap trial: thread-instructions the method needs per candidate.
+def mc_ops_per_trial(Z, S, M):
+    philox = 10 * 4 + 4                 # 10 rounds x (2 wide multiplies + 2 three-input xors) + 4 bounded draws
+    gather = 2 * Z * 5                  # per neighbour entry: index, species load, 2 compares folded, shift, add
+    objective = S * M * M * 6 + S * M + S * 2   # per cell: cvt, mul, sub, sub, mul, add; row/shell/weight combines
+    return philox + gather + objective
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------ oracle legs (CPU)
+def oracle_mc_sample(w, n_chains, n_steps, threads):
+    """Times the oracle (all K candidates evaluated every step) on n_chains x n_steps of workload w."""
+    from oracle import hea_oracle
+    o = hea_oracle.Oracle(*w.create_args())
+    occ = o.init_random(n_chains, w.seed)
+    cnt, _, _ = o.sro_full(occ, n_threads=threads)
+    t0 = time.perf_counter()
+    o.sro_full(occ, n_threads=threads)
+    t_rc = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    o.mc_run(occ, cnt, n_steps, w.K, w.seed, n_threads=threads, eval_all=True)
+    t_mc = time.perf_counter() - t0
+    return t_rc, t_mc, min(threads, n_chains)
+
+
+def cpu_baseline(w, budget_s=12.0):
+    cores = os.cpu_count() or 1
+    n_chains = w.n_chains
+    t_rc, t_mc, used = oracle_mc_sample(w, n_chains, 200, cores)          # calibration
+    n_steps = int(max(200, min(2_000_000, 200 * budget_s / max(t_mc, 1e-6))))
+    t_rc, t_mc, used = oracle_mc_sample(w, n_chains, n_steps, cores)
+    trials = n_chains * n_steps * w.K
+    return {"value": trials / (t_rc + t_mc), "unit": UNIT, "cores": used, "kind": "oracle",
+            "sample": f"{n_chains} chains x {n_steps} MC steps x K={w.K} of c4 (all K evaluated) after one recount of "
+                      f"the {n_chains} configurations; oracle/hea_oracle.c, gcc -O2, one thread per chain",
+            "mc_trials_per_s": trials / t_mc, "recount_atoms_per_s": n_chains * w.n_sites / t_rc,
+            "seconds": t_rc + t_mc}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores, same metric/config, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2411_18906_b200 import workloads
+    w = workloads.config(4)
+    cores = os.cpu_count() or 1
+    n_steps = args.ref_mc_steps
+    for _ in range(args.warmup):
+        oracle_mc_sample(w, w.n_chains, max(1, n_steps // 10), cores)
+    t_all, used = 0.0, 1
+    for _ in range(args.steps):
+        t_rc, t_mc, used = oracle_mc_sample(w, w.n_chains, n_steps, cores)
+        t_all += t_rc + t_mc
+    trials = w.n_chains * n_steps * w.K
+    value = trials * args.steps / t_all
+    sample = (f"per step: one recount of {w.n_chains} configurations + {n_steps} MC steps x K={w.K} on "
+              f"{w.n_chains} chains of c4 (all K evaluated)")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t_all / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int32 counts + f64 objective", "data": "synthetic",
+        "config": {"workload": "c4: fcc 40x40x40 (256,000 atoms), 4 species 0.25 each, shells 1-2, target seed 11, "
+                               "16 chains, K=128", "mc_steps_per_step": n_steps},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------------------ GPU arm
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--mc-steps", type=int, default=50_000, help="MC steps per chain per bench step")
+    ap.add_argument("--ref-mc-steps", type=int, default=2_000, help="MC steps per bench step of the reference arm")
+    ap.add_argument("--recount-L", type=int, default=100, help="fcc L^3 cells of the recount roofline point")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-recount", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], help="tuning option name=value (hea_set_option)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        args.warmup = 3                                   # timing rule: W >= 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2411_18906_b200 import binding, workloads
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libhea_b200 has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    hbm_peak, sm_max_mhz, peak_src = load_peaks()
+
+    w = workloads.config(4)
+    h = binding.Hea(*w.create_args(), device=local_rank)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        h.set_option(k, int(v))
+    C, K, N, n_mc = w.n_chains, w.K, w.n_sites, args.mc_steps
+    SMM = h.S * h.M * h.M
+    chain0 = rank * C
+    occ = h.init_random(C, w.seed, chain0)
+    counts = torch.empty((C, h.S, h.M, h.M), dtype=torch.int32, device=dev)
+    stats = h.new_stats(C)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
+    state = {"step0": 0}
+
+    def one_step(ev=None):
+        if ev: ev[0].record()
+        h.sro_full(occ, counts=counts)
+        if ev: ev[1].record()
+        h.mc_run(occ, counts, n_mc, K, w.seed, chain0=chain0, step0=state["step0"], stats=stats)
+        if ev: ev[2].record()
+        state["step0"] += n_mc
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    st0 = binding.stats_to_numpy(stats).copy()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    l0 = h.launch_count()
+    barrier()
+    t_wall0 = time.perf_counter()
+    for i in range(args.steps):
+        flush.fill_(i & 0xFF)                              # L2 flush between timed iterations (outside the events)
+        one_step(evs[i])
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = h.launch_count() - l0
+    t_rc = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
+    t_mc = sum(e[1].elapsed_time(e[2]) for e in evs) * 1e-3
+    t_dev = t_rc + t_mc
+    st1 = binding.stats_to_numpy(stats).copy()
+
+    # sanity outside the timed region: the incremental counts equal a fresh recount of the final occupancies
+    chk, _, _ = h.sro_full(occ)
+    assert bool((chk == counts).all()), "incremental counts diverged from the recount"
+
+    # ---- e2e: host buffers through hea_mc_run_host, copies inside the timed region
+    occ_host = torch.empty((C, N), dtype=torch.uint8).pin_memory()
+    occ_host.copy_(occ.cpu())
+    occ_np = occ_host.numpy()
+    st_host = binding.stats_to_numpy(stats).copy()
+    cnt_host = np.empty((C, h.S, h.M, h.M), dtype=np.int32)
+    e2e_step0 = state["step0"]
+    for _ in range(2):
+        h.mc_run_host(occ_np, n_mc, K, w.seed, chain0=chain0, step0=e2e_step0, stats=st_host, counts_out=cnt_host)
+        e2e_step0 += n_mc
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        h.mc_run_host(occ_np, n_mc, K, w.seed, chain0=chain0, step0=e2e_step0, stats=st_host, counts_out=cnt_host)
+        e2e_step0 += n_mc
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    clocks = sampler.stop()
+    h2d = C * N + 40 * C
+    d2h = C * N + 4 * SMM * C + 40 * C
+
+    # ---- recount roofline point: table larger than L2 (inputs > L2, so no flush needed)
+    recount = None
+    if not args.no_recount:
+        wr = workloads.recount_sweep_workload(args.recount_L, 1)
+        hr = binding.Hea(*wr.create_args(), device=local_rank)
+        occ_r = hr.init_random(1, wr.seed)
+        cnt_r = torch.empty((1, hr.S, hr.M, hr.M), dtype=torch.int32, device=dev)
+        for _ in range(3):
+            hr.sro_full(occ_r, counts=cnt_r, want_alpha=False, want_obj=False)
+        reps = 10
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            hr.sro_full(occ_r, counts=cnt_r, want_alpha=False, want_obj=False)
+        e1.record()
+        torch.cuda.synchronize()
+        t_r = e0.elapsed_time(e1) * 1e-3 / reps
+        Zr = sum(hr.z)
+        bytes_r = (4 * Zr + 1) * hr.N
+        recount = {"bound": "hbm", "achieved": bytes_r / t_r / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                   "frac": bytes_r / t_r / 1e9 / hbm_peak, "traffic": None, "peak_source": peak_src,
+                   "kernel": "sro_count_kernel", "workload": f"fcc {args.recount_L}^3 ({hr.N} atoms), 5 species, "
+                   f"3 shells (Z={Zr}), batch 1; table {4 * Zr * hr.N / 1e6:.0f} MB > L2",
+                   "bytes_per_atom": 4 * Zr + 1, "atoms_per_s": hr.N / t_r, "ms_per_launch": t_r * 1e3}
+        hr.close()
+
+    # ---- reduce over ranks: max time
+    times = torch.tensor([t_dev, t_rc, t_mc, t_e2e, t_wall], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    t_dev, t_rc, t_mc, t_e2e, t_wall = [float(x) for x in times.cpu()]
+    trials_per_step = world * C * n_mc * K
+    value = trials_per_step * args.steps / t_dev
+    ops = mc_ops_per_trial(sum(h.z), h.S, h.M)
+    n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    alu_peak = n_sms * 128 * sm_max_mhz * 1e6 / 1e12                    # T thread-instr/s: 4 SMSPs x 32 lanes / clk
+    mc_rate_1gpu = C * n_mc * K * args.steps / t_mc
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int32 counts + f64 objective", "data": "synthetic",
+        "config": {"workload": "c4: fcc 40x40x40 (256,000 atoms), 4 species 0.25 each, shells 1-2 (w 1, 0.5), "
+                               "first-shell target in [-0.2, 0.2] from seed 11, 16 chains per GPU, K=128, chain seed 4",
+                   "mc_steps_per_step": n_mc, "chains_per_gpu": C, "K": K, "l2": "flushed between timed iterations "
+                   "(256 MB fill, outside the events)", "parallelism": f"chains sharded, {world} rank(s), no collective"},
+        "recount_atoms_per_s": world * C * N * args.steps / t_rc,
+        "mc_trials_per_s": world * mc_rate_1gpu,
+        "accept_rate": float((st1["n_accept"] - st0["n_accept"]).sum()) / (C * n_mc * args.steps),
+        "null_rate": float((st1["n_null"] - st0["n_null"]).sum()) / (C * n_mc * args.steps * K),
+        "J_mean": float(st1["J"].mean()),
+        "wall_ms_per_step_incl_flush": 1e3 * t_wall / args.steps,
+        "clocks": clocks,
+        "e2e": {"value": trials_per_step * args.steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "api": "hea_mc_run_host (pinned host occupancies)"},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "achieved": mc_rate_1gpu * ops / 1e12, "peak": alu_peak,
+                     "unit": "T thread-instr/s", "frac": mc_rate_1gpu * ops / 1e12 / alu_peak, "traffic": None,
+                     "kernel": "mc_chain_kernel", "ops_per_trial": ops, "ms_per_launch": 1e3 * t_mc / args.steps,
+                     "peak_source": f"{n_sms} SMs x 128 lanes/clk x {sm_max_mhz:.0f} MHz (DESIGN.md section 6)"},
+    }
+    if recount:
+        line["recount_roofline"] = recount
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -292,9 +292,10 @@ int hea_launch_count(const hea_ctx* ctx, int64_t* n)
 
 int hea_init_random(hea_ctx* ctx, uint8_t* occ_dev, int64_t C, uint64_t seed, uint64_t chain0, void* cuda_stream)
 {
-    if (!ctx || !occ_dev) return fail(HEA_EINVAL, "ctx / occ_dev is NULL");
+    if (!ctx) return fail(HEA_EINVAL, "ctx is NULL");
     if (C < 0 || chain0 + (uint64_t)C > (1ull << 32)) return fail(HEA_EINVAL, "chain ids must be < 2^32");
     if (C == 0) return HEA_OK;
+    if (!occ_dev) return fail(HEA_EINVAL, "occ_dev is NULL");
     DeviceGuard guard(ctx->device);
     cudaError_t e = hea::launch_init_random(ctx->P, occ_dev, C, seed, chain0, ctx->d_nps, (cudaStream_t)cuda_stream,
                                             &ctx->n_launches);
@@ -304,9 +305,10 @@ int hea_init_random(hea_ctx* ctx, uint8_t* occ_dev, int64_t C, uint64_t seed, ui
 int hea_sro_full(hea_ctx* ctx, const uint8_t* occ_dev, int64_t B, int32_t* counts_dev, double* alpha_dev,
                  double* obj_dev, void* cuda_stream)
 {
-    if (!ctx || !occ_dev || !counts_dev) return fail(HEA_EINVAL, "ctx / occ_dev / counts_dev is NULL");
+    if (!ctx) return fail(HEA_EINVAL, "ctx is NULL");
     if (B < 0) return fail(HEA_EINVAL, "B must be >= 0");
-    if (B == 0) return HEA_OK;
+    if (B == 0) return HEA_OK;                      // empty batch: nothing is read or written, pointers may be NULL
+    if (!occ_dev || !counts_dev) return fail(HEA_EINVAL, "occ_dev / counts_dev is NULL");
     DeviceGuard guard(ctx->device);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = hea::launch_sro_count(ctx->P, occ_dev, B, counts_dev, ctx->n_sms, st, &ctx->n_launches);
@@ -317,9 +319,10 @@ int hea_sro_full(hea_ctx* ctx, const uint8_t* occ_dev, int64_t B, int32_t* count
 
 int hea_mc_stats_reset(hea_ctx* ctx, hea_mc_stats* stats_dev, int64_t C, void* cuda_stream)
 {
-    if (!ctx || !stats_dev) return fail(HEA_EINVAL, "ctx / stats_dev is NULL");
+    if (!ctx) return fail(HEA_EINVAL, "ctx is NULL");
     if (C < 0) return fail(HEA_EINVAL, "C must be >= 0");
     if (C == 0) return HEA_OK;
+    if (!stats_dev) return fail(HEA_EINVAL, "stats_dev is NULL");
     DeviceGuard guard(ctx->device);
     cudaError_t e = hea::launch_stats_reset(stats_dev, C, (cudaStream_t)cuda_stream, &ctx->n_launches);
     return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_mc_stats_reset launch");
@@ -331,7 +334,8 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
 {
     static_assert(sizeof(hea_mc_stats) == 40, "hea_mc_stats layout");
     static_assert(sizeof(hea_move) == 24, "hea_move layout");
-    if (!ctx || !occ_dev || !counts_dev || !stats_dev) return fail(HEA_EINVAL, "ctx / occ_dev / counts_dev / stats_dev is NULL");
+    if (!ctx) return fail(HEA_EINVAL, "ctx is NULL");
+    if (C != 0 && (!occ_dev || !counts_dev || !stats_dev)) return fail(HEA_EINVAL, "occ_dev / counts_dev / stats_dev is NULL");
     if (K < 1 || K > HEA_MAX_K) return fail(HEA_EINVAL, "K must be in [1, 1024]");
     if (C < 0 || chain0 + (uint64_t)C > (1ull << 32)) return fail(HEA_EINVAL, "chain ids must be < 2^32");
     if (log_cap < 0 || (log_cap > 0 && !log_dev)) return fail(HEA_EINVAL, "log_cap > 0 needs log_dev");
