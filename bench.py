@@ -327,7 +327,7 @@ def main():
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "achieved": mc_rate_1gpu * ops / 1e12, "peak": alu_peak,
                      "unit": "T thread-instr/s", "frac": mc_rate_1gpu * ops / 1e12 / alu_peak, "traffic": None,
-                     "kernel": "mc_chain_kernel", "ops_per_trial": ops, "ms_per_launch": 1e3 * t_mc / args.steps,
+                     "kernel": "mc_window_kernel", "ops_per_trial": ops, "ms_per_launch": 1e3 * t_mc / args.steps,
                      "peak_source": f"{n_sms} SMs x 128 lanes/clk x {sm_max_mhz:.0f} MHz (DESIGN.md section 6)"},
     }
     if recount:

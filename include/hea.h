@@ -23,6 +23,7 @@
  *   - Site order (D1): site = ((x*Ly + y)*Lz + z)*A + b with basis fcc A=4 (0,0,0),(0,1,1),(1,0,1),(1,1,0),
  *     bcc A=2 (0,0,0),(1,1,1) in units of a/2.  Shells (D2): fcc |o|^2 = 2,4,6 (z = 12,6,24), bcc 3,4,8 (z = 8,6,12),
  *     offsets in lexicographic order, periodic; tiny cells keep exactly z_s table entries (multi-edge semantics).
+ *   - Empty batches (B == 0 / C == 0) return HEA_OK without touching the buffers (their pointers may be NULL).
  *   - There is no CPU fallback: without a CUDA device every compute call returns HEA_ECUDA.
  */
 #ifndef HEA_H
@@ -91,12 +92,11 @@ int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host);
 
 /*
  * Tuning knobs (never change results).  name:
- *   "mc_lanes"        lanes cooperating on one candidate: 0 = auto, else 1,2,4,8,16,32
  *   "mc_occ_mode"     0 = auto, 1 = shared uint8, 2 = shared 4-bit packed, 3 = global memory (through L2)
- *   "mc_threads"      threads per chain block: 0 = auto, else a multiple of 32 in [32, 1024]
- *   "mc_cluster"      CTAs per chain (thread-block cluster, replicated occupancy): 0 = auto, 1, 2, 4, 8
- *   "mc_neighbors"    0 = auto, 1 = neighbour table, 2 = computed from the lattice stencil
- *   "sro_variant"     0 = auto, 1 = direct table gather, 2 = shared-memory staged table tiles
+ *   "mc_threads"      threads per block: 0 = auto, else a multiple of 32 in [32, 1024]
+ *   "mc_cluster"      blocks per chain (thread-block cluster, replicated chain state): 0 = auto, 1, 2, 4, 8
+ *   "mc_window"       cap on the speculative step window (steps evaluated against one configuration before the
+ *                     lowest improving (step, k) is applied): 0 = auto, 1 = strictly step by step, up to 2^20
  * Unknown name or value -> HEA_EINVAL.
  */
 int hea_set_option(hea_ctx* ctx, const char* name, int64_t value);

@@ -21,9 +21,9 @@ cudaError_t launch_stats_reset(void* stats, int64_t C, cudaStream_t st, int64_t*
 cudaError_t launch_transpose_table(const int32_t* site_major, int32_t* slot_major, int N, int Npad, int Z,
                                    cudaStream_t st, int64_t* n_launches);
 size_t mc_shared_bytes(int occ_mode, int N);
-cudaError_t launch_mc(const KParams& P, int lanes, int occ_mode, int threads, uint8_t* occ, int32_t* counts,
-                      int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0, uint64_t step0,
-                      void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches);
+cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode, int threads, int cluster, int w_max,
+                      uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
+                      uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches);
 }  // namespace hea
 
 struct hea_ctx {
@@ -36,10 +36,11 @@ struct hea_ctx {
     int32_t* d_nbr_site = nullptr;
     int32_t* d_nbr_slot = nullptr;
     hea::DevTables* d_tab = nullptr;
+    hea::DevTables tab_host{};
     int64_t* d_nps = nullptr;
     hea::KParams P{};
     // tuning options (0 = auto)
-    int64_t opt_lanes = 0, opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_neighbors = 0, opt_sro_variant = 0;
+    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0;
     int64_t n_launches = 0;
     // internal stream and scratch for the *_host entry points
     cudaStream_t stream = nullptr;
@@ -92,24 +93,20 @@ int ensure_scratch(hea_ctx* ctx, int slot, size_t bytes)
 int64_t* option_slot(hea_ctx* ctx, const char* name)
 {
     if (!name) return nullptr;
-    if (!strcmp(name, "mc_lanes")) return &ctx->opt_lanes;
     if (!strcmp(name, "mc_occ_mode")) return &ctx->opt_occ_mode;
     if (!strcmp(name, "mc_threads")) return &ctx->opt_threads;
     if (!strcmp(name, "mc_cluster")) return &ctx->opt_cluster;
-    if (!strcmp(name, "mc_neighbors")) return &ctx->opt_neighbors;
-    if (!strcmp(name, "sro_variant")) return &ctx->opt_sro_variant;
+    if (!strcmp(name, "mc_window")) return &ctx->opt_window;
     return nullptr;
 }
 
 bool option_value_ok(const char* name, int64_t v)
 {
     if (v == 0) return true;
-    if (!strcmp(name, "mc_lanes")) return v == 1 || v == 2 || v == 4 || v == 8 || v == 16 || v == 32;
     if (!strcmp(name, "mc_occ_mode")) return v >= 1 && v <= 3;
     if (!strcmp(name, "mc_threads")) return v >= 32 && v <= 1024 && v % 32 == 0;
     if (!strcmp(name, "mc_cluster")) return v == 1 || v == 2 || v == 4 || v == 8;
-    if (!strcmp(name, "mc_neighbors")) return v == 1 || v == 2;
-    if (!strcmp(name, "sro_variant")) return v == 1 || v == 2;
+    if (!strcmp(name, "mc_window")) return v >= 1 && v <= (1 << 20);
     return false;
 }
 
@@ -227,6 +224,7 @@ int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz, int n_species
     P.nbr_site = ctx->d_nbr_site;
     P.nbr_slot = ctx->d_nbr_slot;
     P.tab = ctx->d_tab;
+    ctx->tab_host = tab[0];
     *out = ctx;
     return HEA_OK;
 }
@@ -354,20 +352,26 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
     } else if (hea::mc_shared_bytes(occ_mode, N) > budget) {
         return fail(HEA_EINVAL, "mc_occ_mode does not fit in shared memory for this N");
     }
-    int lanes = (int)ctx->opt_lanes;
-    if (lanes == 0) {
-        const int64_t total = (int64_t)C * K;
-        lanes = floor_pow2(std::max<int64_t>(1, (int64_t)ctx->n_sms * 2048 / std::max<int64_t>(1, total)));
-        lanes = std::min(lanes, 32);
-        lanes = std::min(lanes, floor_pow2(std::max(1, 1024 / K)));
+    // blocks per chain: spread few chains over the SMs with thread-block clusters (replicated chain state)
+    int cluster = (int)ctx->opt_cluster;
+    if (cluster == 0) {
+        cluster = 1;
+        while (cluster < 8 && C * cluster * 2 <= ctx->n_sms) cluster *= 2;
     }
     int threads = (int)ctx->opt_threads;
     if (threads == 0) {
-        threads = (int)std::min<int64_t>(1024, (int64_t)K * lanes);
-        threads = (threads + 31) & ~31;
+        // 64 registers per thread -> 1024 resident threads per SM, shared between the blocks that land on one SM
+        const int64_t blocks_per_sm = (C * cluster + ctx->n_sms - 1) / ctx->n_sms;
+        threads = std::max(32, std::min(1024, floor_pow2(std::max<int64_t>(1, 1024 / blocks_per_sm))));
     }
-    cudaError_t e = hea::launch_mc(ctx->P, lanes, occ_mode, threads, occ_dev, counts_dev, C, n_steps, K, seed, chain0,
-                                   step0, stats_dev, log_dev, log_cap, (cudaStream_t)cuda_stream, &ctx->n_launches);
+    const int w_max = ctx->opt_window ? (int)ctx->opt_window : (1 << 20);
+    cudaError_t e = cudaErrorUnknown;
+    for (; cluster >= 1; cluster /= 2) {     // a cluster shape the device cannot place falls back to a smaller one
+        e = hea::launch_mc(ctx->P, ctx->tab_host, occ_mode, threads, cluster, w_max, occ_dev, counts_dev, C, n_steps, K,
+                           seed, chain0, step0, stats_dev, log_dev, log_cap, (cudaStream_t)cuda_stream, &ctx->n_launches);
+        if (e == cudaSuccess || ctx->opt_cluster != 0) break;
+        (void)cudaGetLastError();
+    }
     return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_mc_run launch");
 }
 

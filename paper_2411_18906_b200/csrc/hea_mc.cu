@@ -1,19 +1,29 @@
 // hea_mc.cu -- chain-parallel Monte Carlo local search (hea_mc_run).
-// DESIGN.md D6, D7, D9; Alg. 3, Eq. 4, Eq. 5, Eq. 6.
+// DESIGN.md D6, D7, D9 and section 5; Alg. 3, Eq. 4, Eq. 5, Eq. 6.
 //
-// One persistent launch runs all n_steps steps; no host round trip inside.  One thread block per chain.
-//   - the chain's configuration lives in shared memory (uint8, or 4-bit packed when that is what fits), else it is
-//     read through L1/L2 from global memory; counts, g, t, w live in shared memory;
-//   - a GROUP of G lanes (G = 1..32, a power of two) owns one candidate: all lanes derive the same Philox block
-//     (counter = step, k, chain), then split the 2Z neighbour entries of the two sites between them; each lane
-//     accumulates sum_{nbrs of b} e_r - sum_{nbrs of a} e_r as one packed 64-bit word per shell (8-bit fields,
-//     wrap-around arithmetic; a bias makes the fields non-negative after the group reduction by shuffles);
-//   - the S*M rows of the objective are split between the lanes of the group, then combined by shuffles in the
-//     fixed D6 order (rows i ascending within a shell, shells ascending), every operation individually rounded;
-//   - improving candidates post their index with a shared-memory atomicMin (triple-buffered so that a step without
-//     an accepted move needs ONE block barrier); the owning group applies the move.
-// Results are a function of (seed, chain, step) only: independent of G, block size and occupancy placement.
+// One persistent launch runs all n_steps steps of every chain; no host round trip inside.
+//
+// Mapping.  A chain is owned by one thread block, or by a thread-block CLUSTER of R blocks (R = 2, 4, 8) when there
+// are fewer chains than SMs; every block of a cluster keeps its own replica of the chain state (occupancy, pair
+// counts, J) in shared memory and all replicas apply the same moves.  One THREAD evaluates one candidate swap:
+// Philox block -> sites (a, b) -> species histograms of the neighbours of a and b as one packed word per shell
+// (8-bit fields, wrap-around arithmetic) -> J from counts + delta in the fixed D6 order (fp64, no FMA).
+//
+// Speculative step windows.  The steps of a chain depend on each other only through accepted moves, and D9 applies
+// the lowest-index improving candidate.  So a WINDOW of W consecutive steps (W*K candidates, ordered by (step, k))
+// is evaluated against the same configuration; the lowest improving (step, k) in the window is exactly the move D9
+// would apply first; it is applied, the steps after it are discarded and the next window starts at step + 1.
+// Without an accepted move the whole window is committed.  W adapts (doubles after a window without a move, falls
+// back to the observed gap after one), so the converged "reject regime" fills the machine while the early "accept
+// regime" wastes little.  The trajectory is identical to the step-by-step definition for every W, R and block size.
+//
+// Per window: one block barrier (+ one cluster barrier when R > 1: every block posts its local best move record into
+// every peer's shared memory through DSMEM, then all replicas apply the global minimum).
+#include <cooperative_groups.h>
+
 #include "hea_device.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace hea {
 
@@ -21,8 +31,9 @@ namespace {
 
 enum { OCC_SMEM_U8 = 1, OCC_SMEM_NIB = 2, OCC_GLOBAL = 3 };
 
-constexpr uint64_t kBias = 0x8080808080808080ULL;
-constexpr int kNoCandidate = 0x7FFFFFFF;
+constexpr uint32_t kNoKey = 0xFFFFFFFFu;     // "no improving candidate"; real keys are (window step << 10) | k
+constexpr int kMaxCluster = 8;
+constexpr int kMaxRounds = 8;                // candidates per thread per window when W > 1
 
 template <int OCC>
 struct OccView {
@@ -30,6 +41,7 @@ struct OccView {
     __device__ __forceinline__ uint32_t get(uint32_t i) const
     {
         if (OCC == OCC_SMEM_NIB) return (p[i >> 1] >> ((i & 1u) * 4u)) & 0xFu;
+        if (OCC == OCC_GLOBAL) return __ldcg(p + i);       // L2: coherent across the blocks of a cluster
         return p[i];
     }
     __device__ __forceinline__ void set(uint32_t i, uint32_t v) const
@@ -43,53 +55,92 @@ struct OccView {
     }
 };
 
+// The best move of one block in one window, posted to every replica.
+struct MoveRec {
+    uint32_t key;                 // (window step << 10) | k, kNoKey if none
+    uint32_t a, b, pq;            // sites; species p | q << 8
+    double J;
+    uint64_t d[3];                // packed neighbour-histogram differences per shell (biased 8-bit fields)
+};
+
 struct ChainShared {
-    double g[kSMM];
-    double t[kSMM];
-    double w[4];
     int cnt[kSMM];
     double J;
     unsigned long long n_accept, n_null, hash, last_accept, n_logged;
-    int best[3];
-    int pad;
+    uint32_t best[3];             // local minimum key, triple-buffered (one block barrier per window)
+    uint32_t pad;
+    MoveRec rec[2][kMaxCluster];  // [window parity][source block]
 };
+
+// Objective constants in kernel-parameter (constant-bank) space: operands of the fp64 instructions, no loads.
+template <int M>
+struct McConst {
+    double g[3 * M * M];
+    double t[3 * M * M];
+    double w[4];
+};
+
+struct McArgs {
+    uint8_t* occ_all;
+    int32_t* counts_all;
+    unsigned long long n_steps, seed, chain0, step0;
+    unsigned long long* stats_all;
+    unsigned long long* log_all;
+    long long log_cap;
+    int K;
+    int R;                        // blocks per chain (cluster size)
+    int w_max;                    // cap on the window length in steps (>= 1)
+};
+
+constexpr uint64_t kBias = 0x8080808080808080ULL;
 
 __device__ __forceinline__ int field8(uint64_t packed, int r) { return (int)((packed >> (8 * r)) & 0xFFu) - 128; }
 
-// dN[s][i][j] for a swap of species p (site a) and q (site b), given the biased packed word of shell s whose
-// field r is  #(nbrs of b with species r) - #(nbrs of a with species r)  (a, b themselves excluded):
-//   N[p][r] += d[r]; N[r][p] += d[r]; N[q][r] -= d[r]; N[r][q] -= d[r]
-__device__ __forceinline__ int delta_cell(uint64_t packed, int i, int j, int p, int q)
+// One shell's contribution  sum_i sum_j (1 - (N_ij + dN_ij) g_ij - t_ij)^2  in the D6 order.
+// dN[i][j] = ci*F[j] + cj*F[i], ci = [i==p] - [i==q], F[r] = #(nbrs of b of species r) - #(nbrs of a ...) (a, b excluded).
+template <int M>
+__device__ __forceinline__ double shell_sum(const int* __restrict__ cnt, const double* __restrict__ g,
+                                            const double* __restrict__ t, uint64_t dpacked, int p, int q)
 {
-    const int ci = (i == p) - (i == q);
-    const int cj = (j == p) - (j == q);
-    return ci * field8(packed, j) + cj * field8(packed, i);
+    int F[M], c[M];
+#pragma unroll
+    for (int r = 0; r < M; ++r) { F[r] = field8(dpacked, r); c[r] = (r == p) - (r == q); }
+    double sh = 0.0;
+#pragma unroll
+    for (int i = 0; i < M; ++i) {
+        double row = 0.0;
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            const int n = cnt[i * M + j] + c[i] * F[j] + c[j] * F[i];
+            row = __dadd_rn(row, sq_dev(n, g[i * M + j], t[i * M + j]));
+        }
+        sh = __dadd_rn(sh, row);
+    }
+    return sh;
 }
 
-template <int G, int OCC>
+template <int M, int OCC>
 __global__ void __launch_bounds__(1024)
-mc_chain_kernel(const KParams P, uint8_t* __restrict__ occ_all, int32_t* __restrict__ counts_all,
-                unsigned long long n_steps, int K, unsigned long long seed, unsigned long long chain0,
-                unsigned long long step0, unsigned long long* __restrict__ stats_all,
-                unsigned long long* __restrict__ log_all, long long log_cap)
+mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const McArgs A)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
     ChainShared& sh = *reinterpret_cast<ChainShared*>(s_raw);
     uint8_t* s_occ = s_raw + sizeof(ChainShared);
 
     const int tid = threadIdx.x, T = blockDim.x;
-    const int M = P.M, S = P.S, Z = P.Z, N = P.N;
-    const int SM = S * M, SMM = SM * M;
-    const size_t chain_local = blockIdx.x;
-    uint8_t* g_occ = occ_all + chain_local * (size_t)N;
-    int32_t* g_cnt = counts_all + chain_local * (size_t)SMM;
-    unsigned long long* g_stats = stats_all + chain_local * 5;
-    const uint32_t chain = (uint32_t)(chain0 + chain_local);
-    const uint32_t key0 = (uint32_t)seed, key1 = (uint32_t)(seed >> 32);
+    const int S = P.S, Z = P.Z, N = P.N, K = A.K, R = A.R;
+    constexpr int MM = M * M;
+    const int SMM = S * MM;
+    const uint32_t rank = R > 1 ? cg::this_cluster().block_rank() : 0u;
+    const size_t chain_local = blockIdx.x / (unsigned)R;
+    uint8_t* g_occ = A.occ_all + chain_local * (size_t)N;
+    int32_t* g_cnt = A.counts_all + chain_local * (size_t)SMM;
+    unsigned long long* g_stats = A.stats_all + chain_local * 5;
+    const uint32_t chain = (uint32_t)(A.chain0 + chain_local);
+    const uint32_t key0 = (uint32_t)A.seed, key1 = (uint32_t)(A.seed >> 32);
 
-    // ---- prologue: constants, counts, configuration -> shared memory
-    for (int i = tid; i < SMM; i += T) { sh.g[i] = P.tab->g[i]; sh.t[i] = P.tab->t[i]; sh.cnt[i] = g_cnt[i]; }
-    if (tid < 4) sh.w[tid] = P.tab->w[tid];
+    // ---- prologue: counts, configuration -> shared memory; J of the supplied counts (D6 order)
+    for (int i = tid; i < SMM; i += T) sh.cnt[i] = g_cnt[i];
     if (OCC == OCC_SMEM_U8) {
         for (int i = tid; i < N; i += T) s_occ[i] = g_occ[i];
     } else if (OCC == OCC_SMEM_NIB) {
@@ -100,49 +151,57 @@ mc_chain_kernel(const KParams P, uint8_t* __restrict__ occ_all, int32_t* __restr
     }
     if (tid == 0) {
         sh.n_accept = g_stats[0]; sh.n_null = 0; sh.hash = g_stats[2]; sh.last_accept = g_stats[3]; sh.n_logged = 0;
-        sh.best[0] = sh.best[1] = sh.best[2] = kNoCandidate;
+        sh.best[0] = sh.best[1] = sh.best[2] = kNoKey;
     }
+    if (tid < 2 * kMaxCluster) sh.rec[tid / kMaxCluster][tid % kMaxCluster].key = kNoKey;
     __syncthreads();
-    if (tid == 0) {       // J of the supplied counts, D6 order
+    if (tid == 0) {
         double J = 0.0;
-        for (int s = 0; s < S; ++s) {
-            double shs = 0.0;
-            for (int i = 0; i < M; ++i) {
-                double row = 0.0;
-                for (int j = 0; j < M; ++j) {
-                    const int idx = (s * M + i) * M + j;
-                    row = __dadd_rn(row, sq_dev(sh.cnt[idx], sh.g[idx], sh.t[idx]));
-                }
-                shs = __dadd_rn(shs, row);
-            }
-            J = __dadd_rn(J, __dmul_rn(sh.w[s], shs));
-        }
+        for (int s = 0; s < S; ++s)
+            J = __dadd_rn(J, __dmul_rn(Kc.w[s], shell_sum<M>(sh.cnt + s * MM, Kc.g + s * MM, Kc.t + s * MM, kBias, 0, 0)));
         sh.J = J;
     }
-    __syncthreads();
+    if (R > 1) cg::this_cluster().sync(); else __syncthreads();   // peers' shared memory is initialised before any post
 
     const OccView<OCC> occ{OCC == OCC_GLOBAL ? g_occ : s_occ};
-    const int gl = tid & (G - 1);                 // lane within the group
-    // shuffle mask = the lanes of this group (groups of one warp may be at different candidates)
-    const uint32_t gmask = G == 32 ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((tid & 31) & ~(G - 1)));
-    const int group = tid / G, n_groups = T / G;
-    const int z1 = P.zoff[1], z2 = P.zoff[2];
     const int32_t* __restrict__ nbr = P.nbr_site;
-    unsigned int my_null = 0;
+    const int zq0 = P.zoff[1] >> 1, zq1 = P.zoff[2] >> 1, zq2 = P.zoff[3] >> 1;   // shell boundaries in int2 units (z even)
 
-    for (unsigned long long it = 0; it < n_steps; ++it) {
-        const unsigned long long step = step0 + it;
-        const int buf = (int)(it % 3);
+    // this thread's candidates in a window: c = gtid + j*GT, j = 0, 1, ...; kept as (window step, k)
+    const uint32_t GT = (uint32_t)T * (uint32_t)R;
+    const uint32_t gtid = (uint32_t)tid * (uint32_t)R + rank;
+    const uint32_t ts_first = gtid / (uint32_t)K, k_first = gtid - ts_first * (uint32_t)K;
+    const uint32_t ts_inc = GT / (uint32_t)K, k_inc = GT - ts_inc * (uint32_t)K;
+    // window cap: at most kMaxRounds candidates per thread (W = 1 is always allowed: K <= 1024 <= 32 * 32)
+    uint32_t w_cap = (uint32_t)(((uint64_t)kMaxRounds * GT) / (uint32_t)K);
+    if (w_cap < 1u) w_cap = 1u;
+    if (w_cap > (uint32_t)A.w_max) w_cap = (uint32_t)A.w_max;
+    if (w_cap > (1u << 20)) w_cap = 1u << 20;
+
+    unsigned long long t0 = A.step0;
+    const unsigned long long t_end = A.step0 + A.n_steps;
+    uint32_t W = 1;
+    unsigned long long my_null = 0;
+    uint32_t it = 0;
+
+    while (t0 < t_end) {
+        const uint32_t Wc = (uint32_t)min((unsigned long long)W, t_end - t0);
+        const int buf = (int)(it % 3u);
+        volatile uint32_t* best_slot = &sh.best[buf];
         const double J_cur = sh.J;
-        // first improving candidate of this group (k ascending within the group's loop)
-        int win_k = kNoCandidate;
-        uint32_t win_a = 0, win_b = 0, win_p = 0, win_q = 0;
+        uint32_t win_key = kNoKey, win_a = 0, win_b = 0, win_pq = 0;
         uint64_t win_d0 = 0, win_d1 = 0, win_d2 = 0;
         double win_J = 0.0;
+        uint64_t nullmask = 0;
 
-        for (int k = group; k < K; k += n_groups) {
+        uint32_t ts = ts_first, k = k_first;
+        for (int j = 0; ts < Wc; ++j) {
+            const uint32_t hint = *best_slot;
+            if ((hint >> 10) < ts) break;                       // a move at an earlier step exists: this step is void
+            const uint32_t key = (ts << 10) | k;
             // ---- D9.1 proposal
-            const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), (uint32_t)k, chain, key0, key1);
+            const unsigned long long step = t0 + ts;
+            const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), k, chain, key0, key1);
             uint32_t a = __umulhi(r.x, (uint32_t)N), b = __umulhi(r.y, (uint32_t)N - 1u);
             b += (b >= a);
             uint32_t p = occ.get(a), q = occ.get(b);
@@ -150,145 +209,196 @@ mc_chain_kernel(const KParams P, uint8_t* __restrict__ occ_all, int32_t* __restr
                 a = __umulhi(r.z, (uint32_t)N); b = __umulhi(r.w, (uint32_t)N - 1u);
                 b += (b >= a);
                 p = occ.get(a); q = occ.get(b);
-                if (p == q) { my_null += (gl == 0); continue; }
             }
-            // ---- D9.2 integer delta: packed per-shell  sum_b - sum_a  over this lane's share of the 2Z entries
-            uint64_t d0 = 0, d1 = 0, d2 = 0;
-            for (int e = gl; e < 2 * Z; e += G) {
-                const bool second = e >= Z;
-                const int ee = second ? e - Z : e;
-                const uint32_t u = second ? b : a;
-                const uint32_t v = (uint32_t)__ldg(nbr + (size_t)u * Z + ee);
-                if (v != a && v != b) {
-                    const uint64_t one = 1ull << (8 * occ.get(v));
-                    const uint64_t val = second ? one : (0ull - one);
-                    if (ee < z1) d0 += val; else if (ee < z2) d1 += val; else d2 += val;
-                }
-            }
-            if (G > 1) {
-#pragma unroll
-                for (int off = G / 2; off >= 1; off >>= 1) {
-                    d0 += __shfl_xor_sync(gmask, d0, off, G);
-                    d1 += __shfl_xor_sync(gmask, d1, off, G);
-                    if (S > 2) d2 += __shfl_xor_sync(gmask, d2, off, G);
-                }
-            }
-            d0 += kBias; d1 += kBias; d2 += kBias;
-            // ---- D6 objective from counts + delta: rows split over the lanes, combined in fixed order
-            double Jk = 0.0, shell_sum = 0.0;
-            for (int base = 0; base < SM; base += G) {
-                const int row = base + gl;
-                double row_sum = 0.0;
-                if (row < SM) {
-                    const int s = row / M, i = row - s * M;
-                    const uint64_t d = s == 0 ? d0 : (s == 1 ? d1 : d2);
-                    const int idx0 = row * M;
-                    for (int j = 0; j < M; ++j) {
-                        const int n = sh.cnt[idx0 + j] + delta_cell(d, i, j, (int)p, (int)q);
-                        row_sum = __dadd_rn(row_sum, sq_dev(n, sh.g[idx0 + j], sh.t[idx0 + j]));
+            if (p == q) {
+                nullmask |= 1ull << j;
+            } else if (key < hint) {                             // same step, higher k than a known move: only nullness counts
+                // ---- D9.2 integer delta: per shell  sum_{nbrs of b} e_r - sum_{nbrs of a} e_r  (a, b excluded)
+                uint64_t d0 = 0, d1 = 0, d2 = 0;
+                const int2* __restrict__ ra = reinterpret_cast<const int2*>(nbr + (size_t)a * Z);
+                const int2* __restrict__ rb = reinterpret_cast<const int2*>(nbr + (size_t)b * Z);
+                auto shell = [&](int e0, int e1) {
+                    uint64_t d = 0;
+#pragma unroll 3
+                    for (int e = e0; e < e1; ++e) {
+                        const int2 va = __ldg(ra + e), vb = __ldg(rb + e);
+                        const uint32_t v0 = (uint32_t)va.x, v1 = (uint32_t)va.y, v2 = (uint32_t)vb.x, v3 = (uint32_t)vb.y;
+                        const uint64_t o0 = 1ull << (8 * occ.get(v0)), o1 = 1ull << (8 * occ.get(v1));
+                        const uint64_t o2 = 1ull << (8 * occ.get(v2)), o3 = 1ull << (8 * occ.get(v3));
+                        d -= (v0 != a && v0 != b) ? o0 : 0ull;
+                        d -= (v1 != a && v1 != b) ? o1 : 0ull;
+                        d += (v2 != a && v2 != b) ? o2 : 0ull;
+                        d += (v3 != a && v3 != b) ? o3 : 0ull;
                     }
-                }
-#pragma unroll
-                for (int l = 0; l < G; ++l) {
-                    const int rr = base + l;
-                    const double v = G > 1 ? __shfl_sync(gmask, row_sum, l, G) : row_sum;
-                    if (rr < SM) {
-                        shell_sum = __dadd_rn(shell_sum, v);
-                        const int s = rr / M;
-                        if (rr - s * M == M - 1) {
-                            Jk = __dadd_rn(Jk, __dmul_rn(sh.w[s], shell_sum));
-                            shell_sum = 0.0;
-                        }
-                    }
+                    return d + kBias;
+                };
+                d0 = shell(0, zq0);
+                if (S > 1) d1 = shell(zq0, zq1);
+                if (S > 2) d2 = shell(zq1, zq2);
+                // ---- D6 objective from counts + delta
+                double Jk = __dmul_rn(Kc.w[0], shell_sum<M>(sh.cnt, Kc.g, Kc.t, d0, (int)p, (int)q));
+                Jk = __dadd_rn(0.0, Jk);
+                if (S > 1) Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[1], shell_sum<M>(sh.cnt + MM, Kc.g + MM, Kc.t + MM, d1, (int)p, (int)q)));
+                if (S > 2) Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[2], shell_sum<M>(sh.cnt + 2 * MM, Kc.g + 2 * MM, Kc.t + 2 * MM, d2, (int)p, (int)q)));
+                if (Jk < J_cur && win_key == kNoKey) {
+                    win_key = key; win_a = a; win_b = b; win_pq = p | (q << 8);
+                    win_d0 = d0; win_d1 = d1; win_d2 = d2; win_J = Jk;
+                    atomicMin(&sh.best[buf], key);
                 }
             }
-            if (Jk < J_cur && win_k == kNoCandidate) {
-                win_k = k; win_a = a; win_b = b; win_p = p; win_q = q;
-                win_d0 = d0; win_d1 = d1; win_d2 = d2; win_J = Jk;
-                if (gl == 0) atomicMin(&sh.best[buf], k);
-            }
+            k += k_inc; ts += ts_inc;
+            if (k >= (uint32_t)K) { k -= (uint32_t)K; ++ts; }
         }
-        __syncthreads();                                   // B1: all candidates evaluated, minimum posted
-        const int k_best = sh.best[buf];
-        if (tid == 0) sh.best[(buf + 2) % 3] = kNoCandidate;   // next user of that slot is two barriers away
-        if (k_best != kNoCandidate) {
-            if (win_k == k_best) {                         // the owning group applies the move (D9.4)
-                for (int idx = gl; idx < SMM; idx += G) {
-                    const int s = idx / (M * M), rem = idx - s * M * M, i = rem / M, j = rem - i * M;
-                    const uint64_t d = s == 0 ? win_d0 : (s == 1 ? win_d1 : win_d2);
-                    sh.cnt[idx] += delta_cell(d, i, j, (int)win_p, (int)win_q);
-                }
-                if (gl == 0) {
-                    occ.set(win_a, win_q);
-                    occ.set(win_b, win_p);
-                    sh.J = win_J;
-                    sh.n_accept += 1;
-                    sh.last_accept = step;
-                    unsigned long long h = sh.hash;
-                    h = (h ^ (uint32_t)step) * 0x100000001b3ULL;
-                    h = (h ^ (uint32_t)(step >> 32)) * 0x100000001b3ULL;
-                    h = (h ^ (uint32_t)k_best) * 0x100000001b3ULL;
-                    h = (h ^ win_a) * 0x100000001b3ULL;
-                    h = (h ^ win_b) * 0x100000001b3ULL;
-                    sh.hash = h;
-                    const unsigned long long nl = sh.n_logged;
-                    if (log_all != nullptr && (long long)nl < log_cap) {
-                        unsigned long long* rec = log_all + (chain_local * (size_t)log_cap + nl) * 3;
-                        rec[0] = step;
-                        rec[1] = (unsigned long long)(uint32_t)k_best | ((unsigned long long)win_a << 32);
-                        rec[2] = (unsigned long long)win_b;
-                    }
-                    sh.n_logged = nl + 1;
+        __syncthreads();                                        // B1: window evaluated, local minimum posted
+        uint32_t key_best = sh.best[buf];
+        if (tid == 0) sh.best[(buf + 2) % 3] = kNoKey;          // next user of that slot is two barriers away
+
+        const int warp = tid >> 5, lane = tid & 31;
+        const MoveRec* mv = nullptr;                            // the move to apply (in this block's shared memory)
+        if (R > 1) {
+            // post this block's best record into every replica's rec[parity][rank], then pick the global minimum
+            const int par = (int)(it & 1u);
+            const uint32_t owner_lane_mask = __ballot_sync(0xFFFFFFFFu, win_key == key_best && key_best != kNoKey);
+            const bool poster = key_best != kNoKey ? owner_lane_mask != 0u : warp == 0;
+            if (poster) {
+                const int src = key_best != kNoKey ? __ffs((int)owner_lane_mask) - 1 : 0;
+                MoveRec m;
+                m.key = key_best;
+                m.a = __shfl_sync(0xFFFFFFFFu, win_a, src); m.b = __shfl_sync(0xFFFFFFFFu, win_b, src);
+                m.pq = __shfl_sync(0xFFFFFFFFu, win_pq, src); m.J = __shfl_sync(0xFFFFFFFFu, win_J, src);
+                m.d[0] = __shfl_sync(0xFFFFFFFFu, win_d0, src); m.d[1] = __shfl_sync(0xFFFFFFFFu, win_d1, src);
+                m.d[2] = __shfl_sync(0xFFFFFFFFu, win_d2, src);
+                if (lane < R) {
+                    MoveRec* dst = cg::this_cluster().map_shared_rank(&sh.rec[par][rank], lane);
+                    *dst = m;
                 }
             }
-            __syncthreads();                               // B2: the move is visible before the next step's reads
+            cg::this_cluster().sync();                          // release/acquire: all records visible in every replica
+            uint32_t kb = kNoKey; int src_rank = 0;
+            for (int r2 = 0; r2 < R; ++r2) {
+                const uint32_t kk = sh.rec[par][r2].key;
+                if (kk < kb) { kb = kk; src_rank = r2; }
+            }
+            key_best = kb;
+            mv = &sh.rec[par][src_rank];
+        } else if (key_best != kNoKey) {
+            // single block: the owner's warp copies the record to shared memory for the cooperative apply
+            const uint32_t owner_lane_mask = __ballot_sync(0xFFFFFFFFu, win_key == key_best);
+            if (owner_lane_mask != 0u && lane == __ffs((int)owner_lane_mask) - 1) {
+                MoveRec& m = sh.rec[0][0];
+                m.key = key_best; m.a = win_a; m.b = win_b; m.pq = win_pq; m.J = win_J;
+                m.d[0] = win_d0; m.d[1] = win_d1; m.d[2] = win_d2;
+            }
+            __syncthreads();
+            mv = &sh.rec[0][0];
         }
+
+        // ---- commit: null counts of the committed steps, then the move (D9.4)
+        const uint32_t steps_done = key_best != kNoKey ? (key_best >> 10) + 1u : Wc;
+        if (nullmask) {
+            const uint32_t lim = steps_done * (uint32_t)K;       // candidates c < lim are committed
+            const uint32_t n_comm = gtid < lim ? (lim - 1u - gtid) / GT + 1u : 0u;
+            my_null += __popcll(n_comm >= 64u ? nullmask : (nullmask & ((1ull << n_comm) - 1ull)));
+        }
+        if (key_best != kNoKey) {
+            const int p = (int)(mv->pq & 0xFFu), q = (int)(mv->pq >> 8);
+            for (int idx = tid; idx < SMM; idx += T) {
+                const int s = idx / MM, rem = idx - s * MM, i = rem / M, jj = rem - i * M;
+                const uint64_t d = mv->d[s];
+                const int ci = (i == p) - (i == q), cj = (jj == p) - (jj == q);
+                sh.cnt[idx] += ci * field8(d, jj) + cj * field8(d, i);
+            }
+            if (tid == T - 1) {                                 // one thread (not among the count updaters when T > SMM)
+                const uint32_t a = mv->a, b = mv->b, kk = key_best & 1023u;
+                const unsigned long long step = t0 + (key_best >> 10);
+                if (OCC != OCC_GLOBAL || rank == 0) { occ.set(a, (uint32_t)q); occ.set(b, (uint32_t)p); }
+                sh.J = mv->J;
+                sh.n_accept += 1;
+                sh.last_accept = step;
+                unsigned long long h = sh.hash;
+                h = (h ^ (uint32_t)step) * 0x100000001b3ULL;
+                h = (h ^ (uint32_t)(step >> 32)) * 0x100000001b3ULL;
+                h = (h ^ kk) * 0x100000001b3ULL;
+                h = (h ^ a) * 0x100000001b3ULL;
+                h = (h ^ b) * 0x100000001b3ULL;
+                sh.hash = h;
+                const unsigned long long nl = sh.n_logged;
+                if (rank == 0 && A.log_all != nullptr && (long long)nl < A.log_cap) {
+                    unsigned long long* rec = A.log_all + (chain_local * (size_t)A.log_cap + nl) * 3;
+                    rec[0] = step;
+                    rec[1] = (unsigned long long)kk | ((unsigned long long)a << 32);
+                    rec[2] = (unsigned long long)b;
+                }
+                sh.n_logged = nl + 1;
+            }
+            // the move must be visible before the next window's reads; with a global occupancy shared by a cluster
+            // the writer is rank 0, so the whole cluster waits
+            if (OCC == OCC_GLOBAL && R > 1) cg::this_cluster().sync(); else __syncthreads();
+            W = min(steps_done, w_cap);                         // the observed gap
+        } else {
+            W = min(W * 2u, w_cap);
+        }
+        t0 += steps_done;
+        ++it;
     }
 
-    // ---- epilogue: write back
-    if (my_null) atomicAdd(&sh.n_null, (unsigned long long)my_null);
+    // ---- epilogue: write back (rank 0 owns the global copy; null counts are summed over the blocks)
+    if (my_null) atomicAdd(&sh.n_null, my_null);
     __syncthreads();
-    if (OCC == OCC_SMEM_U8) {
-        for (int i = tid; i < N; i += T) g_occ[i] = s_occ[i];
-    } else if (OCC == OCC_SMEM_NIB) {
-        for (int i = tid; i < N; i += T) g_occ[i] = (uint8_t)occ.get(i);
+    if (rank == 0) {
+        if (OCC == OCC_SMEM_U8) {
+            for (int i = tid; i < N; i += T) g_occ[i] = s_occ[i];
+        } else if (OCC == OCC_SMEM_NIB) {
+            for (int i = tid; i < N; i += T) g_occ[i] = (uint8_t)occ.get(i);
+        }
+        for (int i = tid; i < SMM; i += T) g_cnt[i] = sh.cnt[i];
+        if (tid == 0) {
+            g_stats[0] = sh.n_accept;
+            g_stats[2] = sh.hash;
+            g_stats[3] = sh.last_accept;
+            g_stats[4] = (unsigned long long)__double_as_longlong(sh.J);
+        }
     }
-    for (int i = tid; i < SMM; i += T) g_cnt[i] = sh.cnt[i];
-    if (tid == 0) {
-        g_stats[0] = sh.n_accept;
-        g_stats[1] += sh.n_null;
-        g_stats[2] = sh.hash;
-        g_stats[3] = sh.last_accept;
-        g_stats[4] = (unsigned long long)__double_as_longlong(sh.J);
-    }
+    if (tid == 0 && sh.n_null) atomicAdd(&g_stats[1], sh.n_null);
 }
 
-template <int G, int OCC>
-cudaError_t launch_one(const KParams& P, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K,
-                       uint64_t seed, uint64_t chain0, uint64_t step0, void* stats, void* log, int64_t log_cap,
+template <int M, int OCC>
+cudaError_t launch_one(const KParams& P, const DevTables& host_tab, const McArgs& A, int64_t C, int threads,
+                       size_t smem, cudaStream_t st)
+{
+    McConst<M> Kc;
+    for (int s = 0; s < 3; ++s)
+        for (int i = 0; i < M * M; ++i) {
+            Kc.g[s * M * M + i] = s < P.S ? host_tab.g[s * M * M + i] : 0.0;
+            Kc.t[s * M * M + i] = s < P.S ? host_tab.t[s * M * M + i] : 0.0;
+        }
+    for (int s = 0; s < 4; ++s) Kc.w[s] = host_tab.w[s];
+    auto kern = mc_window_kernel<M, OCC>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(C * A.R));
+    cfg.blockDim = dim3((unsigned)threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)A.R;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, P, Kc, A);
+}
+
+template <int M>
+cudaError_t launch_occ(int occ_mode, const KParams& P, const DevTables& host_tab, const McArgs& A, int64_t C,
                        int threads, size_t smem, cudaStream_t st)
 {
-    cudaError_t e = cudaFuncSetAttribute(mc_chain_kernel<G, OCC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    mc_chain_kernel<G, OCC><<<(unsigned)C, threads, smem, st>>>(
-        P, occ, counts, (unsigned long long)n_steps, K, (unsigned long long)seed, (unsigned long long)chain0,
-        (unsigned long long)step0, reinterpret_cast<unsigned long long*>(stats),
-        reinterpret_cast<unsigned long long*>(log), (long long)log_cap);
-    return cudaGetLastError();
-}
-
-template <int G>
-cudaError_t launch_occ(int occ_mode, const KParams& P, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps,
-                       int K, uint64_t seed, uint64_t chain0, uint64_t step0, void* stats, void* log,
-                       int64_t log_cap, int threads, size_t smem, cudaStream_t st)
-{
     switch (occ_mode) {
-        case OCC_SMEM_U8:
-            return launch_one<G, OCC_SMEM_U8>(P, occ, counts, C, n_steps, K, seed, chain0, step0, stats, log, log_cap, threads, smem, st);
-        case OCC_SMEM_NIB:
-            return launch_one<G, OCC_SMEM_NIB>(P, occ, counts, C, n_steps, K, seed, chain0, step0, stats, log, log_cap, threads, smem, st);
-        default:
-            return launch_one<G, OCC_GLOBAL>(P, occ, counts, C, n_steps, K, seed, chain0, step0, stats, log, log_cap, threads, smem, st);
+        case OCC_SMEM_U8: return launch_one<M, OCC_SMEM_U8>(P, host_tab, A, C, threads, smem, st);
+        case OCC_SMEM_NIB: return launch_one<M, OCC_SMEM_NIB>(P, host_tab, A, C, threads, smem, st);
+        default: return launch_one<M, OCC_GLOBAL>(P, host_tab, A, C, threads, smem, st);
     }
 }
 
@@ -302,23 +412,28 @@ size_t mc_shared_bytes(int occ_mode, int N)
     return (s + 15) & ~(size_t)15;
 }
 
-cudaError_t launch_mc(const KParams& P, int lanes, int occ_mode, int threads, uint8_t* occ, int32_t* counts,
-                      int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0, uint64_t step0,
-                      void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches)
+cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode, int threads, int cluster, int w_max,
+                      uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
+                      uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches)
 {
     const size_t smem = mc_shared_bytes(occ_mode, P.N);
+    McArgs A;
+    A.occ_all = occ; A.counts_all = counts;
+    A.n_steps = n_steps; A.seed = seed; A.chain0 = chain0; A.step0 = step0;
+    A.stats_all = reinterpret_cast<unsigned long long*>(stats);
+    A.log_all = reinterpret_cast<unsigned long long*>(log);
+    A.log_cap = log_cap; A.K = K; A.R = cluster; A.w_max = w_max;
     cudaError_t e;
-#define HEA_MC_CASE(GG) \
-    case GG: e = launch_occ<GG>(occ_mode, P, occ, counts, C, n_steps, K, seed, chain0, step0, stats, log, log_cap, threads, smem, st); break;
-    switch (lanes) {
-        HEA_MC_CASE(1)
-        HEA_MC_CASE(2)
-        HEA_MC_CASE(4)
-        HEA_MC_CASE(8)
-        HEA_MC_CASE(16)
-        default: e = launch_occ<32>(occ_mode, P, occ, counts, C, n_steps, K, seed, chain0, step0, stats, log, log_cap, threads, smem, st); break;
+    switch (P.M) {
+        case 1: e = launch_occ<1>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
+        case 2: e = launch_occ<2>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
+        case 3: e = launch_occ<3>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
+        case 4: e = launch_occ<4>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
+        case 5: e = launch_occ<5>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
+        case 6: e = launch_occ<6>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
+        case 7: e = launch_occ<7>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
+        default: e = launch_occ<8>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
     }
-#undef HEA_MC_CASE
     if (e == cudaSuccess) ++*n_launches;
     return e;
 }

@@ -121,12 +121,23 @@ def run_both(hb, w, n_chains, n_steps, log_cap=16, chain0=0, step0=0, opts=None,
     return o_stats
 
 
-@pytest.mark.parametrize("lanes", [1, 2, 4, 8, 16, 32])
+@pytest.mark.parametrize("cluster", [1, 2, 4, 8])
+@pytest.mark.parametrize("window", [0, 1, 3, 64])
 @pytest.mark.parametrize("occ_mode", [1, 2, 3])
-def test_mc_parity_all_launch_variants(hb, lanes, occ_mode):
-    w = small("fcc", (4, 4, 4), [0.2, 0.2, 0.2, 0.4], 3, target_seed=5, K=24, n_steps=120)
-    st = run_both(hb, w, 5, 120, opts={"mc_lanes": lanes, "mc_occ_mode": occ_mode})
+def test_mc_parity_all_launch_variants(hb, cluster, window, occ_mode):
+    # results never depend on the launch shape: blocks per chain, speculative window cap, occupancy placement
+    w = small("fcc", (4, 4, 4), [0.2, 0.2, 0.2, 0.4], 3, target_seed=5, K=24, n_steps=400)
+    st = run_both(hb, w, 5, 400, opts={"mc_cluster": cluster, "mc_window": window, "mc_occ_mode": occ_mode})
     assert st["n_accept"].sum() > 50
+
+
+@pytest.mark.parametrize("threads", [32, 64, 256, 1024])
+@pytest.mark.parametrize("cluster", [1, 4])
+def test_mc_parity_block_sizes_reject_regime(hb, threads, cluster):
+    # target 0 on a small cell converges quickly: long windows without a move, then rare moves inside windows
+    w = small("bcc", (6, 6, 6), [0.25] * 4, 3, K=32, n_steps=3000)
+    st = run_both(hb, w, 3, 3000, log_cap=256, opts={"mc_threads": threads, "mc_cluster": cluster})
+    assert (st["n_accept"] > 20).all()
 
 
 @pytest.mark.parametrize("lattice,dims,conc,S", LATTICES[:9])
@@ -166,7 +177,7 @@ def test_mc_c4_prefix(hb):
 
 def test_mc_c4_global_occupancy_path(hb):
     w = wl.config(4)
-    run_both(hb, w, 2, 100, opts={"mc_occ_mode": 3, "mc_lanes": 32})
+    run_both(hb, w, 2, 100, opts={"mc_occ_mode": 3, "mc_cluster": 8})
 
 
 def test_mc_split_run_and_chain_offset(hb):
@@ -181,7 +192,8 @@ def test_mc_split_run_and_chain_offset(hb):
     st_s, _ = h.mc_run(occ_s, cnt_s, 250, w.K, w.seed, step0=150, stats=st_s)
     assert (occ == occ_s).all() and (cnt == cnt_s).all() and (st == st_s).all()
     occ_c, cnt_c = occ0[2:].clone(), cnt0[2:].clone()
-    h.set_option("mc_lanes", 4)
+    h.set_option("mc_cluster", 4)
+    h.set_option("mc_threads", 64)
     st_c, _ = h.mc_run(occ_c, cnt_c, 400, w.K, w.seed, chain0=2)
     assert (occ[2:] == occ_c).all() and (st[2:] == st_c).all()
 
@@ -217,7 +229,7 @@ def test_argument_errors(hb):
     with pytest.raises(hb.HeaError):
         h.mc_run(occ, counts, 1, 2000, 1)
     with pytest.raises(hb.HeaError):
-        h.set_option("mc_lanes", 3)
+        h.set_option("mc_cluster", 3)
     with pytest.raises(hb.HeaError):
         h.set_option("nonsense", 1)
     with pytest.raises(hb.HeaError) as e:
