@@ -173,6 +173,8 @@ def main():
     ap.add_argument("--recount-L", type=int, default=100, help="fcc L^3 cells of the recount roofline point")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-recount", action="store_true")
+    ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config 1..4 (default 4 = the metric's)")
+    ap.add_argument("--chains", type=int, default=0, help="override the chain count (exploration only)")
     ap.add_argument("--opt", action="append", default=[], help="tuning option name=value (hea_set_option)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
@@ -195,7 +197,7 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
     hbm_peak, sm_max_mhz, peak_src = load_peaks()
 
-    w = workloads.config(4)
+    w = workloads.config(args.workload) if not args.chains else workloads.config(args.workload, n_chains=args.chains)
     h = binding.Hea(*w.create_args(), device=local_rank)
     for kv in args.opt:
         k, v = kv.split("=")
@@ -330,6 +332,8 @@ def main():
                      "kernel": "mc_window_kernel", "ops_per_trial": ops, "ms_per_launch": 1e3 * t_mc / args.steps,
                      "peak_source": f"{n_sms} SMs x 128 lanes/clk x {sm_max_mhz:.0f} MHz (DESIGN.md section 6)"},
     }
+    if args.workload != 4 or args.chains:
+        line["config"]["workload"] = f"EXPLORATION (not the metric's workload): {w.name}, {C} chains, K={K}, N={N}"
     if recount:
         line["recount_roofline"] = recount
     if rank == 0:

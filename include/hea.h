@@ -94,9 +94,10 @@ int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host);
  * Tuning knobs (never change results).  name:
  *   "mc_occ_mode"     0 = auto, 1 = shared uint8, 2 = shared 4-bit packed, 3 = global memory (through L2)
  *   "mc_threads"      threads per block: 0 = auto, else a multiple of 32 in [32, 1024]
- *   "mc_cluster"      blocks per chain (thread-block cluster, replicated chain state): 0 = auto, 1, 2, 4, 8
+ *   "mc_cluster"      blocks per chain (thread-block cluster, replicated chain state): 0 = auto, 1..8
  *   "mc_window"       cap on the speculative step window (steps evaluated against one configuration before the
  *                     lowest improving (step, k) is applied): 0 = auto, 1 = strictly step by step, up to 2^20
+ *   "mc_neighbors"    0 = auto, 1 = always the neighbour table, 2 = interior sites use site + offset (no table load)
  * Unknown name or value -> HEA_EINVAL.
  */
 int hea_set_option(hea_ctx* ctx, const char* name, int64_t value);

@@ -20,10 +20,11 @@ cudaError_t launch_init_random(const KParams& P, uint8_t* occ, int64_t C, uint64
 cudaError_t launch_stats_reset(void* stats, int64_t C, cudaStream_t st, int64_t* n_launches);
 cudaError_t launch_transpose_table(const int32_t* site_major, int32_t* slot_major, int N, int Npad, int Z,
                                    cudaStream_t st, int64_t* n_launches);
-size_t mc_shared_bytes(int occ_mode, int N);
+size_t mc_shared_bytes(int occ_mode, int N, int AZ, bool fast_nbr);
 cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode, int threads, int cluster, int w_max,
-                      uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
-                      uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches);
+                      bool fast_nbr, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
+                      uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches,
+                      int* query_max_clusters);
 }  // namespace hea
 
 struct hea_ctx {
@@ -40,7 +41,7 @@ struct hea_ctx {
     int64_t* d_nps = nullptr;
     hea::KParams P{};
     // tuning options (0 = auto)
-    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0;
+    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0, opt_neighbors = 0;
     int64_t n_launches = 0;
     // internal stream and scratch for the *_host entry points
     cudaStream_t stream = nullptr;
@@ -97,6 +98,7 @@ int64_t* option_slot(hea_ctx* ctx, const char* name)
     if (!strcmp(name, "mc_threads")) return &ctx->opt_threads;
     if (!strcmp(name, "mc_cluster")) return &ctx->opt_cluster;
     if (!strcmp(name, "mc_window")) return &ctx->opt_window;
+    if (!strcmp(name, "mc_neighbors")) return &ctx->opt_neighbors;
     return nullptr;
 }
 
@@ -105,8 +107,9 @@ bool option_value_ok(const char* name, int64_t v)
     if (v == 0) return true;
     if (!strcmp(name, "mc_occ_mode")) return v >= 1 && v <= 3;
     if (!strcmp(name, "mc_threads")) return v >= 32 && v <= 1024 && v % 32 == 0;
-    if (!strcmp(name, "mc_cluster")) return v == 1 || v == 2 || v == 4 || v == 8;
+    if (!strcmp(name, "mc_cluster")) return v >= 1 && v <= 8;
     if (!strcmp(name, "mc_window")) return v >= 1 && v <= (1 << 20);
+    if (!strcmp(name, "mc_neighbors")) return v == 1 || v == 2;
     return false;
 }
 
@@ -221,6 +224,14 @@ int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz, int n_species
     for (int d = 0; d < 3; ++d) P.L[d] = lat.L[d];
     for (int s = 0; s < 3; ++s) P.z[s] = s < S ? lat.z[s] : 0;
     for (int s = 0; s < 4; ++s) P.zoff[s] = s <= S ? lat.zoff[s] : Z;
+    for (int sh = 0; sh < 3; ++sh) {
+        P.m_self[sh] = 0;
+        if (sh < S)
+            for (int k = lat.zoff[sh]; k < lat.zoff[sh + 1]; ++k) {
+                const hea::StencilEntry& st = lat.stencil[0][k];
+                if (st.nb == 0 && st.sx % lat.L[0] == 0 && st.sy % lat.L[1] == 0 && st.sz % lat.L[2] == 0) ++P.m_self[sh];
+            }
+    }
     P.nbr_site = ctx->d_nbr_site;
     P.nbr_slot = ctx->d_nbr_slot;
     P.tab = ctx->d_tab;
@@ -345,33 +356,42 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
     // ---- launch configuration (results never depend on it)
     int occ_mode = (int)ctx->opt_occ_mode;
     const size_t budget = ctx->smem_optin;
+    const int AZ = ctx->P.A * ctx->P.Z;
+    const bool fast_nbr = ctx->opt_neighbors != 1;      // interior sites: neighbour = site + offset (no table load)
     if (occ_mode == 0) {
-        if (hea::mc_shared_bytes(1, N) <= budget) occ_mode = 1;
-        else if (hea::mc_shared_bytes(2, N) <= budget) occ_mode = 2;
+        if (hea::mc_shared_bytes(1, N, AZ, fast_nbr) <= budget) occ_mode = 1;
+        else if (hea::mc_shared_bytes(2, N, AZ, fast_nbr) <= budget) occ_mode = 2;
         else occ_mode = 3;
-    } else if (hea::mc_shared_bytes(occ_mode, N) > budget) {
+    } else if (hea::mc_shared_bytes(occ_mode, N, AZ, fast_nbr) > budget) {
         return fail(HEA_EINVAL, "mc_occ_mode does not fit in shared memory for this N");
     }
-    // blocks per chain: spread few chains over the SMs with thread-block clusters (replicated chain state)
+    // blocks per chain: spread few chains over the SMs with thread-block clusters (replicated chain state); the
+    // largest cluster size for which all C clusters are resident at once (GPC boundaries limit this: 16 clusters of 8
+    // do not fit on the 148 SMs of a B200, 16 of 7 do)
+    const int w_max = ctx->opt_window ? (int)ctx->opt_window : (1 << 20);
+    auto pick_threads = [&](int cl) {
+        if (ctx->opt_threads) return (int)ctx->opt_threads;
+        // 64 registers per thread -> 1024 resident threads per SM, shared between the blocks that land on one SM
+        const int64_t blocks_per_sm = (C * cl + ctx->n_sms - 1) / ctx->n_sms;
+        return std::max(32, std::min(1024, floor_pow2(std::max<int64_t>(1, 1024 / blocks_per_sm))));
+    };
+    cudaStream_t st = (cudaStream_t)cuda_stream;
     int cluster = (int)ctx->opt_cluster;
     if (cluster == 0) {
         cluster = 1;
-        while (cluster < 8 && C * cluster * 2 <= ctx->n_sms) cluster *= 2;
+        for (int cl = 8; cl >= 2; --cl) {
+            if (C * cl > ctx->n_sms) continue;
+            int fit = 0;
+            cudaError_t q = hea::launch_mc(ctx->P, ctx->tab_host, occ_mode, pick_threads(cl), cl, w_max, fast_nbr, occ_dev,
+                                           counts_dev, C, n_steps, K, seed, chain0, step0, stats_dev, log_dev, log_cap, st,
+                                           &ctx->n_launches, &fit);
+            if (q != cudaSuccess) { (void)cudaGetLastError(); continue; }
+            if (fit >= C) { cluster = cl; break; }
+        }
     }
-    int threads = (int)ctx->opt_threads;
-    if (threads == 0) {
-        // 64 registers per thread -> 1024 resident threads per SM, shared between the blocks that land on one SM
-        const int64_t blocks_per_sm = (C * cluster + ctx->n_sms - 1) / ctx->n_sms;
-        threads = std::max(32, std::min(1024, floor_pow2(std::max<int64_t>(1, 1024 / blocks_per_sm))));
-    }
-    const int w_max = ctx->opt_window ? (int)ctx->opt_window : (1 << 20);
-    cudaError_t e = cudaErrorUnknown;
-    for (; cluster >= 1; cluster /= 2) {     // a cluster shape the device cannot place falls back to a smaller one
-        e = hea::launch_mc(ctx->P, ctx->tab_host, occ_mode, threads, cluster, w_max, occ_dev, counts_dev, C, n_steps, K,
-                           seed, chain0, step0, stats_dev, log_dev, log_cap, (cudaStream_t)cuda_stream, &ctx->n_launches);
-        if (e == cudaSuccess || ctx->opt_cluster != 0) break;
-        (void)cudaGetLastError();
-    }
+    cudaError_t e = hea::launch_mc(ctx->P, ctx->tab_host, occ_mode, pick_threads(cluster), cluster, w_max, fast_nbr, occ_dev,
+                                   counts_dev, C, n_steps, K, seed, chain0, step0, stats_dev, log_dev, log_cap, st,
+                                   &ctx->n_launches, nullptr);
     return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_mc_run launch");
 }
 

@@ -24,6 +24,7 @@ struct KParams {
     int L[3];
     int z[3];
     int zoff[4];
+    int m_self[3];                        // per shell: table entries of a site that are the site itself (0 unless a tiny cell)
     const int32_t* nbr_site;              // [N][Z]   site-major: the Z neighbours of one site are contiguous
     const int32_t* nbr_slot;              // [Z][Npad] slot-major: one slot of consecutive sites is contiguous
     const DevTables* tab;
@@ -49,10 +50,17 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
+// Exact int32 -> double without the conversion (XU) pipe: 2^52 + 2^31 + n is exactly representable, so the mantissa
+// can be written directly and the constant subtracted exactly.  Bit-identical to (double)n for every int32.
+__device__ __forceinline__ double i2d_exact(int n)
+{
+    return __dsub_rn(__hiloint2double(0x43300000, (int)((unsigned)n ^ 0x80000000u)), 4503601774854144.0);
+}
+
 // D6: one squared deviation, every operation individually rounded (no FMA contraction).
 __device__ __forceinline__ double sq_dev(int n, double g, double t)
 {
-    const double x = __dmul_rn((double)n, g);
+    const double x = __dmul_rn(i2d_exact(n), g);
     const double al = __dsub_rn(1.0, x);
     const double d = __dsub_rn(al, t);
     return __dmul_rn(d, d);

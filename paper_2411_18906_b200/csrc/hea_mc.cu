@@ -21,6 +21,8 @@
 // every peer's shared memory through DSMEM, then all replicas apply the global minimum).
 #include <cooperative_groups.h>
 
+#include <type_traits>
+
 #include "hea_device.cuh"
 
 namespace cg = cooperative_groups;
@@ -60,7 +62,7 @@ struct MoveRec {
     uint32_t key;                 // (window step << 10) | k, kNoKey if none
     uint32_t a, b, pq;            // sites; species p | q << 8
     double J;
-    uint64_t d[3];                // packed neighbour-histogram differences per shell (biased 8-bit fields)
+    uint64_t d[3];                // packed neighbour-histogram differences per shell (Pack<M>::W, biased fields)
 };
 
 struct ChainShared {
@@ -90,21 +92,37 @@ struct McArgs {
     int K;
     int R;                        // blocks per chain (cluster size)
     int w_max;                    // cap on the window length in steps (>= 1)
+    int fast_nbr;                 // 1: interior sites take neighbours as site + offset (shared-memory stencil), no table load
 };
 
-constexpr uint64_t kBias = 0x8080808080808080ULL;
-
-__device__ __forceinline__ int field8(uint64_t packed, int r) { return (int)((packed >> (8 * r)) & 0xFFu) - 128; }
+// Packed per-shell histogram difference: one signed field per species, value in [-24, 24] (a shell has <= 24
+// neighbours), stored biased so that the fields never borrow from each other after the final add of the bias.
+//   M <= 4: 8-bit fields in 32 bits;  M == 5: 6-bit fields in 32 bits (30 used);  M >= 6: 8-bit fields in 64 bits.
+template <int M>
+struct Pack {
+    static constexpr int FB = (M == 5) ? 6 : 8;
+    static constexpr bool k32 = M * FB <= 32;
+    using W = typename std::conditional<k32, uint32_t, uint64_t>::type;
+    static constexpr int kHalf = 1 << (FB - 1);
+    __host__ __device__ static constexpr W bias()
+    {
+        W b = 0;
+        for (int r = 0; r < M; ++r) b |= (W)kHalf << (FB * r);
+        return b;
+    }
+    __device__ __forceinline__ static W one(uint32_t species) { return (W)1 << (FB * species); }
+    __device__ __forceinline__ static int field(W packed, int r) { return (int)((packed >> (FB * r)) & (W)((1 << FB) - 1)) - kHalf; }
+};
 
 // One shell's contribution  sum_i sum_j (1 - (N_ij + dN_ij) g_ij - t_ij)^2  in the D6 order.
 // dN[i][j] = ci*F[j] + cj*F[i], ci = [i==p] - [i==q], F[r] = #(nbrs of b of species r) - #(nbrs of a ...) (a, b excluded).
 template <int M>
 __device__ __forceinline__ double shell_sum(const int* __restrict__ cnt, const double* __restrict__ g,
-                                            const double* __restrict__ t, uint64_t dpacked, int p, int q)
+                                            const double* __restrict__ t, typename Pack<M>::W dpacked, int p, int q)
 {
     int F[M], c[M];
 #pragma unroll
-    for (int r = 0; r < M; ++r) { F[r] = field8(dpacked, r); c[r] = (r == p) - (r == q); }
+    for (int r = 0; r < M; ++r) { F[r] = Pack<M>::field(dpacked, r); c[r] = (r == p) - (r == q); }
     double sh = 0.0;
 #pragma unroll
     for (int i = 0; i < M; ++i) {
@@ -125,11 +143,16 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
     ChainShared& sh = *reinterpret_cast<ChainShared*>(s_raw);
-    uint8_t* s_occ = s_raw + sizeof(ChainShared);
+    // shared layout: ChainShared | neighbour index offsets [A][Z] | interior-site bitmap [ceil(N/32)] | occupancy
+    int* s_ds = reinterpret_cast<int*>(s_raw + sizeof(ChainShared));
+    uint32_t* s_bm = reinterpret_cast<uint32_t*>(s_ds + ((P.A * P.Z + 3) & ~3));
+    const bool FAST = OCC != OCC_GLOBAL && A.fast_nbr != 0;
+    uint8_t* s_occ = reinterpret_cast<uint8_t*>(s_bm + (FAST ? ((P.N + 127) >> 7) << 2 : 0));
 
     const int tid = threadIdx.x, T = blockDim.x;
     const int S = P.S, Z = P.Z, N = P.N, K = A.K, R = A.R;
     constexpr int MM = M * M;
+    using PW = typename Pack<M>::W;
     const int SMM = S * MM;
     const uint32_t rank = R > 1 ? cg::this_cluster().block_rank() : 0u;
     const size_t chain_local = blockIdx.x / (unsigned)R;
@@ -154,11 +177,30 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
         sh.best[0] = sh.best[1] = sh.best[2] = kNoKey;
     }
     if (tid < 2 * kMaxCluster) sh.rec[tid / kMaxCluster][tid % kMaxCluster].key = kNoKey;
+    if (FAST) {
+        // index offset of neighbour e of a site with basis index b when no periodic wrap occurs
+        const int Ly = P.L[1], Lz = P.L[2];
+        for (int i = tid; i < P.A * Z; i += T) {
+            const int8_t* st = P.tab->stencil + i * 4;
+            const int b = i / Z;
+            s_ds[i] = (((int)st[1] * Ly + (int)st[2]) * Lz + (int)st[3]) * P.A + ((int)st[0] - b);
+        }
+        // interior sites: every cell coordinate in [1, L-2], so no neighbour (cell shifts are -1, 0, +1) wraps
+        const int n_words = (N + 31) >> 5;
+        for (int wd = tid >> 5; wd < n_words; wd += T >> 5) {
+            const int site = wd * 32 + (tid & 31);
+            const int cell = site / P.A;
+            const int cz = cell % Lz, cy = (cell / Lz) % Ly, cx = cell / (Lz * Ly);
+            const bool in = site < N && cx >= 1 && cx <= P.L[0] - 2 && cy >= 1 && cy <= Ly - 2 && cz >= 1 && cz <= Lz - 2;
+            const uint32_t word = __ballot_sync(0xFFFFFFFFu, in);
+            if ((tid & 31) == 0) s_bm[wd] = word;
+        }
+    }
     __syncthreads();
     if (tid == 0) {
         double J = 0.0;
         for (int s = 0; s < S; ++s)
-            J = __dadd_rn(J, __dmul_rn(Kc.w[s], shell_sum<M>(sh.cnt + s * MM, Kc.g + s * MM, Kc.t + s * MM, kBias, 0, 0)));
+            J = __dadd_rn(J, __dmul_rn(Kc.w[s], shell_sum<M>(sh.cnt + s * MM, Kc.g + s * MM, Kc.t + s * MM, Pack<M>::bias(), 0, 0)));
         sh.J = J;
     }
     if (R > 1) cg::this_cluster().sync(); else __syncthreads();   // peers' shared memory is initialised before any post
@@ -190,7 +232,7 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
         volatile uint32_t* best_slot = &sh.best[buf];
         const double J_cur = sh.J;
         uint32_t win_key = kNoKey, win_a = 0, win_b = 0, win_pq = 0;
-        uint64_t win_d0 = 0, win_d1 = 0, win_d2 = 0;
+        PW win_d0 = 0, win_d1 = 0, win_d2 = 0;
         double win_J = 0.0;
         uint64_t nullmask = 0;
 
@@ -214,27 +256,35 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
                 nullmask |= 1ull << j;
             } else if (key < hint) {                             // same step, higher k than a known move: only nullness counts
                 // ---- D9.2 integer delta: per shell  sum_{nbrs of b} e_r - sum_{nbrs of a} e_r  (a, b excluded)
-                uint64_t d0 = 0, d1 = 0, d2 = 0;
+                // No per-entry exclusion: with m = #(entries of row a equal to b) and m_self = #(entries of a row equal
+                // to its own site) -- the table is symmetric with multiplicity and every site is equivalent -- the
+                // excluded sum is  d_all + (m - m_self) (e_q - e_p).
+                PW d0 = 0, d1 = 0, d2 = 0;
                 const int2* __restrict__ ra = reinterpret_cast<const int2*>(nbr + (size_t)a * Z);
                 const int2* __restrict__ rb = reinterpret_cast<const int2*>(nbr + (size_t)b * Z);
-                auto shell = [&](int e0, int e1) {
-                    uint64_t d = 0;
+                const bool ia = FAST && ((s_bm[a >> 5] >> (a & 31u)) & 1u), ib = FAST && ((s_bm[b >> 5] >> (b & 31u)) & 1u);
+                const int2* da = reinterpret_cast<const int2*>(s_ds + (a & (uint32_t)(P.A - 1)) * Z);
+                const int2* db = reinterpret_cast<const int2*>(s_ds + (b & (uint32_t)(P.A - 1)) * Z);
+                const PW eqp = Pack<M>::one(q) - Pack<M>::one(p);
+                auto shell = [&](int e0, int e1, int m_self) {
+                    PW d = 0;
+                    int m = -m_self;
 #pragma unroll 3
                     for (int e = e0; e < e1; ++e) {
-                        const int2 va = __ldg(ra + e), vb = __ldg(rb + e);
-                        const uint32_t v0 = (uint32_t)va.x, v1 = (uint32_t)va.y, v2 = (uint32_t)vb.x, v3 = (uint32_t)vb.y;
-                        const uint64_t o0 = 1ull << (8 * occ.get(v0)), o1 = 1ull << (8 * occ.get(v1));
-                        const uint64_t o2 = 1ull << (8 * occ.get(v2)), o3 = 1ull << (8 * occ.get(v3));
-                        d -= (v0 != a && v0 != b) ? o0 : 0ull;
-                        d -= (v1 != a && v1 != b) ? o1 : 0ull;
-                        d += (v2 != a && v2 != b) ? o2 : 0ull;
-                        d += (v3 != a && v3 != b) ? o3 : 0ull;
+                        int2 va, vb;
+                        if (ia) { const int2 o = da[e]; va = make_int2((int)a + o.x, (int)a + o.y); } else va = __ldg(ra + e);
+                        if (ib) { const int2 o = db[e]; vb = make_int2((int)b + o.x, (int)b + o.y); } else vb = __ldg(rb + e);
+                        d -= Pack<M>::one(occ.get((uint32_t)va.x));
+                        d -= Pack<M>::one(occ.get((uint32_t)va.y));
+                        d += Pack<M>::one(occ.get((uint32_t)vb.x));
+                        d += Pack<M>::one(occ.get((uint32_t)vb.y));
+                        m += ((uint32_t)va.x == b) + ((uint32_t)va.y == b);
                     }
-                    return d + kBias;
+                    return d + (PW)m * eqp + Pack<M>::bias();
                 };
-                d0 = shell(0, zq0);
-                if (S > 1) d1 = shell(zq0, zq1);
-                if (S > 2) d2 = shell(zq1, zq2);
+                d0 = shell(0, zq0, P.m_self[0]);
+                if (S > 1) d1 = shell(zq0, zq1, P.m_self[1]);
+                if (S > 2) d2 = shell(zq1, zq2, P.m_self[2]);
                 // ---- D6 objective from counts + delta
                 double Jk = __dmul_rn(Kc.w[0], shell_sum<M>(sh.cnt, Kc.g, Kc.t, d0, (int)p, (int)q));
                 Jk = __dadd_rn(0.0, Jk);
@@ -266,8 +316,8 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
                 m.key = key_best;
                 m.a = __shfl_sync(0xFFFFFFFFu, win_a, src); m.b = __shfl_sync(0xFFFFFFFFu, win_b, src);
                 m.pq = __shfl_sync(0xFFFFFFFFu, win_pq, src); m.J = __shfl_sync(0xFFFFFFFFu, win_J, src);
-                m.d[0] = __shfl_sync(0xFFFFFFFFu, win_d0, src); m.d[1] = __shfl_sync(0xFFFFFFFFu, win_d1, src);
-                m.d[2] = __shfl_sync(0xFFFFFFFFu, win_d2, src);
+                m.d[0] = __shfl_sync(0xFFFFFFFFu, (uint64_t)win_d0, src); m.d[1] = __shfl_sync(0xFFFFFFFFu, (uint64_t)win_d1, src);
+                m.d[2] = __shfl_sync(0xFFFFFFFFu, (uint64_t)win_d2, src);
                 if (lane < R) {
                     MoveRec* dst = cg::this_cluster().map_shared_rank(&sh.rec[par][rank], lane);
                     *dst = m;
@@ -304,9 +354,9 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
             const int p = (int)(mv->pq & 0xFFu), q = (int)(mv->pq >> 8);
             for (int idx = tid; idx < SMM; idx += T) {
                 const int s = idx / MM, rem = idx - s * MM, i = rem / M, jj = rem - i * M;
-                const uint64_t d = mv->d[s];
+                const PW d = (PW)mv->d[s];
                 const int ci = (i == p) - (i == q), cj = (jj == p) - (jj == q);
-                sh.cnt[idx] += ci * field8(d, jj) + cj * field8(d, i);
+                sh.cnt[idx] += ci * Pack<M>::field(d, jj) + cj * Pack<M>::field(d, i);
             }
             if (tid == T - 1) {                                 // one thread (not among the count updaters when T > SMM)
                 const uint32_t a = mv->a, b = mv->b, kk = key_best & 1023u;
@@ -362,9 +412,10 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
     if (tid == 0 && sh.n_null) atomicAdd(&g_stats[1], sh.n_null);
 }
 
+// query != nullptr: no launch, *query = how many clusters of A.R blocks of this shape can be resident at once.
 template <int M, int OCC>
 cudaError_t launch_one(const KParams& P, const DevTables& host_tab, const McArgs& A, int64_t C, int threads,
-                       size_t smem, cudaStream_t st)
+                       size_t smem, cudaStream_t st, int* query)
 {
     McConst<M> Kc;
     for (int s = 0; s < 3; ++s)
@@ -388,53 +439,56 @@ cudaError_t launch_one(const KParams& P, const DevTables& host_tab, const McArgs
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+    if (query) return cudaOccupancyMaxActiveClusters(query, kern, &cfg);
     return cudaLaunchKernelEx(&cfg, kern, P, Kc, A);
 }
 
 template <int M>
 cudaError_t launch_occ(int occ_mode, const KParams& P, const DevTables& host_tab, const McArgs& A, int64_t C,
-                       int threads, size_t smem, cudaStream_t st)
+                       int threads, size_t smem, cudaStream_t st, int* query)
 {
     switch (occ_mode) {
-        case OCC_SMEM_U8: return launch_one<M, OCC_SMEM_U8>(P, host_tab, A, C, threads, smem, st);
-        case OCC_SMEM_NIB: return launch_one<M, OCC_SMEM_NIB>(P, host_tab, A, C, threads, smem, st);
-        default: return launch_one<M, OCC_GLOBAL>(P, host_tab, A, C, threads, smem, st);
+        case OCC_SMEM_U8: return launch_one<M, OCC_SMEM_U8>(P, host_tab, A, C, threads, smem, st, query);
+        case OCC_SMEM_NIB: return launch_one<M, OCC_SMEM_NIB>(P, host_tab, A, C, threads, smem, st, query);
+        default: return launch_one<M, OCC_GLOBAL>(P, host_tab, A, C, threads, smem, st, query);
     }
 }
 
 }  // namespace
 
-size_t mc_shared_bytes(int occ_mode, int N)
+size_t mc_shared_bytes(int occ_mode, int N, int AZ, bool fast_nbr)
 {
-    size_t s = sizeof(ChainShared);
+    size_t s = sizeof(ChainShared) + sizeof(int) * (size_t)((AZ + 3) & ~3);
+    if (fast_nbr && occ_mode != OCC_GLOBAL) s += sizeof(uint32_t) * (size_t)(((N + 127) >> 7) << 2);
     if (occ_mode == OCC_SMEM_U8) s += (size_t)N;
     else if (occ_mode == OCC_SMEM_NIB) s += (size_t)(N + 1) / 2;
     return (s + 15) & ~(size_t)15;
 }
 
 cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode, int threads, int cluster, int w_max,
-                      uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
-                      uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches)
+                      bool fast_nbr, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
+                      uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches,
+                      int* query_max_clusters)
 {
-    const size_t smem = mc_shared_bytes(occ_mode, P.N);
+    const size_t smem = mc_shared_bytes(occ_mode, P.N, P.A * P.Z, fast_nbr);
     McArgs A;
     A.occ_all = occ; A.counts_all = counts;
     A.n_steps = n_steps; A.seed = seed; A.chain0 = chain0; A.step0 = step0;
     A.stats_all = reinterpret_cast<unsigned long long*>(stats);
     A.log_all = reinterpret_cast<unsigned long long*>(log);
-    A.log_cap = log_cap; A.K = K; A.R = cluster; A.w_max = w_max;
+    A.log_cap = log_cap; A.K = K; A.R = cluster; A.w_max = w_max; A.fast_nbr = fast_nbr ? 1 : 0;
     cudaError_t e;
     switch (P.M) {
-        case 1: e = launch_occ<1>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
-        case 2: e = launch_occ<2>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
-        case 3: e = launch_occ<3>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
-        case 4: e = launch_occ<4>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
-        case 5: e = launch_occ<5>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
-        case 6: e = launch_occ<6>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
-        case 7: e = launch_occ<7>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
-        default: e = launch_occ<8>(occ_mode, P, host_tab, A, C, threads, smem, st); break;
+        case 1: e = launch_occ<1>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 2: e = launch_occ<2>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 3: e = launch_occ<3>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 4: e = launch_occ<4>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 5: e = launch_occ<5>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 6: e = launch_occ<6>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 7: e = launch_occ<7>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        default: e = launch_occ<8>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
     }
-    if (e == cudaSuccess) ++*n_launches;
+    if (e == cudaSuccess && !query_max_clusters) ++*n_launches;
     return e;
 }
 

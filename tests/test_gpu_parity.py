@@ -121,7 +121,7 @@ def run_both(hb, w, n_chains, n_steps, log_cap=16, chain0=0, step0=0, opts=None,
     return o_stats
 
 
-@pytest.mark.parametrize("cluster", [1, 2, 4, 8])
+@pytest.mark.parametrize("cluster", [1, 2, 5, 8])
 @pytest.mark.parametrize("window", [0, 1, 3, 64])
 @pytest.mark.parametrize("occ_mode", [1, 2, 3])
 def test_mc_parity_all_launch_variants(hb, cluster, window, occ_mode):
@@ -133,11 +133,21 @@ def test_mc_parity_all_launch_variants(hb, cluster, window, occ_mode):
 
 @pytest.mark.parametrize("threads", [32, 64, 256, 1024])
 @pytest.mark.parametrize("cluster", [1, 4])
-def test_mc_parity_block_sizes_reject_regime(hb, threads, cluster):
+@pytest.mark.parametrize("neighbors", [1, 2])
+def test_mc_parity_block_sizes_reject_regime(hb, threads, cluster, neighbors):
     # target 0 on a small cell converges quickly: long windows without a move, then rare moves inside windows
     w = small("bcc", (6, 6, 6), [0.25] * 4, 3, K=32, n_steps=3000)
-    st = run_both(hb, w, 3, 3000, log_cap=256, opts={"mc_threads": threads, "mc_cluster": cluster})
+    st = run_both(hb, w, 3, 3000, log_cap=256,
+                  opts={"mc_threads": threads, "mc_cluster": cluster, "mc_neighbors": neighbors})
     assert (st["n_accept"] > 20).all()
+
+
+@pytest.mark.parametrize("lattice,dims", [("fcc", (7, 5, 6)), ("bcc", (5, 8, 6)), ("fcc", (3, 3, 9)), ("bcc", (2, 7, 7))])
+@pytest.mark.parametrize("occ_mode", [1, 2])
+def test_mc_parity_interior_fast_path(hb, lattice, dims, occ_mode):
+    # interior sites take neighbours as site + offset; boundary sites (and cells with an L < 3) use the table
+    w = small(lattice, dims, [0.3, 0.3, 0.4], 3, target_seed=21, K=48, n_steps=300)
+    run_both(hb, w, 4, 300, opts={"mc_neighbors": 2, "mc_occ_mode": occ_mode})
 
 
 @pytest.mark.parametrize("lattice,dims,conc,S", LATTICES[:9])
@@ -229,7 +239,7 @@ def test_argument_errors(hb):
     with pytest.raises(hb.HeaError):
         h.mc_run(occ, counts, 1, 2000, 1)
     with pytest.raises(hb.HeaError):
-        h.set_option("mc_cluster", 3)
+        h.set_option("mc_cluster", 9)
     with pytest.raises(hb.HeaError):
         h.set_option("nonsense", 1)
     with pytest.raises(hb.HeaError) as e:
