@@ -184,7 +184,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2411_18906_b200 import binding, workloads
+    from paper_2411_18906_b200 import binding, sharding, workloads
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -204,7 +204,7 @@ def main():
         h.set_option(k, int(v))
     C, K, N, n_mc = w.n_chains, w.K, w.n_sites, args.mc_steps
     SMM = h.S * h.M * h.M
-    chain0 = rank * C
+    chain0, _ = sharding.weak_chain_range(rank, C)
     occ = h.init_random(C, w.seed, chain0)
     counts = torch.empty((C, h.S, h.M, h.M), dtype=torch.int32, device=dev)
     stats = h.new_stats(C)
