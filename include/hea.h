@@ -72,8 +72,8 @@ const char* hea_last_error(void);
  *                    else floor + largest remainder, ties to the lower index); any N_i == 0 -> HEA_EINVAL
  *   shell_w          [n_shells] host;  alpha_target [n_shells][n_species][n_species] host, row-major
  *   n_species in [1, 8], n_shells in [1, 3] (else HEA_EUNSUPPORTED)
- *   device           CUDA device ordinal.  Builds both device copies of the neighbour table
- *                    (site-major for the MC kernel, slot-major for the recount kernel).
+ *   device           CUDA device ordinal.  Builds the device neighbour table (site-major [N][Z], rows padded to
+ *                    whole 32-site tiles; shared by the recount and the MC kernel).
  * All host arrays are copied.  Errors: HEA_EINVAL, HEA_EUNSUPPORTED, HEA_ENOMEM, HEA_ECUDA (no device / alloc failed).
  */
 int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz,
@@ -98,6 +98,9 @@ int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host);
  *   "mc_window"       cap on the speculative step window (steps evaluated against one configuration before the
  *                     lowest improving (step, k) is applied): 0 = auto, 1 = strictly step by step, up to 2^20
  *   "mc_neighbors"    0 = auto, 1 = always the neighbour table, 2 = interior sites use site + offset (no table load)
+ *   "sro_warps"       recount: warps per block, 0 = auto (16), 1..16
+ *   "sro_stages"      recount: cap on the per-warp ring of 32-site table tiles in shared memory, 0 = auto, 1..8
+ *   "sro_blocks_per_sm"  recount: resident blocks per SM the grid and the shared-memory split are sized for, 0 = auto, 1..4
  * Unknown name or value -> HEA_EINVAL.
  */
 int hea_set_option(hea_ctx* ctx, const char* name, int64_t value);

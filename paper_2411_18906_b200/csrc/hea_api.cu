@@ -11,15 +11,13 @@
 
 namespace hea {
 // launchers (hea_sro.cu / hea_mc.cu)
-cudaError_t launch_sro_count(const KParams& P, const uint8_t* occ, int64_t B, int32_t* counts, int n_sms,
-                             cudaStream_t st, int64_t* n_launches);
+cudaError_t launch_sro_count(const KParams& P, int lat, const uint8_t* occ, int64_t B, int32_t* counts, int n_sms,
+                             size_t smem_budget, int opt_stages, int opt_blocks_per_sm, int opt_warps, cudaStream_t st, int64_t* n_launches);
 cudaError_t launch_sro_epilogue(const KParams& P, const int32_t* counts, int64_t B, double* alpha, double* obj,
                                 cudaStream_t st, int64_t* n_launches);
 cudaError_t launch_init_random(const KParams& P, uint8_t* occ, int64_t C, uint64_t seed, uint64_t chain0,
                                const int64_t* n_per_species_dev, cudaStream_t st, int64_t* n_launches);
 cudaError_t launch_stats_reset(void* stats, int64_t C, cudaStream_t st, int64_t* n_launches);
-cudaError_t launch_transpose_table(const int32_t* site_major, int32_t* slot_major, int N, int Npad, int Z,
-                                   cudaStream_t st, int64_t* n_launches);
 size_t mc_shared_bytes(int occ_mode, int N, int AZ, bool fast_nbr);
 cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode, int threads, int cluster, int w_max,
                       bool fast_nbr, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
@@ -35,13 +33,12 @@ struct hea_ctx {
     int n_sms = 0;
     size_t smem_optin = 0;
     int32_t* d_nbr_site = nullptr;
-    int32_t* d_nbr_slot = nullptr;
     hea::DevTables* d_tab = nullptr;
     hea::DevTables tab_host{};
     int64_t* d_nps = nullptr;
     hea::KParams P{};
     // tuning options (0 = auto)
-    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0, opt_neighbors = 0;
+    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0, opt_neighbors = 0, opt_sro_stages = 0, opt_sro_bps = 0, opt_sro_warps = 0;
     int64_t n_launches = 0;
     // internal stream and scratch for the *_host entry points
     cudaStream_t stream = nullptr;
@@ -99,6 +96,9 @@ int64_t* option_slot(hea_ctx* ctx, const char* name)
     if (!strcmp(name, "mc_cluster")) return &ctx->opt_cluster;
     if (!strcmp(name, "mc_window")) return &ctx->opt_window;
     if (!strcmp(name, "mc_neighbors")) return &ctx->opt_neighbors;
+    if (!strcmp(name, "sro_stages")) return &ctx->opt_sro_stages;
+    if (!strcmp(name, "sro_blocks_per_sm")) return &ctx->opt_sro_bps;
+    if (!strcmp(name, "sro_warps")) return &ctx->opt_sro_warps;
     return nullptr;
 }
 
@@ -110,6 +110,9 @@ bool option_value_ok(const char* name, int64_t v)
     if (!strcmp(name, "mc_cluster")) return v >= 1 && v <= 8;
     if (!strcmp(name, "mc_window")) return v >= 1 && v <= (1 << 20);
     if (!strcmp(name, "mc_neighbors")) return v == 1 || v == 2;
+    if (!strcmp(name, "sro_stages")) return v >= 1 && v <= 8;
+    if (!strcmp(name, "sro_blocks_per_sm")) return v >= 1 && v <= 4;
+    if (!strcmp(name, "sro_warps")) return v >= 1 && v <= 16;
     return false;
 }
 
@@ -166,7 +169,7 @@ int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz, int n_species
 
     const hea::Lattice& lat = ctx->lat;
     const int N = (int)lat.N, Z = lat.Z, M = n_species, S = n_shells;
-    const int Npad = (N + 3) & ~3;
+    const int Npad = (N + 31) & ~31;      // table rows padded to whole 32-site tiles (padding rows point at site 0)
 
     // constant tables (D5-D6: den exact in fp64, one correctly rounded divide)
     std::vector<hea::DevTables> tab(1);
@@ -196,14 +199,13 @@ int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz, int n_species
         return bail(HEA_ECUDA, std::string("cudaStreamCreate: ") + cudaGetErrorString(e));
     if ((e = cudaMalloc(&ctx->d_tab, sizeof(hea::DevTables))) != cudaSuccess ||
         (e = cudaMalloc(&ctx->d_nps, sizeof(int64_t) * hea::kMaxSpecies)) != cudaSuccess ||
-        (e = cudaMalloc(&ctx->d_nbr_site, sizeof(int32_t) * (size_t)N * Z)) != cudaSuccess ||
-        (e = cudaMalloc(&ctx->d_nbr_slot, sizeof(int32_t) * (size_t)Npad * Z)) != cudaSuccess)
+        (e = cudaMalloc(&ctx->d_nbr_site, sizeof(int32_t) * (size_t)Npad * Z)) != cudaSuccess)
         return bail(HEA_ENOMEM, std::string("cudaMalloc tables: ") + cudaGetErrorString(e));
     if ((e = cudaMemcpy(ctx->d_tab, tab.data(), sizeof(hea::DevTables), cudaMemcpyHostToDevice)) != cudaSuccess ||
         (e = cudaMemcpy(ctx->d_nps, ctx->n_per_species, sizeof(int64_t) * hea::kMaxSpecies, cudaMemcpyHostToDevice)) != cudaSuccess)
         return bail(HEA_ECUDA, std::string("cudaMemcpy tables: ") + cudaGetErrorString(e));
 
-    // host table builder -> site-major device table, in chunks; slot-major copy by a device transpose
+    // host table builder -> site-major device table, in chunks
     {
         const int64_t chunk_sites = 1 << 20;
         std::vector<int32_t> buf((size_t)std::min<int64_t>(chunk_sites, N) * Z);
@@ -214,9 +216,10 @@ int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz, int n_species
                            cudaMemcpyHostToDevice);
             if (e != cudaSuccess) return bail(HEA_ECUDA, std::string("cudaMemcpy table: ") + cudaGetErrorString(e));
         }
-        e = hea::launch_transpose_table(ctx->d_nbr_site, ctx->d_nbr_slot, N, Npad, Z, ctx->stream, &ctx->n_launches);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-        if (e != cudaSuccess) return bail(HEA_ECUDA, std::string("table transpose: ") + cudaGetErrorString(e));
+        if (Npad > N) {
+            e = cudaMemset(ctx->d_nbr_site + (size_t)N * Z, 0, sizeof(int32_t) * (size_t)(Npad - N) * Z);
+            if (e != cudaSuccess) return bail(HEA_ECUDA, std::string("cudaMemset table padding: ") + cudaGetErrorString(e));
+        }
     }
 
     hea::KParams& P = ctx->P;
@@ -233,7 +236,6 @@ int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz, int n_species
             }
     }
     P.nbr_site = ctx->d_nbr_site;
-    P.nbr_slot = ctx->d_nbr_slot;
     P.tab = ctx->d_tab;
     ctx->tab_host = tab[0];
     *out = ctx;
@@ -249,7 +251,6 @@ int hea_destroy(hea_ctx* ctx)
         cudaFree(ctx->d_tab);
         cudaFree(ctx->d_nps);
         cudaFree(ctx->d_nbr_site);
-        cudaFree(ctx->d_nbr_slot);
         for (void* p : ctx->scratch) cudaFree(p);
     }
     delete ctx;
@@ -320,7 +321,8 @@ int hea_sro_full(hea_ctx* ctx, const uint8_t* occ_dev, int64_t B, int32_t* count
     if (!occ_dev || !counts_dev) return fail(HEA_EINVAL, "occ_dev / counts_dev is NULL");
     DeviceGuard guard(ctx->device);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    cudaError_t e = hea::launch_sro_count(ctx->P, occ_dev, B, counts_dev, ctx->n_sms, st, &ctx->n_launches);
+    cudaError_t e = hea::launch_sro_count(ctx->P, ctx->lat.type, occ_dev, B, counts_dev, ctx->n_sms, ctx->smem_optin,
+                                          (int)ctx->opt_sro_stages, (int)ctx->opt_sro_bps, (int)ctx->opt_sro_warps, st, &ctx->n_launches);
     if (e != cudaSuccess) return fail_cuda(e, "hea_sro_full count launch");
     e = hea::launch_sro_epilogue(ctx->P, counts_dev, B, alpha_dev, obj_dev, st, &ctx->n_launches);
     return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_sro_full epilogue launch");

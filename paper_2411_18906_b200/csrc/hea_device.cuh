@@ -19,14 +19,13 @@ struct DevTables {
 // Scalars passed by value to every kernel.
 struct KParams {
     int N;                                // sites
-    int Npad;                             // N rounded up to a multiple of 4 (row stride of the slot-major table)
+    int Npad;                             // N rounded up to a multiple of 32: rows of the table (whole 32-site tiles)
     int M, S, Z, A;
     int L[3];
     int z[3];
     int zoff[4];
     int m_self[3];                        // per shell: table entries of a site that are the site itself (0 unless a tiny cell)
-    const int32_t* nbr_site;              // [N][Z]   site-major: the Z neighbours of one site are contiguous
-    const int32_t* nbr_slot;              // [Z][Npad] slot-major: one slot of consecutive sites is contiguous
+    const int32_t* nbr_site;              // [Npad][Z] site-major: the Z neighbours of one site are contiguous
     const DevTables* tab;
 };
 

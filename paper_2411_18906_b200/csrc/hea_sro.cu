@@ -2,115 +2,199 @@
 // DESIGN.md D4-D6, D8; Eq. 2, Eq. 3, P:207, P:275 (the recount is >99% of the
 // time of the non-incremental search).
 //
-// Recount kernel (direct variant).  HBM-bound by the slot-major neighbour table: 4*Z bytes per site per pass.
-//   - one thread owns 4 consecutive sites; for every slot it reads the 4 neighbour indices with one 16-byte
-//     coalesced load (a warp reads 512 contiguous bytes of the table per slot) and gathers the 4 neighbour species
-//     bytes (lattice-local, L1/L2 hits);
-//   - per site and shell the neighbour species are counted in a packed register histogram (8-bit fields), then
-//     folded into per-thread rows acc[s][own species] of 16-bit fields with predicated adds (no dynamic indexing);
+// Recount kernel.  HBM-bound by the neighbour table: 4*Z bytes per site per pass, plus one occupancy byte.
+//   - the site-major table [Npad][Z] is streamed through shared memory with bulk asynchronous copies
+//     (cp.async.bulk global -> shared, completion on an mbarrier): a TILE is 32 consecutive sites = one contiguous
+//     128*Z-byte run of the table = one copy.  Every WARP owns a private ring of stages and its own mbarriers; lane 0
+//     refills a stage as soon as the warp has consumed it, so there is no block-level synchronisation in the main loop
+//     and the bytes in flight per SM (warps x stages x 128 Z) are set by shared memory, not by registers;
+//   - lane = site of the tile: it reads its table row from shared memory as 8-byte words (row stride 4 Z bytes, Z even
+//     but Z/2 odd or = 2 mod 4 for every supported lattice/shell set: conflict-free or 2-way), gathers the Z neighbour
+//     species bytes (neighbours of consecutive sites are consecutive: one or two 32-byte sectors per warp gather,
+//     L1/L2 hits) with all gathers of a site in flight at once (shell sizes are template constants);
+//   - per site and shell the neighbour species are counted in a packed register histogram, then folded into per-thread
+//     rows acc[s][own species] of 16-bit fields with multiply-adds by the 0/1 "row is mine" flags (no dynamic
+//     register indexing);
 //   - at the end: unpack, warp REDUX add, shared-memory bins, one global atomicAdd per bin per block.
-// Integer adds commute, so the result is bit-exact whatever the order.
+// A block walks a contiguous range of tiles (its warps interleaved), so the occupancy lines it gathers from form a
+// few sliding windows that stay in L1.  Integer adds commute, so the result is bit-exact whatever the order.
+#include <algorithm>
+#include <type_traits>
+
 #include "hea_device.cuh"
 
 namespace hea {
 
 namespace {
 
-constexpr int kSroThreads = 256;
-constexpr int kFlushSites = 2048;         // 16-bit fields: 2048 sites * z<=24 < 65536
+constexpr int kSroMaxWarps = 16;
+constexpr int kSroMaxThreads = kSroMaxWarps * 32;
+constexpr int kSroMaxStages = 8;
+constexpr int kFlushTiles = 2048;         // 16-bit fields: 2048 sites per lane * z <= 24 < 65536
 
-template <int M>
-__global__ void __launch_bounds__(kSroThreads)
-sro_count_kernel(const KParams P, const uint8_t* __restrict__ occ_all, int32_t* __restrict__ counts_all)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
 {
-    constexpr int W = (M + 1) / 2;        // 32-bit words per row, two 16-bit fields (species 2w, 2w+1) each
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+
+// arm the barrier with the byte count, then start the bulk copy that completes on it
+__device__ __forceinline__ void bulk_load(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "HEA_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra HEA_DONE_%=;\n"
+        "bra HEA_WAIT_%=;\n"
+        "HEA_DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+
+// Packed per-site neighbour histogram of one shell (counts <= 24): M <= 4 -> 8-bit fields in 32 bits, M == 5 -> 6-bit
+// fields in 32 bits, M >= 6 -> 8-bit fields in 64 bits.  spread16(w) = fields 2w and 2w+1 as two 16-bit fields.
+template <int M>
+struct Hist {
+    static constexpr int FB = (M == 5) ? 6 : 8;
+    using W = typename std::conditional<(M * FB <= 32), uint32_t, uint64_t>::type;
+    __device__ __forceinline__ static W one(uint32_t species) { return (W)1 << (FB * species); }
+    __device__ __forceinline__ static uint32_t spread16(W h, int w)
+    {
+        if (FB == 8) {
+            const uint32_t half = (w < 2) ? (uint32_t)h : (uint32_t)((uint64_t)h >> 32);
+            return __byte_perm(half, 0, (w & 1) ? 0x4342 : 0x4140);
+        }
+        const uint32_t x = (uint32_t)h >> (12 * w);
+        return (x & 63u) | ((x << 10) & (63u << 16));
+    }
+};
+
+// LAT 0 = fcc (z = 12, 6, 24), 1 = bcc (z = 8, 6, 12): D2.
+template <int LAT, int S>
+struct Shells {
+    static constexpr int z0 = LAT == 0 ? 12 : 8, z1 = S > 1 ? 6 : 0, z2 = S > 2 ? (LAT == 0 ? 24 : 12) : 0;
+    static constexpr int Z = z0 + z1 + z2;
+};
+
+template <int M, int LAT, int S>
+__global__ void __launch_bounds__(kSroMaxThreads)
+sro_count_kernel(const KParams P, const uint8_t* __restrict__ occ_all, int32_t* __restrict__ counts_all,
+                 int tiles_per_block, int n_stages)
+{
+    using SH = Shells<LAT, S>;
+    using H = Hist<M>;
+    using HW = typename H::W;
+    constexpr int Z = SH::Z, ZH = Z / 2;
+    constexpr int W16 = (M + 1) / 2;      // 32-bit words per accumulator row, two 16-bit fields (species 2w, 2w+1) each
+    constexpr uint32_t kStageBytes = 128u * Z;
+
+    extern __shared__ __align__(128) uint8_t s_stage[];              // [warp][stage][32 sites][Z] int32
+    __shared__ uint64_t s_bar[kSroMaxWarps * kSroMaxStages];
     __shared__ int s_bins[kSMM];
-    const int SMM = P.S * M * M;
+    constexpr int SMM = S * M * M;
     for (int i = threadIdx.x; i < SMM; i += blockDim.x) s_bins[i] = 0;
-    __syncthreads();
 
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int kSroWarps = (int)(blockDim.x >> 5);
     const uint8_t* __restrict__ occ = occ_all + (size_t)blockIdx.y * P.N;
-    const bool aligned4 = ((reinterpret_cast<uintptr_t>(occ) & 3) == 0);
+    const int n_tiles = P.Npad >> 5;
+    const int t_begin = blockIdx.x * tiles_per_block;
+    const int t_end = min(n_tiles, t_begin + tiles_per_block);
+    uint8_t* my_stage = s_stage + (size_t)warp * n_stages * kStageBytes;
+    uint64_t* my_bar = s_bar + warp * kSroMaxStages;
+    const uint8_t* tab = reinterpret_cast<const uint8_t*>(P.nbr_site);
 
-    uint32_t acc[3][M][W];
+    // this warp's tiles: t_begin + warp + i * kSroWarps
+    const int first = t_begin + warp;
+    const int n_mine = first < t_end ? (t_end - first + kSroWarps - 1) / kSroWarps : 0;
+    if (lane == 0) {
+        for (int st = 0; st < n_stages; ++st) mbar_init(my_bar + st, 1);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        for (int st = 0; st < n_stages && st < n_mine; ++st)
+            bulk_load(my_stage + (size_t)st * kStageBytes, tab + (size_t)(first + st * kSroWarps) * kStageBytes,
+                      kStageBytes, my_bar + st);
+    }
+    __syncthreads();                                                  // s_bins zeroed, barriers initialised
+
+    uint32_t acc[S][M][W16];
 #pragma unroll
-    for (int s = 0; s < 3; ++s)
+    for (int s = 0; s < S; ++s)
 #pragma unroll
         for (int i = 0; i < M; ++i)
 #pragma unroll
-            for (int w = 0; w < W; ++w) acc[s][i][w] = 0;
+            for (int w = 0; w < W16; ++w) acc[s][i][w] = 0;
 
     auto flush = [&]() {
 #pragma unroll
-        for (int s = 0; s < 3; ++s) {
-            if (s < P.S) {
-#pragma unroll
-                for (int i = 0; i < M; ++i)
-#pragma unroll
-                    for (int j = 0; j < M; ++j) {
-                        const int v = (acc[s][i][j >> 1] >> ((j & 1) * 16)) & 0xFFFF;
-                        const int tot = __reduce_add_sync(0xFFFFFFFFu, v);
-                        if ((threadIdx.x & 31) == 0 && tot) atomicAdd(&s_bins[(s * M + i) * M + j], tot);
-                    }
-            }
-        }
-#pragma unroll
-        for (int s = 0; s < 3; ++s)
+        for (int s = 0; s < S; ++s)
 #pragma unroll
             for (int i = 0; i < M; ++i)
 #pragma unroll
-                for (int w = 0; w < W; ++w) acc[s][i][w] = 0;
+                for (int j = 0; j < M; ++j) {
+                    const int v = (acc[s][i][j >> 1] >> ((j & 1) * 16)) & 0xFFFF;
+                    const int tot = __reduce_add_sync(0xFFFFFFFFu, v);
+                    if (lane == 0 && tot) atomicAdd(&s_bins[(s * M + i) * M + j], tot);
+                }
+#pragma unroll
+        for (int s = 0; s < S; ++s)
+#pragma unroll
+            for (int i = 0; i < M; ++i)
+#pragma unroll
+                for (int w = 0; w < W16; ++w) acc[s][i][w] = 0;
     };
 
-    const int n_quads = P.Npad >> 2;
     int since_flush = 0;
-    const int lane = threadIdx.x & 31;
-    // warp-uniform trip count (flush() uses full-warp REDUX): lanes past the end work on quad 0 with a species
-    // id that matches no row, so they add nothing.
-    for (int quad = blockIdx.x * blockDim.x + threadIdx.x; quad - lane < n_quads; quad += gridDim.x * blockDim.x) {
-        const bool active = quad < n_quads;
-        const int site0 = active ? quad << 2 : 0;
-        const int n_valid = active ? min(4, P.N - site0) : 0;
-        uint32_t own[4];
-        if (aligned4 && n_valid == 4) {
-            const uint32_t o4 = *reinterpret_cast<const uint32_t*>(occ + site0);
-            own[0] = o4 & 0xFF; own[1] = (o4 >> 8) & 0xFF; own[2] = (o4 >> 16) & 0xFF; own[3] = o4 >> 24;
-        } else {
+    int st = 0;
+    uint32_t parity = 0;
+    for (int i = 0; i < n_mine; ++i) {
+        const int tile = first + i * kSroWarps;
+        const int site = (tile << 5) + lane;
+        const uint32_t own = site < P.N ? (uint32_t)__ldg(occ + site) : 0xFFu;   // 0xFF matches no row
+        uint32_t mine[M];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) own[c] = c < n_valid ? occ[site0 + c] : 0xFFu;   // 0xFF never matches a row
+        for (int r = 0; r < M; ++r) mine[r] = own == (uint32_t)r;
+        mbar_wait(my_bar + st, parity);
+        const int2* __restrict__ row = reinterpret_cast<const int2*>(my_stage + (size_t)st * kStageBytes) + lane * ZH;
+        int2 nb[ZH];
+#pragma unroll
+        for (int e = 0; e < ZH; ++e) nb[e] = row[e];
+        uint32_t sp[Z];
+#pragma unroll
+        for (int e = 0; e < ZH; ++e) {
+            sp[2 * e] = __ldg(occ + (uint32_t)nb[e].x);
+            sp[2 * e + 1] = __ldg(occ + (uint32_t)nb[e].y);
         }
+        // the stage is consumed (its words are in registers): refill it with the tile n_stages ahead
+        __syncwarp();
+        if (lane == 0 && i + n_stages < n_mine)
+            bulk_load(my_stage + (size_t)st * kStageBytes, tab + (size_t)(tile + n_stages * kSroWarps) * kStageBytes,
+                      kStageBytes, my_bar + st);
+        if (++st == n_stages) { st = 0; parity ^= 1u; }
 #pragma unroll
-        for (int s = 0; s < 3; ++s) {
-            if (s < P.S) {
-                uint64_t h[4] = {0, 0, 0, 0};
-                const int e0 = P.zoff[s], e1 = P.zoff[s + 1];
-#pragma unroll 6
-                for (int e = e0; e < e1; ++e) {
-                    const int4 nb = __ldg(reinterpret_cast<const int4*>(P.nbr_slot + (size_t)e * P.Npad + site0));
-                    h[0] += 1ull << (8 * occ[nb.x]);
-                    h[1] += 1ull << (8 * occ[nb.y]);
-                    h[2] += 1ull << (8 * occ[nb.z]);
-                    h[3] += 1ull << (8 * occ[nb.w]);
-                }
+        for (int s = 0; s < S; ++s) {
+            constexpr int zo[4] = {0, SH::z0, SH::z0 + SH::z1, SH::Z};
+            HW h = 0;
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    const uint32_t hlo = (uint32_t)h[c], hhi = (uint32_t)(h[c] >> 32);
-                    uint32_t e16[4];      // bytes spread into 16-bit fields: species (0,1) (2,3) (4,5) (6,7)
-                    e16[0] = __byte_perm(hlo, 0, 0x4140);
-                    e16[1] = __byte_perm(hlo, 0, 0x4342);
-                    e16[2] = __byte_perm(hhi, 0, 0x4140);
-                    e16[3] = __byte_perm(hhi, 0, 0x4342);
+            for (int e = zo[s]; e < zo[s + 1]; ++e) h += H::one(sp[e]);
 #pragma unroll
-                    for (int i = 0; i < M; ++i) {
-                        const bool mine = (own[c] == (uint32_t)i);
+            for (int w = 0; w < W16; ++w) {
+                const uint32_t e16 = H::spread16(h, w);
 #pragma unroll
-                        for (int w = 0; w < W; ++w) acc[s][i][w] += mine ? e16[w] : 0u;
-                    }
-                }
+                for (int r = 0; r < M; ++r) acc[s][r][w] += e16 * mine[r];
             }
         }
-        since_flush += 4;
-        if (since_flush >= kFlushSites) { flush(); since_flush = 0; }   // trip count is warp-uniform
+        if (++since_flush >= kFlushTiles) { flush(); since_flush = 0; }          // warp-uniform
     }
     flush();
     __syncthreads();
@@ -208,50 +292,83 @@ __global__ void stats_reset_kernel(uint64_t* stats_words, int64_t C)
     st[0] = 0; st[1] = 0; st[2] = 0xcbf29ce484222325ULL; st[3] = 0xffffffffffffffffULL; st[4] = 0;   // J = +0.0
 }
 
-// site-major [N][Z] -> slot-major [Z][Npad] (padding entries point at site 0)
-__global__ void transpose_table_kernel(const int32_t* __restrict__ site_major, int32_t* __restrict__ slot_major,
-                                       int N, int Npad, int Z)
+}  // namespace
+
+// ---------------------------------------------------------------- launchers (called from hea_api.cu)
+namespace {
+
+template <int M, int LAT, int S>
+cudaError_t launch_sro_one(const KParams& P, const uint8_t* occ, int32_t* counts, dim3 grid, int tiles_per_block,
+                           int n_stages, int n_warps, cudaStream_t st)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= (int64_t)Z * Npad) return;
-    const int e = (int)(i / Npad), site = (int)(i % Npad);
-    slot_major[i] = site < N ? site_major[(size_t)site * Z + e] : 0;
+    auto kern = sro_count_kernel<M, LAT, S>;
+    const size_t smem = (size_t)n_stages * n_warps * 128u * Shells<LAT, S>::Z;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, n_warps * 32, smem, st>>>(P, occ, counts, tiles_per_block, n_stages);
+    return cudaGetLastError();
+}
+
+template <int M>
+cudaError_t launch_sro_m(const KParams& P, int lat, const uint8_t* occ, int32_t* counts, dim3 grid, int tiles_per_block,
+                         int n_stages, int n_warps, cudaStream_t st)
+{
+    switch (lat * 3 + P.S) {
+        case 1: return launch_sro_one<M, 0, 1>(P, occ, counts, grid, tiles_per_block, n_stages, n_warps, st);
+        case 2: return launch_sro_one<M, 0, 2>(P, occ, counts, grid, tiles_per_block, n_stages, n_warps, st);
+        case 3: return launch_sro_one<M, 0, 3>(P, occ, counts, grid, tiles_per_block, n_stages, n_warps, st);
+        case 4: return launch_sro_one<M, 1, 1>(P, occ, counts, grid, tiles_per_block, n_stages, n_warps, st);
+        case 5: return launch_sro_one<M, 1, 2>(P, occ, counts, grid, tiles_per_block, n_stages, n_warps, st);
+        default: return launch_sro_one<M, 1, 3>(P, occ, counts, grid, tiles_per_block, n_stages, n_warps, st);
+    }
 }
 
 }  // namespace
 
-// ---------------------------------------------------------------- launchers (called from hea_api.cu)
-cudaError_t launch_sro_count(const KParams& P, const uint8_t* occ, int64_t B, int32_t* counts, int n_sms,
-                             cudaStream_t st, int64_t* n_launches)
+// lat: 0 fcc, 1 bcc (the shell sizes are template constants of the kernel).  smem_budget: opt-in shared memory per block.
+cudaError_t launch_sro_count(const KParams& P, int lat, const uint8_t* occ, int64_t B, int32_t* counts, int n_sms,
+                             size_t smem_budget, int opt_stages, int opt_blocks_per_sm, int opt_warps, cudaStream_t st, int64_t* n_launches)
 {
     const int SMM = P.S * P.M * P.M;
     cudaError_t e = cudaMemsetAsync(counts, 0, sizeof(int32_t) * (size_t)SMM * (size_t)B, st);
     if (e != cudaSuccess) return e;
-    const int n_quads = P.Npad >> 2;
-    int bx = (n_quads + kSroThreads - 1) / kSroThreads;
-    // grid sized in multiples of the SM count: up to 8 resident blocks of 256 threads per SM
-    const int64_t cap = (int64_t)n_sms * 8;
-    int64_t want = cap / (B < 1 ? 1 : B);
-    if (want < 1) want = 1;
-    if (bx > want) bx = (int)want;
+    const int n_tiles = P.Npad >> 5;
+    const int kSroWarps = opt_warps > 0 ? opt_warps : 16, n_warps = kSroWarps;
+    const size_t stage_bytes = (size_t)kSroWarps * 128u * P.Z;      // one stage of every warp of a block
+    // resident blocks per SM (default one block of 16 warps; measured within 2 % of 2 x 8 warps on B200), each with an
+    // equal share of the SM's shared memory for its stage ring; at least one stage per warp must fit
+    const size_t per_sm = smem_budget + 1024;                       // opt-in per-block limit + its 1 KB reservation
+    int bps = opt_blocks_per_sm > 0 ? opt_blocks_per_sm : 1;
+    while (bps > 1 && per_sm / bps < stage_bytes + 5120) --bps;
+    const size_t usable = per_sm / bps > 5120 ? per_sm / bps - 5120 : 0;   // static (barriers, bins) + reservation
+    int max_stages = (int)std::min<size_t>(kSroMaxStages, usable / stage_bytes);
+    if (max_stages < 1) return cudaErrorInvalidConfiguration;
+    if (opt_stages > 0 && opt_stages < max_stages) max_stages = opt_stages;
+    // blocks per configuration: bps blocks per SM over the whole batch, each walking a contiguous range of tiles
+    int64_t bx = std::max<int64_t>(1, (int64_t)n_sms * bps / std::max<int64_t>(1, B));
+    bx = std::min<int64_t>(bx, (n_tiles + kSroWarps - 1) / kSroWarps);
+    const int tiles_per_block = (int)((n_tiles + bx - 1) / bx);
+    bx = (n_tiles + tiles_per_block - 1) / tiles_per_block;
+    const int n_stages = std::max(1, std::min(max_stages, (tiles_per_block + kSroWarps - 1) / kSroWarps));
     for (int64_t b0 = 0; b0 < B; b0 += 65535) {
         const int by = (int)((B - b0) < 65535 ? (B - b0) : 65535);
-        dim3 grid(bx, by);
+        dim3 grid((unsigned)bx, by);
         const uint8_t* o = occ + (size_t)b0 * P.N;
         int32_t* c = counts + (size_t)b0 * SMM;
         switch (P.M) {
-            case 1: sro_count_kernel<1><<<grid, kSroThreads, 0, st>>>(P, o, c); break;
-            case 2: sro_count_kernel<2><<<grid, kSroThreads, 0, st>>>(P, o, c); break;
-            case 3: sro_count_kernel<3><<<grid, kSroThreads, 0, st>>>(P, o, c); break;
-            case 4: sro_count_kernel<4><<<grid, kSroThreads, 0, st>>>(P, o, c); break;
-            case 5: sro_count_kernel<5><<<grid, kSroThreads, 0, st>>>(P, o, c); break;
-            case 6: sro_count_kernel<6><<<grid, kSroThreads, 0, st>>>(P, o, c); break;
-            case 7: sro_count_kernel<7><<<grid, kSroThreads, 0, st>>>(P, o, c); break;
-            default: sro_count_kernel<8><<<grid, kSroThreads, 0, st>>>(P, o, c); break;
+            case 1: e = launch_sro_m<1>(P, lat, o, c, grid, tiles_per_block, n_stages, n_warps, st); break;
+            case 2: e = launch_sro_m<2>(P, lat, o, c, grid, tiles_per_block, n_stages, n_warps, st); break;
+            case 3: e = launch_sro_m<3>(P, lat, o, c, grid, tiles_per_block, n_stages, n_warps, st); break;
+            case 4: e = launch_sro_m<4>(P, lat, o, c, grid, tiles_per_block, n_stages, n_warps, st); break;
+            case 5: e = launch_sro_m<5>(P, lat, o, c, grid, tiles_per_block, n_stages, n_warps, st); break;
+            case 6: e = launch_sro_m<6>(P, lat, o, c, grid, tiles_per_block, n_stages, n_warps, st); break;
+            case 7: e = launch_sro_m<7>(P, lat, o, c, grid, tiles_per_block, n_stages, n_warps, st); break;
+            default: e = launch_sro_m<8>(P, lat, o, c, grid, tiles_per_block, n_stages, n_warps, st); break;
         }
+        if (e != cudaSuccess) return e;
         ++*n_launches;
     }
-    return cudaGetLastError();
+    return cudaSuccess;
 }
 
 cudaError_t launch_sro_epilogue(const KParams& P, const int32_t* counts, int64_t B, double* alpha, double* obj,
@@ -285,15 +402,6 @@ cudaError_t launch_init_random(const KParams& P, uint8_t* occ, int64_t C, uint64
 cudaError_t launch_stats_reset(void* stats, int64_t C, cudaStream_t st, int64_t* n_launches)
 {
     stats_reset_kernel<<<(unsigned)((C + 255) / 256), 256, 0, st>>>(reinterpret_cast<uint64_t*>(stats), C);
-    ++*n_launches;
-    return cudaGetLastError();
-}
-
-cudaError_t launch_transpose_table(const int32_t* site_major, int32_t* slot_major, int N, int Npad, int Z,
-                                   cudaStream_t st, int64_t* n_launches)
-{
-    const int64_t total = (int64_t)Z * Npad;
-    transpose_table_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(site_major, slot_major, N, Npad, Z);
     ++*n_launches;
     return cudaGetLastError();
 }
