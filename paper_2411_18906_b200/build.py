@@ -9,7 +9,7 @@ LIB = os.path.join(HERE, "libhea_b200.so")
 SOURCES = ["hea_api.cu", "hea_sro.cu", "hea_mc.cu", "hea_lattice.cpp"]
 HEADERS = ["hea_device.cuh", "hea_lattice.hpp", os.path.join("..", "..", "include", "hea.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "-shared"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "-shared", "--threads", "0"]
 
 
 def _stale():

@@ -21,6 +21,7 @@
 // every peer's shared memory through DSMEM, then all replicas apply the global minimum).
 #include <cooperative_groups.h>
 
+#include <cstring>
 #include <type_traits>
 
 #include "hea_device.cuh"
@@ -93,6 +94,7 @@ struct McArgs {
     int R;                        // blocks per chain (cluster size)
     int w_max;                    // cap on the window length in steps (>= 1)
     int fast_nbr;                 // 1: interior sites take neighbours as site + offset (shared-memory stencil), no table load
+    int prune;                    // 1: all shell weights >= 0, so every shell term w_s*sh_s is an exact lower bound of J (see below)
 };
 
 // Packed per-shell histogram difference: one signed field per species, value in [-24, 24] (a shell has <= 24
@@ -116,28 +118,38 @@ struct Pack {
 
 // One shell's contribution  sum_i sum_j (1 - (N_ij + dN_ij) g_ij - t_ij)^2  in the D6 order.
 // dN[i][j] = ci*F[j] + cj*F[i], ci = [i==p] - [i==q], F[r] = #(nbrs of b of species r) - #(nbrs of a ...) (a, b excluded).
-template <int M>
+// SYM: target symmetric (t_ij == t_ji bitwise; g and the counts of a recount always are), so e_ji is the same sequence of
+// operations on the same operands as e_ij and is reused instead of recomputed; the additions keep the D6 order.
+template <int M, bool SYM>
 __device__ __forceinline__ double shell_sum(const int* __restrict__ cnt, const double* __restrict__ g,
                                             const double* __restrict__ t, typename Pack<M>::W dpacked, int p, int q)
 {
     int F[M], c[M];
 #pragma unroll
     for (int r = 0; r < M; ++r) { F[r] = Pack<M>::field(dpacked, r); c[r] = (r == p) - (r == q); }
+    double up[M * M];               // only entries (i, j > i) are live when SYM
     double sh = 0.0;
 #pragma unroll
     for (int i = 0; i < M; ++i) {
         double row = 0.0;
 #pragma unroll
         for (int j = 0; j < M; ++j) {
-            const int n = cnt[i * M + j] + c[i] * F[j] + c[j] * F[i];
-            row = __dadd_rn(row, sq_dev(n, g[i * M + j], t[i * M + j]));
+            double e;
+            if (SYM && j < i) {
+                e = up[j * M + i];
+            } else {
+                const int n = cnt[i * M + j] + c[i] * F[j] + c[j] * F[i];
+                e = sq_dev(n, g[i * M + j], t[i * M + j]);
+                if (SYM && j > i) up[i * M + j] = e;
+            }
+            row = __dadd_rn(row, e);
         }
         sh = __dadd_rn(sh, row);
     }
     return sh;
 }
 
-template <int M, int OCC>
+template <int M, int OCC, bool SYM>
 __global__ void __launch_bounds__(1024)
 mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const McArgs A)
 {
@@ -200,7 +212,7 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
     if (tid == 0) {
         double J = 0.0;
         for (int s = 0; s < S; ++s)
-            J = __dadd_rn(J, __dmul_rn(Kc.w[s], shell_sum<M>(sh.cnt + s * MM, Kc.g + s * MM, Kc.t + s * MM, Pack<M>::bias(), 0, 0)));
+            J = __dadd_rn(J, __dmul_rn(Kc.w[s], shell_sum<M, false>(sh.cnt + s * MM, Kc.g + s * MM, Kc.t + s * MM, Pack<M>::bias(), 0, 0)));
         sh.J = J;
     }
     if (R > 1) cg::this_cluster().sync(); else __syncthreads();   // peers' shared memory is initialised before any post
@@ -282,14 +294,25 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
                     }
                     return d + (PW)m * eqp + Pack<M>::bias();
                 };
+                // ---- D6 objective from counts + delta, shell by shell.  With w_s >= 0 every partial sum is an exact
+                // lower bound of J_k (each term is >= 0 and rounding is monotonic), so once it reaches J_cur the candidate
+                // cannot improve and the remaining shells are skipped when no lane of the warp still needs them.
+                const bool prune = A.prune != 0;
                 d0 = shell(0, zq0, P.m_self[0]);
-                if (S > 1) d1 = shell(zq0, zq1, P.m_self[1]);
-                if (S > 2) d2 = shell(zq1, zq2, P.m_self[2]);
-                // ---- D6 objective from counts + delta
-                double Jk = __dmul_rn(Kc.w[0], shell_sum<M>(sh.cnt, Kc.g, Kc.t, d0, (int)p, (int)q));
+                double Jk = __dmul_rn(Kc.w[0], shell_sum<M, SYM>(sh.cnt, Kc.g, Kc.t, d0, (int)p, (int)q));
                 Jk = __dadd_rn(0.0, Jk);
-                if (S > 1) Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[1], shell_sum<M>(sh.cnt + MM, Kc.g + MM, Kc.t + MM, d1, (int)p, (int)q)));
-                if (S > 2) Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[2], shell_sum<M>(sh.cnt + 2 * MM, Kc.g + 2 * MM, Kc.t + 2 * MM, d2, (int)p, (int)q)));
+                if (S > 1 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
+                    d1 = shell(zq0, zq1, P.m_self[1]);
+                    Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[1], shell_sum<M, SYM>(sh.cnt + MM, Kc.g + MM, Kc.t + MM, d1, (int)p, (int)q)));
+                    if (S > 2 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
+                        d2 = shell(zq1, zq2, P.m_self[2]);
+                        Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[2], shell_sum<M, SYM>(sh.cnt + 2 * MM, Kc.g + 2 * MM, Kc.t + 2 * MM, d2, (int)p, (int)q)));
+                    } else if (S > 2) {
+                        Jk = J_cur;                       // pruned: not improving
+                    }
+                } else if (S > 1) {
+                    Jk = J_cur;
+                }
                 if (Jk < J_cur && win_key == kNoKey) {
                     win_key = key; win_a = a; win_b = b; win_pq = p | (q << 8);
                     win_d0 = d0; win_d1 = d1; win_d2 = d2; win_J = Jk;
@@ -413,7 +436,7 @@ mc_window_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const M
 }
 
 // query != nullptr: no launch, *query = how many clusters of A.R blocks of this shape can be resident at once.
-template <int M, int OCC>
+template <int M, int OCC, bool SYM>
 cudaError_t launch_one(const KParams& P, const DevTables& host_tab, const McArgs& A, int64_t C, int threads,
                        size_t smem, cudaStream_t st, int* query)
 {
@@ -424,7 +447,7 @@ cudaError_t launch_one(const KParams& P, const DevTables& host_tab, const McArgs
             Kc.t[s * M * M + i] = s < P.S ? host_tab.t[s * M * M + i] : 0.0;
         }
     for (int s = 0; s < 4; ++s) Kc.w[s] = host_tab.w[s];
-    auto kern = mc_window_kernel<M, OCC>;
+    auto kern = mc_window_kernel<M, OCC, SYM>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
@@ -443,15 +466,23 @@ cudaError_t launch_one(const KParams& P, const DevTables& host_tab, const McArgs
     return cudaLaunchKernelEx(&cfg, kern, P, Kc, A);
 }
 
-template <int M>
+template <int M, bool SYM>
 cudaError_t launch_occ(int occ_mode, const KParams& P, const DevTables& host_tab, const McArgs& A, int64_t C,
                        int threads, size_t smem, cudaStream_t st, int* query)
 {
     switch (occ_mode) {
-        case OCC_SMEM_U8: return launch_one<M, OCC_SMEM_U8>(P, host_tab, A, C, threads, smem, st, query);
-        case OCC_SMEM_NIB: return launch_one<M, OCC_SMEM_NIB>(P, host_tab, A, C, threads, smem, st, query);
-        default: return launch_one<M, OCC_GLOBAL>(P, host_tab, A, C, threads, smem, st, query);
+        case OCC_SMEM_U8: return launch_one<M, OCC_SMEM_U8, SYM>(P, host_tab, A, C, threads, smem, st, query);
+        case OCC_SMEM_NIB: return launch_one<M, OCC_SMEM_NIB, SYM>(P, host_tab, A, C, threads, smem, st, query);
+        default: return launch_one<M, OCC_GLOBAL, SYM>(P, host_tab, A, C, threads, smem, st, query);
     }
+}
+
+template <int M>
+cudaError_t launch_sym(bool sym, int occ_mode, const KParams& P, const DevTables& host_tab, const McArgs& A, int64_t C,
+                       int threads, size_t smem, cudaStream_t st, int* query)
+{
+    return sym ? launch_occ<M, true>(occ_mode, P, host_tab, A, C, threads, smem, st, query)
+               : launch_occ<M, false>(occ_mode, P, host_tab, A, C, threads, smem, st, query);
 }
 
 }  // namespace
@@ -477,16 +508,27 @@ cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode,
     A.stats_all = reinterpret_cast<unsigned long long*>(stats);
     A.log_all = reinterpret_cast<unsigned long long*>(log);
     A.log_cap = log_cap; A.K = K; A.R = cluster; A.w_max = w_max; A.fast_nbr = fast_nbr ? 1 : 0;
+    // exact pruning needs every shell term to be >= 0; the symmetric evaluation needs t_ij == t_ji bit for bit
+    bool sym = true;
+    A.prune = 1;
+    for (int s = 0; s < P.S; ++s) {
+        if (!(host_tab.w[s] >= 0.0)) A.prune = 0;
+        for (int i = 0; i < P.M; ++i)
+            for (int j = 0; j < i; ++j) {
+                const double x = host_tab.t[(s * P.M + i) * P.M + j], y = host_tab.t[(s * P.M + j) * P.M + i];
+                if (memcmp(&x, &y, sizeof(double)) != 0) sym = false;
+            }
+    }
     cudaError_t e;
     switch (P.M) {
-        case 1: e = launch_occ<1>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
-        case 2: e = launch_occ<2>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
-        case 3: e = launch_occ<3>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
-        case 4: e = launch_occ<4>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
-        case 5: e = launch_occ<5>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
-        case 6: e = launch_occ<6>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
-        case 7: e = launch_occ<7>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
-        default: e = launch_occ<8>(occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 1: e = launch_sym<1>(sym, occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 2: e = launch_sym<2>(sym, occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 3: e = launch_sym<3>(sym, occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 4: e = launch_sym<4>(sym, occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 5: e = launch_sym<5>(sym, occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 6: e = launch_sym<6>(sym, occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        case 7: e = launch_sym<7>(sym, occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
+        default: e = launch_sym<8>(sym, occ_mode, P, host_tab, A, C, threads, smem, st, query_max_clusters); break;
     }
     if (e == cudaSuccess && !query_max_clusters) ++*n_launches;
     return e;
