@@ -1,0 +1,751 @@
+// hea_mc2.cu -- chain-parallel Monte Carlo local search, second engine ("halo" engine) of hea_mc_run.
+// DESIGN.md D6, D7, D9; Alg. 3, Eq. 4, Eq. 5, Eq. 6.
+//
+// Same algorithm, windows and results as hea_mc.cu (bit-exact trajectories); different data layout and gather:
+//
+//  * The chain's configuration lives in shared memory on a lattice PADDED by one ghost cell on every side
+//    ((Lx+2)(Ly+2)(Lz+2) cells), ghosts holding the periodic images.  Every neighbour of every real site is then
+//    `padded index + constant`, the constants depending only on the basis index of the site: no interior/boundary
+//    distinction, no neighbour-table traffic in the kernel.  An accepted move also rewrites the ghost images (rare).
+//  * A site is stored ONE-HOT (bit r = species r): a byte per site, or a nibble per site when M <= 4 and the bytes
+//    do not fit (c4: 296,352 padded sites -> 148 KB).  A gather drops the loaded code into a byte slot of an
+//    accumulator word (one IMAD); species counts of a shell come from (acc >> r) & 0x01010101 summed over the words
+//    and one multiply by 0x01010101 -- no per-neighbour shift-by-species, no compare.
+//  * Whether b is a neighbour of a (the exclusion of D9.2) comes from the lattice coordinates of the two sites
+//    (minimum-image displacement, squared length == shell distance), not from a compare per table entry.
+//  * Shell sizes and the basis count are template constants (fcc 12/6/24, bcc 8/6/12), so every gather is unrolled.
+#include <cstring>
+
+#include "hea_device.cuh"
+#include "hea_mc_common.cuh"
+
+namespace hea {
+
+namespace {
+
+enum { OCC2_U8 = 1, OCC2_NIB = 2 };
+
+template <int LAT> struct LatC;
+template <> struct LatC<0> { static constexpr int A = 4, lgA = 2, z0 = 12, z1 = 6, z2 = 24; };   // fcc
+template <> struct LatC<1> { static constexpr int A = 2, lgA = 1, z0 = 8, z1 = 6, z2 = 12; };    // bcc
+__host__ __device__ constexpr int pad4(int x) { return (x + 3) & ~3; }
+template <int LAT> __host__ __device__ constexpr int zpad() { return pad4(LatC<LAT>::z0) + pad4(LatC<LAT>::z1) + pad4(LatC<LAT>::z2); }
+
+// Lattice geometry of the padded layout (kernel parameter).
+struct Geo {
+    int L[3];
+    uint32_t magy, magz;          // floor(2^32 / Ly), floor(2^32 / Lz) (0xFFFFFFFF for a divisor of 1): quotient off by <= 1
+    uint32_t pmagy, pmagz;        // the same for the padded counts Ly + 2, Lz + 2
+    int PLy, PLz;                 // padded cell counts L + 2
+    int NP;                       // padded sites
+    uint32_t basis;               // bit 3b + d = doubled coordinate d of basis site b
+    int d2[3];                    // squared shell distances in doubled units
+    int distinct;                 // every L >= 3: a site pair is joined by at most one lattice vector of a shell
+};
+
+struct Sh2 {
+    int cnt[kSMM];
+    double J;
+    unsigned long long n_accept, n_null, hash, last_accept, n_logged;
+    uint32_t best[3];
+    uint32_t team_key;            // minimum key over the team (TEAM windows)
+    unsigned long long bc_t0;     // follower: broadcast of the leader's phase record
+    double bc_J;
+    uint32_t bc_W, pad;
+    MoveRec rec;
+};
+
+struct SiteC {
+    uint32_t pidx;                // padded site index
+    int x, y, z, b;               // cell coordinates and basis index
+};
+
+template <int LAT>
+__device__ __forceinline__ SiteC decode_site(const Geo& G, uint32_t a)
+{
+    SiteC s;
+    const uint32_t cell = a >> LatC<LAT>::lgA;
+    s.b = (int)(a & (uint32_t)(LatC<LAT>::A - 1));
+    uint32_t q1 = __umulhi(cell, G.magz);
+    uint32_t z = cell - q1 * (uint32_t)G.L[2];
+    if (z >= (uint32_t)G.L[2]) { z -= (uint32_t)G.L[2]; ++q1; }
+    uint32_t q2 = __umulhi(q1, G.magy);
+    uint32_t y = q1 - q2 * (uint32_t)G.L[1];
+    if (y >= (uint32_t)G.L[1]) { y -= (uint32_t)G.L[1]; ++q2; }
+    s.x = (int)q2; s.y = (int)y; s.z = (int)z;
+    s.pidx = ((((q2 + 1u) * (uint32_t)G.PLy + (y + 1u)) * (uint32_t)G.PLz + (z + 1u)) << LatC<LAT>::lgA) | (uint32_t)s.b;
+    return s;
+}
+
+template <int OCC>
+__device__ __forceinline__ uint32_t occ_get(const uint8_t* s_occ, uint32_t pidx)
+{
+    if (OCC == OCC2_NIB) return ((uint32_t)s_occ[pidx >> 1] >> ((pidx & 1u) * 4u)) & 0xFu;
+    return s_occ[pidx];
+}
+
+template <int OCC>
+__device__ __forceinline__ void occ_set(uint8_t* s_occ, uint32_t pidx, uint32_t onehot)
+{
+    if (OCC == OCC2_NIB) {
+        const uint32_t sh = (pidx & 1u) * 4u;
+        s_occ[pidx >> 1] = (uint8_t)((s_occ[pidx >> 1] & ~(0xFu << sh)) | (onehot << sh));
+    } else {
+        s_occ[pidx] = (uint8_t)onehot;
+    }
+}
+
+// One-hot codes of the ZS neighbours of a site in one shell, four byte slots per accumulator word.
+// Table entries: OCC2_U8 -> padded index offset; OCC2_NIB -> 8 * byte offset + nibble shift (relative to the byte
+// pair of the site, see the table build).
+template <int OCC, int ZS>
+__device__ __forceinline__ void gather_shell(const uint8_t* __restrict__ s_occ, const int4* __restrict__ trow, uint32_t pidx,
+                                             uint32_t (&acc)[(ZS + 3) / 4])
+{
+    const uint32_t base = OCC == OCC2_NIB ? (pidx & ~1u) << 2 : pidx;
+#pragma unroll
+    for (int g = 0; g < (ZS + 3) / 4; ++g) {
+        const int4 o = trow[g];
+        uint32_t w = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (g * 4 + j < ZS) {
+                const int oj = j == 0 ? o.x : j == 1 ? o.y : j == 2 ? o.z : o.w;
+                const uint32_t t = base + (uint32_t)oj;
+                uint32_t x;
+                if (OCC == OCC2_NIB) x = (uint32_t)s_occ[t >> 3] >> (t & 4u);
+                else x = s_occ[t];
+                w += x << (8 * j);
+            }
+        }
+        if (OCC == OCC2_NIB) w &= 0x0F0F0F0Fu;
+        acc[g] = w;
+    }
+}
+
+// F[r] = #(neighbours of b of species r) - #(neighbours of a of species r) from the slot accumulators.
+template <int M, int NA>
+__device__ __forceinline__ void hist_diff(const uint32_t (&accA)[NA], const uint32_t (&accB)[NA], int (&F)[M])
+{
+    int last = 0;
+#pragma unroll
+    for (int r = 0; r < M - 1; ++r) {
+        uint32_t x = (uint32_t)NA * 0x01010101u;             // per-byte bias: the byte sums stay in [0, 2 NA]
+#pragma unroll
+        for (int g = 0; g < NA; ++g) x += ((accB[g] >> r) & 0x01010101u) - ((accA[g] >> r) & 0x01010101u);
+        F[r] = (int)((x * 0x01010101u) >> 24) - 4 * NA;
+        last -= F[r];
+    }
+    F[M - 1] = last;                                          // both sites have z_s entries: the differences sum to 0
+}
+
+// One shell's contribution in the D6 order, from the species-count differences F (see shell_sum in hea_mc_common.cuh).
+template <int M, bool SYM>
+__device__ __forceinline__ double shell_sum_F(const int* __restrict__ cnt, const double* __restrict__ g,
+                                              const double* __restrict__ t, const int (&F)[M], const int (&c)[M])
+{
+    double up[M * M];
+    double sh = 0.0;
+#pragma unroll
+    for (int i = 0; i < M; ++i) {
+        double row = 0.0;
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            double e;
+            if (SYM && j < i) {
+                e = up[j * M + i];
+            } else {
+                const int n = cnt[i * M + j] + c[i] * F[j] + c[j] * F[i];
+                e = sq_dev(n, g[i * M + j], t[i * M + j]);
+                if (SYM && j > i) up[i * M + j] = e;
+            }
+            row = __dadd_rn(row, e);
+        }
+        sh = __dadd_rn(sh, row);
+    }
+    return sh;
+}
+
+template <int M>
+__device__ __forceinline__ typename Pack<M>::W pack_F(const int (&F)[M])
+{
+    typename Pack<M>::W d = 0;
+#pragma unroll
+    for (int r = 0; r < M; ++r) d |= (typename Pack<M>::W)(uint32_t)(F[r] + Pack<M>::kHalf) << (Pack<M>::FB * r);
+    return d;
+}
+
+// ---- teams: R blocks per chain, synchronised through global memory (cooperative launch, all blocks co-resident)
+//
+// Few chains cannot fill 148 SMs with one block each, so a chain may be given a TEAM of R blocks, every block holding
+// a replica of the chain state.  Windows run in one of two modes that all blocks of a team derive from the same
+// history:
+//   TEAM  the W*K candidates of the window are spread over the R*T threads; every block posts its best record into
+//         its slot of the chain's control block and reads all R slots (release/acquire through L2), then every replica
+//         applies the same move.  Worth its ~1-2 us exchange only when a window is several rounds of one block.
+//   SOLO  block 0 (the leader) runs the windows alone -- in the accept regime a window is a fraction of one round and
+//         extra blocks only add latency; the followers wait on the control block.  When the windows have grown, the
+//         leader writes the state back, posts a phase record, and the followers reload and join.
+constexpr int kMaxTeam = 32;
+constexpr int kTeamRounds = 32;             // candidates per thread per TEAM window (the null mask has 64 bits)
+
+struct TeamSlot {                 // 64 bytes
+    uint32_t seq;                 // team-window number + 1 when the record below is valid
+    uint32_t key, a, b, pq, pad;
+    double J;
+    uint64_t d[3];
+};
+
+struct TeamCtl {
+    uint32_t phase_seq;           // number of phase records posted by the leader
+    uint32_t W;                   // window length (steps) to continue with
+    unsigned long long t0;        // next step
+    double J;
+    uint32_t pad[10];
+    TeamSlot slot[2][kMaxTeam];   // [team-window parity][rank]
+};
+
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p)
+{
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ void st_release_u32(uint32_t* p, uint32_t v)
+{
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+struct Mc2Args {
+    McArgs a;                     // a.R = blocks per chain
+    Geo G;
+    TeamCtl* team;                // [C] control blocks, zeroed before the launch (R > 1 only)
+    int team_on, team_off;        // enter TEAM when W*K >= team_on; leave it after a move with steps_done*K < team_off
+};
+
+// Shared memory: occupancy (offset 0, so a gather address is the loaded offset itself) | Sh2 | offset table [A][ZP].
+template <int M, int OCC, bool SYM, int LAT>
+__global__ void __launch_bounds__(1024)
+mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __grid_constant__ Mc2Args AA)
+{
+    extern __shared__ __align__(16) uint8_t s_raw[];
+    using LC = LatC<LAT>;
+    constexpr int ZP = zpad<LAT>();
+    constexpr int NA0 = (LC::z0 + 3) / 4, NA1 = (LC::z1 + 3) / 4, NA2 = (LC::z2 + 3) / 4;
+    constexpr int MM = M * M;
+    using PW = typename Pack<M>::W;
+    const McArgs& A = AA.a;
+    const Geo& G = AA.G;
+    const uint32_t occ_bytes = (uint32_t)(((OCC == OCC2_NIB ? (G.NP + 1) / 2 : G.NP) + 15) & ~15);
+    uint8_t* s_occ = s_raw;
+    Sh2& sh = *reinterpret_cast<Sh2*>(s_raw + occ_bytes);
+    int* s_tab = reinterpret_cast<int*>(s_raw + occ_bytes + ((sizeof(Sh2) + 15) & ~(size_t)15));
+
+    const int tid = threadIdx.x, T = blockDim.x;
+    const int S = P.S, N = P.N, K = A.K, R = A.R;
+    const int SMM = S * MM;
+    const uint32_t rank = R > 1 ? blockIdx.x % (unsigned)R : 0u;
+    const size_t chain_local = R > 1 ? blockIdx.x / (unsigned)R : blockIdx.x;
+    uint8_t* g_occ = A.occ_all + chain_local * (size_t)N;
+    int32_t* g_cnt = A.counts_all + chain_local * (size_t)SMM;
+    unsigned long long* g_stats = A.stats_all + chain_local * 5;
+    TeamCtl* ctl = R > 1 ? AA.team + chain_local : nullptr;
+    const uint32_t chain = (uint32_t)(A.chain0 + chain_local);
+    const uint32_t key0 = (uint32_t)A.seed, key1 = (uint32_t)(A.seed >> 32);
+    const int Lx = G.L[0], Ly = G.L[1], Lz = G.L[2];
+
+    // counts and the padded one-hot configuration from global memory (L2 loads: a leader may just have written them)
+    auto load_state = [&]() {
+        for (int i = tid; i < SMM; i += T) sh.cnt[i] = __ldcg(g_cnt + i);
+        auto code_of = [&](int pi) -> uint32_t {           // one-hot code of padded site pi (ghosts = periodic images)
+            if (pi >= G.NP) return 0u;
+            const int b = pi & (LC::A - 1);
+            const uint32_t cell = (uint32_t)pi >> LC::lgA;
+            uint32_t q1 = __umulhi(cell, G.pmagz);
+            int pz = (int)(cell - q1 * (uint32_t)G.PLz);
+            if (pz >= G.PLz) { pz -= G.PLz; ++q1; }
+            uint32_t q2 = __umulhi(q1, G.pmagy);
+            int py = (int)(q1 - q2 * (uint32_t)G.PLy);
+            if (py >= G.PLy) { py -= G.PLy; ++q2; }
+            const int px = (int)q2;
+            const int x = px == 0 ? Lx - 1 : px == Lx + 1 ? 0 : px - 1;
+            const int y = py == 0 ? Ly - 1 : py == Ly + 1 ? 0 : py - 1;
+            const int z = pz == 0 ? Lz - 1 : pz == Lz + 1 ? 0 : pz - 1;
+            const int site = (((x * Ly + y) * Lz + z) << LC::lgA) | b;
+            return 1u << __ldcg(g_occ + site);
+        };
+        if (OCC == OCC2_NIB) {
+            for (int i = tid; i < (G.NP + 1) / 2; i += T) s_occ[i] = (uint8_t)(code_of(2 * i) | (code_of(2 * i + 1) << 4));
+        } else {
+            for (int i = tid; i < G.NP; i += T) s_occ[i] = (uint8_t)code_of(i);
+        }
+    };
+    auto store_state = [&]() {
+        for (int i = tid; i < N; i += T) {
+            const SiteC sc = decode_site<LAT>(G, (uint32_t)i);
+            g_occ[i] = (uint8_t)(31 - __clz((int)occ_get<OCC>(s_occ, sc.pidx)));
+        }
+        for (int i = tid; i < SMM; i += T) g_cnt[i] = sh.cnt[i];
+    };
+
+    // ---- prologue
+    load_state();
+    for (int i = tid; i < LC::A * ZP; i += T) {
+        const int b = i / ZP, slot = i - b * ZP;
+        int s, e;
+        if (slot < pad4(LC::z0)) { s = 0; e = slot; }
+        else if (slot < pad4(LC::z0) + pad4(LC::z1)) { s = 1; e = slot - pad4(LC::z0); }
+        else { s = 2; e = slot - pad4(LC::z0) - pad4(LC::z1); }
+        const int zs = s == 0 ? LC::z0 : s == 1 ? LC::z1 : LC::z2;
+        int entry = 0;
+        if (s < S && e < zs) {
+            const int8_t* st = P.tab->stencil + (b * P.Z + P.zoff[s] + e) * 4;     // (nb, sx, sy, sz)
+            const int off = ((((int)st[1] * G.PLy + (int)st[2]) * G.PLz + (int)st[3]) << LC::lgA) + ((int)st[0] - b);
+            if (OCC == OCC2_NIB) {
+                const int tt = (b & 1) + off;                 // padded index parity of the site == b & 1 (A is even)
+                entry = (tt >> 1) * 8 + (tt & 1) * 4;         // byte offset * 8 + nibble shift
+            } else {
+                entry = off;
+            }
+        }
+        s_tab[i] = entry;
+    }
+    if (tid == 0) {
+        sh.n_accept = g_stats[0]; sh.n_null = 0; sh.hash = g_stats[2]; sh.last_accept = g_stats[3]; sh.n_logged = 0;
+        sh.best[0] = sh.best[1] = sh.best[2] = kNoKey;
+        sh.rec.key = kNoKey;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double J = 0.0;
+        for (int s = 0; s < S; ++s)
+            J = __dadd_rn(J, __dmul_rn(Kc.w[s], shell_sum<M, false>(sh.cnt + s * MM, Kc.g + s * MM, Kc.t + s * MM, Pack<M>::bias(), 0, 0)));
+        sh.J = J;
+    }
+    __syncthreads();
+
+    const int32_t* __restrict__ nbr = P.nbr_site;
+    const bool prune = A.prune != 0;
+
+    // candidate c of a window (ordered by (step, k)) belongs to thread gtid = c mod GT; GT depends on the mode
+    bool team = false;                                       // every chain starts SOLO with W = 1
+    uint32_t GT, gtid, ts_first, k_first, ts_inc, k_inc, w_cap;
+    auto set_mode = [&](bool tm) {
+        team = tm;
+        GT = tm ? (uint32_t)T * (uint32_t)R : (uint32_t)T;
+        gtid = tm ? (uint32_t)tid * (uint32_t)R + rank : (uint32_t)tid;
+        ts_first = gtid / (uint32_t)K; k_first = gtid - ts_first * (uint32_t)K;
+        ts_inc = GT / (uint32_t)K; k_inc = GT - ts_inc * (uint32_t)K;
+        w_cap = (uint32_t)min((uint64_t)(1u << 20), ((uint64_t)(tm ? kTeamRounds : kMaxRounds) * GT) / (uint32_t)K);
+        if (w_cap < 1u) w_cap = 1u;
+        if (w_cap > (uint32_t)A.w_max) w_cap = (uint32_t)A.w_max;
+    };
+    set_mode(false);
+
+    unsigned long long t0 = A.step0;
+    const unsigned long long t_end = A.step0 + A.n_steps;
+    uint32_t W = 1;
+    unsigned long long my_null = 0;
+    uint32_t it = 0;                                         // windows evaluated by this block
+    uint32_t tw = 0;                                         // TEAM windows so far (same in every block of the team)
+    uint32_t phase = 0;                                      // phase records consumed / posted
+
+    while (t0 < t_end) {
+        if (R > 1 && !team && rank != 0) {
+            // ---- follower in a SOLO phase: wait for the leader's phase record, reload, join the team
+            if (tid == 0) {
+                while (ld_acquire_u32(&ctl->phase_seq) != phase + 1u) __nanosleep(256);
+                sh.bc_W = __ldcg(&ctl->W);                   // broadcast through shared memory
+                sh.bc_t0 = __ldcg(&ctl->t0);
+                sh.J = __ldcg(&ctl->J);
+            }
+            __syncthreads();
+            ++phase;
+            W = sh.bc_W;
+            t0 = sh.bc_t0;
+            if (t0 >= t_end) break;
+            load_state();
+            set_mode(true);
+            __syncthreads();
+            continue;
+        }
+        const uint32_t Wc = (uint32_t)min((unsigned long long)W, t_end - t0);
+        const int buf = (int)(it % 3u);
+        volatile uint32_t* best_slot = &sh.best[buf];
+        const double J_cur = sh.J;
+        uint32_t win_key = kNoKey, win_a = 0, win_b = 0, win_pq = 0;
+        PW win_d0 = 0, win_d1 = 0, win_d2 = 0;
+        double win_J = 0.0;
+        uint64_t nullmask = 0;
+
+        uint32_t ts = ts_first, k = k_first;
+        for (int j = 0; ts < Wc; ++j) {
+            const uint32_t hint = *best_slot;
+            if ((hint >> 10) < ts) break;                       // a move at an earlier step exists: this step is void
+            const uint32_t key = (ts << 10) | k;
+            // ---- D9.1 proposal
+            const unsigned long long step = t0 + ts;
+            const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), k, chain, key0, key1);
+            uint32_t a = __umulhi(r.x, (uint32_t)N), b = __umulhi(r.y, (uint32_t)N - 1u);
+            b += (b >= a);
+            SiteC sa = decode_site<LAT>(G, a), sb = decode_site<LAT>(G, b);
+            uint32_t hp = occ_get<OCC>(s_occ, sa.pidx), hq = occ_get<OCC>(s_occ, sb.pidx);
+            if (hp == hq) {
+                a = __umulhi(r.z, (uint32_t)N); b = __umulhi(r.w, (uint32_t)N - 1u);
+                b += (b >= a);
+                sa = decode_site<LAT>(G, a); sb = decode_site<LAT>(G, b);
+                hp = occ_get<OCC>(s_occ, sa.pidx); hq = occ_get<OCC>(s_occ, sb.pidx);
+            }
+            if (hp == hq) {
+                nullmask |= 1ull << j;
+            } else if (key < hint) {                             // same step, higher k than a known move: only nullness counts
+                const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+                int c[M];
+#pragma unroll
+                for (int r2 = 0; r2 < M; ++r2) c[r2] = (r2 == p) - (r2 == q);
+                // ---- D9.2: is b an entry of a's rows?  (excluded sum = plain sum + (m - m_self)(e_q - e_p))
+                int mm0 = 0, mm1 = 0, mm2 = 0;
+                if (G.distinct) {
+                    const int dx = 2 * (sb.x - sa.x) + (int)((G.basis >> (3 * sb.b)) & 1u) - (int)((G.basis >> (3 * sa.b)) & 1u);
+                    const int dy = 2 * (sb.y - sa.y) + (int)((G.basis >> (3 * sb.b + 1)) & 1u) - (int)((G.basis >> (3 * sa.b + 1)) & 1u);
+                    const int dz = 2 * (sb.z - sa.z) + (int)((G.basis >> (3 * sb.b + 2)) & 1u) - (int)((G.basis >> (3 * sa.b + 2)) & 1u);
+                    const int wx = dx > Lx ? dx - 2 * Lx : dx < -Lx ? dx + 2 * Lx : dx;
+                    const int wy = dy > Ly ? dy - 2 * Ly : dy < -Ly ? dy + 2 * Ly : dy;
+                    const int wz = dz > Lz ? dz - 2 * Lz : dz < -Lz ? dz + 2 * Lz : dz;
+                    const int r2 = wx * wx + wy * wy + wz * wz;
+                    mm0 = r2 == G.d2[0]; mm1 = r2 == G.d2[1]; mm2 = r2 == G.d2[2];
+                } else {
+                    const int32_t* row = nbr + (size_t)a * P.Z;
+                    for (int e = 0; e < P.Z; ++e) {
+                        const int hit = (uint32_t)__ldg(row + e) == b;
+                        if (e < P.zoff[1]) mm0 += hit; else if (e < P.zoff[2]) mm1 += hit; else mm2 += hit;
+                    }
+                    mm0 -= P.m_self[0]; mm1 -= P.m_self[1]; mm2 -= P.m_self[2];
+                }
+                const int4* ta = reinterpret_cast<const int4*>(s_tab + sa.b * ZP);
+                const int4* tb = reinterpret_cast<const int4*>(s_tab + sb.b * ZP);
+                // ---- D6 objective from counts + delta, shell by shell with the exact lower-bound pruning (hea_mc.cu)
+                int F0[M], F1[M], F2[M];
+#pragma unroll
+                for (int r2 = 0; r2 < M; ++r2) { F1[r2] = 0; F2[r2] = 0; }
+                {
+                    uint32_t xa[NA0], xb[NA0];
+                    gather_shell<OCC, LC::z0>(s_occ, ta, sa.pidx, xa);
+                    gather_shell<OCC, LC::z0>(s_occ, tb, sb.pidx, xb);
+                    hist_diff<M, NA0>(xa, xb, F0);
+#pragma unroll
+                    for (int r2 = 0; r2 < M; ++r2) F0[r2] -= mm0 * c[r2];
+                }
+                double Jk = __dmul_rn(Kc.w[0], shell_sum_F<M, SYM>(sh.cnt, Kc.g, Kc.t, F0, c));
+                Jk = __dadd_rn(0.0, Jk);
+                if (S > 1 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
+                    {
+                        uint32_t xa[NA1], xb[NA1];
+                        gather_shell<OCC, LC::z1>(s_occ, ta + NA0, sa.pidx, xa);
+                        gather_shell<OCC, LC::z1>(s_occ, tb + NA0, sb.pidx, xb);
+                        hist_diff<M, NA1>(xa, xb, F1);
+#pragma unroll
+                        for (int r2 = 0; r2 < M; ++r2) F1[r2] -= mm1 * c[r2];
+                    }
+                    Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[1], shell_sum_F<M, SYM>(sh.cnt + MM, Kc.g + MM, Kc.t + MM, F1, c)));
+                    if (S > 2 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
+                        {
+                            uint32_t xa[NA2], xb[NA2];
+                            gather_shell<OCC, LC::z2>(s_occ, ta + NA0 + NA1, sa.pidx, xa);
+                            gather_shell<OCC, LC::z2>(s_occ, tb + NA0 + NA1, sb.pidx, xb);
+                            hist_diff<M, NA2>(xa, xb, F2);
+#pragma unroll
+                            for (int r2 = 0; r2 < M; ++r2) F2[r2] -= mm2 * c[r2];
+                        }
+                        Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[2], shell_sum_F<M, SYM>(sh.cnt + 2 * MM, Kc.g + 2 * MM, Kc.t + 2 * MM, F2, c)));
+                    } else if (S > 2) {
+                        Jk = J_cur;                       // pruned: not improving
+                    }
+                } else if (S > 1) {
+                    Jk = J_cur;
+                }
+                if (Jk < J_cur && win_key == kNoKey) {
+                    win_key = key; win_a = a; win_b = b; win_pq = (uint32_t)p | ((uint32_t)q << 8);
+                    win_d0 = pack_F<M>(F0); win_d1 = pack_F<M>(F1); win_d2 = pack_F<M>(F2); win_J = Jk;
+                    atomicMin(&sh.best[buf], key);
+                }
+            }
+            k += k_inc; ts += ts_inc;
+            if (k >= (uint32_t)K) { k -= (uint32_t)K; ++ts; }
+        }
+        __syncthreads();                                        // B1: window evaluated, local minimum posted
+        uint32_t key_best = sh.best[buf];
+        if (tid == 0) sh.best[(buf + 2) % 3] = kNoKey;          // next user of that slot is two barriers away
+
+        const int lane = tid & 31;
+        if (team) {
+            // ---- TEAM exchange: post this block's best record, read all R slots, take the minimum key
+            const int par = (int)(tw & 1u);
+            TeamSlot* slots = ctl->slot[par];
+            const bool owner = key_best != kNoKey && win_key == key_best;
+            if (owner || (key_best == kNoKey && tid == 0)) {
+                TeamSlot* me = slots + rank;
+                me->key = key_best; me->a = win_a; me->b = win_b; me->pq = win_pq; me->J = win_J;
+                me->d[0] = win_d0; me->d[1] = win_d1; me->d[2] = win_d2;
+                __threadfence();
+                st_release_u32(&me->seq, tw + 1u);
+            }
+            if (tid < 32) {
+                uint32_t kk = kNoKey;
+                if (lane < R) {
+                    while (ld_acquire_u32(&slots[lane].seq) != tw + 1u) { }
+                    kk = __ldcg(&slots[lane].key);
+                }
+                uint32_t kmin = kk;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) kmin = min(kmin, __shfl_xor_sync(0xFFFFFFFFu, kmin, o));
+                if (kmin != kNoKey && kk == kmin) {           // keys are unique: exactly one lane
+                    const TeamSlot* src = slots + lane;
+                    MoveRec& m = sh.rec;
+                    m.key = kmin; m.a = __ldcg(&src->a); m.b = __ldcg(&src->b); m.pq = __ldcg(&src->pq);
+                    m.J = __ldcg(&src->J);
+                    m.d[0] = __ldcg(&src->d[0]); m.d[1] = __ldcg(&src->d[1]); m.d[2] = __ldcg(&src->d[2]);
+                }
+                if (lane == 0) sh.team_key = kmin;
+            }
+            __syncthreads();
+            key_best = sh.team_key;
+            ++tw;
+        } else if (key_best != kNoKey) {
+            const uint32_t owner_lane_mask = __ballot_sync(0xFFFFFFFFu, win_key == key_best);
+            if (owner_lane_mask != 0u && lane == __ffs((int)owner_lane_mask) - 1) {
+                MoveRec& m = sh.rec;
+                m.key = key_best; m.a = win_a; m.b = win_b; m.pq = win_pq; m.J = win_J;
+                m.d[0] = win_d0; m.d[1] = win_d1; m.d[2] = win_d2;
+            }
+            __syncthreads();
+        }
+        const MoveRec* mv = &sh.rec;
+
+        // ---- commit: null counts of the committed steps, then the move (D9.4)
+        const uint32_t steps_done = key_best != kNoKey ? (key_best >> 10) + 1u : Wc;
+        if (nullmask) {
+            const uint32_t lim = steps_done * (uint32_t)K;       // candidates c < lim are committed
+            const uint32_t n_comm = gtid < lim ? (lim - 1u - gtid) / GT + 1u : 0u;
+            my_null += __popcll(n_comm >= 64u ? nullmask : (nullmask & ((1ull << n_comm) - 1ull)));
+        }
+        if (key_best != kNoKey) {
+            const int p = (int)(mv->pq & 0xFFu), q = (int)(mv->pq >> 8);
+            for (int idx = tid; idx < SMM; idx += T) {
+                const int s = idx / MM, rem = idx - s * MM, i = rem / M, jj = rem - i * M;
+                const PW d = (PW)mv->d[s];
+                const int ci = (i == p) - (i == q), cj = (jj == p) - (jj == q);
+                sh.cnt[idx] += ci * Pack<M>::field(d, jj) + cj * Pack<M>::field(d, i);
+            }
+            if (tid == T - 1) {                                 // one thread (not among the count updaters when T > SMM)
+                const uint32_t a = mv->a, b = mv->b, kk = key_best & 1023u;
+                const unsigned long long step = t0 + (key_best >> 10);
+                // the swap, on the real sites and on every ghost image of them
+#pragma unroll 1
+                for (int which = 0; which < 2; ++which) {
+                    const SiteC sc = decode_site<LAT>(G, which ? b : a);
+                    const uint32_t code = 1u << (which ? p : q);
+                    const int px[3] = {sc.x + 1, sc.x == Lx - 1 ? 0 : -1, sc.x == 0 ? Lx + 1 : -1};
+                    const int py[3] = {sc.y + 1, sc.y == Ly - 1 ? 0 : -1, sc.y == 0 ? Ly + 1 : -1};
+                    const int pz[3] = {sc.z + 1, sc.z == Lz - 1 ? 0 : -1, sc.z == 0 ? Lz + 1 : -1};
+                    for (int ix = 0; ix < 3; ++ix)
+                        for (int iy = 0; iy < 3; ++iy)
+                            for (int iz = 0; iz < 3; ++iz) {
+                                if (px[ix] < 0 || py[iy] < 0 || pz[iz] < 0) continue;
+                                const uint32_t pi = (uint32_t)((((px[ix] * G.PLy + py[iy]) * G.PLz + pz[iz]) << LC::lgA) | sc.b);
+                                occ_set<OCC>(s_occ, pi, code);
+                            }
+                }
+                sh.J = mv->J;
+                sh.n_accept += 1;
+                sh.last_accept = step;
+                unsigned long long h = sh.hash;
+                h = (h ^ (uint32_t)step) * 0x100000001b3ULL;
+                h = (h ^ (uint32_t)(step >> 32)) * 0x100000001b3ULL;
+                h = (h ^ kk) * 0x100000001b3ULL;
+                h = (h ^ a) * 0x100000001b3ULL;
+                h = (h ^ b) * 0x100000001b3ULL;
+                sh.hash = h;
+                const unsigned long long nl = sh.n_logged;
+                if (rank == 0 && A.log_all != nullptr && (long long)nl < A.log_cap) {
+                    unsigned long long* rec = A.log_all + (chain_local * (size_t)A.log_cap + nl) * 3;
+                    rec[0] = step;
+                    rec[1] = (unsigned long long)kk | ((unsigned long long)a << 32);
+                    rec[2] = (unsigned long long)b;
+                }
+                sh.n_logged = nl + 1;
+            }
+            __syncthreads();
+            W = min(steps_done, w_cap);                         // the observed gap
+        } else {
+            W = min(W * 2u, w_cap);
+        }
+        t0 += steps_done;
+        ++it;
+
+        // ---- mode switches (R > 1): every block of the team takes the same decision from the same history
+        if (R > 1 && t0 < t_end) {
+            if (team) {
+                if (key_best != kNoKey && (unsigned long long)steps_done * (unsigned)K < (unsigned long long)AA.team_off) {
+                    set_mode(false);                            // followers go and wait at the top of the loop
+                    W = min(W, w_cap);
+                }
+            } else if ((unsigned long long)W * (unsigned)K >= (unsigned long long)AA.team_on) {
+                // leader: windows have grown -> write the state back, call the team
+                store_state();
+                __syncthreads();
+                if (tid == 0) {
+                    ctl->W = W; ctl->t0 = t0; ctl->J = sh.J;
+                    __threadfence();
+                    st_release_u32(&ctl->phase_seq, phase + 1u);
+                }
+                ++phase;
+                set_mode(true);
+            }
+        }
+    }
+
+    // ---- epilogue: release waiting followers, write back (rank 0 owns the global copy; nulls are summed over blocks)
+    if (R > 1 && rank == 0 && !team) {
+        __syncthreads();
+        if (tid == 0) {
+            ctl->W = 1; ctl->t0 = t_end; ctl->J = sh.J;
+            __threadfence();
+            st_release_u32(&ctl->phase_seq, phase + 1u);
+        }
+    }
+    if (my_null) atomicAdd(&sh.n_null, my_null);
+    __syncthreads();
+    if (rank == 0) {
+        store_state();
+        if (tid == 0) {
+            g_stats[0] = sh.n_accept;
+            g_stats[2] = sh.hash;
+            g_stats[3] = sh.last_accept;
+            g_stats[4] = (unsigned long long)__double_as_longlong(sh.J);
+        }
+    }
+    if (tid == 0 && sh.n_null) atomicAdd(&g_stats[1], sh.n_null);
+}
+
+template <int M, int OCC, bool SYM, int LAT>
+cudaError_t launch2_one(const KParams& P, const DevTables& host_tab, const Mc2Args& AA, int64_t C, int threads, size_t smem,
+                        cudaStream_t st)
+{
+    McConst<M> Kc;
+    for (int s = 0; s < 3; ++s)
+        for (int i = 0; i < M * M; ++i) {
+            Kc.g[s * M * M + i] = s < P.S ? host_tab.g[s * M * M + i] : 0.0;
+            Kc.t[s * M * M + i] = s < P.S ? host_tab.t[s * M * M + i] : 0.0;
+        }
+    for (int s = 0; s < 4; ++s) Kc.w[s] = host_tab.w[s];
+    auto kern = mc_halo_kernel<M, OCC, SYM, LAT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(C * AA.a.R));
+    cfg.blockDim = dim3((unsigned)threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;            // teams spin on each other: all blocks must be co-resident
+    attr[0].val.cooperative = AA.a.R > 1 ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, P, Kc, AA);
+}
+
+template <int M, int OCC, bool SYM>
+cudaError_t launch2_lat(int lat, const KParams& P, const DevTables& host_tab, const Mc2Args& AA, int64_t C, int threads,
+                        size_t smem, cudaStream_t st)
+{
+    return lat == 0 ? launch2_one<M, OCC, SYM, 0>(P, host_tab, AA, C, threads, smem, st)
+                    : launch2_one<M, OCC, SYM, 1>(P, host_tab, AA, C, threads, smem, st);
+}
+
+template <int M>
+cudaError_t launch2_m(bool sym, int occ_mode, int lat, const KParams& P, const DevTables& host_tab, const Mc2Args& AA,
+                      int64_t C, int threads, size_t smem, cudaStream_t st)
+{
+    if (occ_mode == OCC2_NIB) {
+        if (M > 4) return cudaErrorInvalidValue;            // a nibble holds a one-hot code of at most 4 species
+        constexpr int MN = M > 4 ? 4 : M;
+        return sym ? launch2_lat<MN, OCC2_NIB, true>(lat, P, host_tab, AA, C, threads, smem, st)
+                   : launch2_lat<MN, OCC2_NIB, false>(lat, P, host_tab, AA, C, threads, smem, st);
+    }
+    return sym ? launch2_lat<M, OCC2_U8, true>(lat, P, host_tab, AA, C, threads, smem, st)
+               : launch2_lat<M, OCC2_U8, false>(lat, P, host_tab, AA, C, threads, smem, st);
+}
+
+}  // namespace
+
+// Shared-memory bytes of the halo engine (occ_mode 1 = one-hot bytes, 2 = one-hot nibbles).
+size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L)
+{
+    const int A = lattice == 0 ? 4 : 2;
+    const size_t NP = (size_t)(L[0] + 2) * (L[1] + 2) * (L[2] + 2) * A;
+    size_t s = ((occ_mode == OCC2_NIB ? (NP + 1) / 2 : NP) + 15) & ~(size_t)15;
+    s += (sizeof(Sh2) + 15) & ~(size_t)15;
+    s += sizeof(int) * (size_t)A * (lattice == 0 ? zpad<0>() : zpad<1>());
+    return (s + 15) & ~(size_t)15;
+}
+
+size_t mc2_team_bytes(int64_t C) { return sizeof(TeamCtl) * (size_t)C; }
+
+cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
+                       void* team_ctl, int team_on, int team_off, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
+                       uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches)
+{
+    Mc2Args AA;
+    McArgs& A = AA.a;
+    A.occ_all = occ; A.counts_all = counts;
+    A.n_steps = n_steps; A.seed = seed; A.chain0 = chain0; A.step0 = step0;
+    A.stats_all = reinterpret_cast<unsigned long long*>(stats);
+    A.log_all = reinterpret_cast<unsigned long long*>(log);
+    A.log_cap = log_cap; A.K = K; A.R = team; A.w_max = w_max; A.fast_nbr = 0;
+    AA.team = reinterpret_cast<TeamCtl*>(team_ctl);
+    AA.team_on = team_on > 0 ? team_on : 4 * threads;
+    AA.team_off = team_off > 0 ? team_off : threads;
+    if (team > 1) {
+        if (team > kMaxTeam || !team_ctl) return cudaErrorInvalidValue;
+        cudaError_t em = cudaMemsetAsync(team_ctl, 0, mc2_team_bytes(C), st);
+        if (em != cudaSuccess) return em;
+    }
+    bool sym = true;
+    A.prune = 1;
+    for (int s = 0; s < P.S; ++s) {
+        if (!(host_tab.w[s] >= 0.0)) A.prune = 0;
+        for (int i = 0; i < P.M; ++i)
+            for (int j = 0; j < i; ++j) {
+                const double x = host_tab.t[(s * P.M + i) * P.M + j], y = host_tab.t[(s * P.M + j) * P.M + i];
+                if (memcmp(&x, &y, sizeof(double)) != 0) sym = false;
+            }
+    }
+    Geo& G = AA.G;
+    for (int d = 0; d < 3; ++d) G.L[d] = P.L[d];
+    auto magic = [](int d) { return d == 1 ? 0xFFFFFFFFu : (uint32_t)((1ull << 32) / (uint64_t)d); };
+    G.magy = magic(P.L[1]); G.magz = magic(P.L[2]);
+    G.PLy = P.L[1] + 2; G.PLz = P.L[2] + 2;
+    G.pmagy = magic(G.PLy); G.pmagz = magic(G.PLz);
+    G.NP = (P.L[0] + 2) * G.PLy * G.PLz * P.A;
+    if (lattice == 0) { G.basis = (1u << 4) | (1u << 5) | (1u << 6) | (1u << 8) | (1u << 9) | (1u << 10); G.d2[0] = 2; G.d2[1] = 4; G.d2[2] = 6; }
+    else { G.basis = (1u << 3) | (1u << 4) | (1u << 5); G.d2[0] = 3; G.d2[1] = 4; G.d2[2] = 8; }
+    G.distinct = P.L[0] >= 3 && P.L[1] >= 3 && P.L[2] >= 3;
+    const size_t smem = mc2_shared_bytes(occ_mode, lattice, P.L);
+    cudaError_t e;
+    switch (P.M) {
+        case 1: e = launch2_m<1>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
+        case 2: e = launch2_m<2>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
+        case 3: e = launch2_m<3>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
+        case 4: e = launch2_m<4>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
+        case 5: e = launch2_m<5>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
+        case 6: e = launch2_m<6>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
+        case 7: e = launch2_m<7>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
+        default: e = launch2_m<8>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
+    }
+    if (e == cudaSuccess) ++*n_launches;
+    return e;
+}
+
+}  // namespace hea

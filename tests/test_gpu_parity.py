@@ -162,6 +162,60 @@ def test_mc_parity_candidate_counts(hb, K, threads):
     run_both(hb, w, 3, 40, opts={"mc_threads": threads})
 
 
+# ---- halo engine (hea_mc2.cu): padded one-hot configuration, coordinate-based adjacency
+@pytest.mark.parametrize("lattice,dims,conc,S", LATTICES[:9])
+@pytest.mark.parametrize("occ_mode", [1, 2])
+def test_mc_halo_engine_lattices_including_degenerate_cells(hb, lattice, dims, conc, S, occ_mode):
+    if occ_mode == 2 and len(conc) > 4:
+        pytest.skip("a nibble holds a one-hot code of at most 4 species")
+    w = small(lattice, dims, conc, S, target_seed=11, K=16)
+    run_both(hb, w, 3, 80, opts={"mc_engine": 2, "mc_occ_mode": occ_mode})
+
+
+@pytest.mark.parametrize("threads", [32, 256, 1024])
+@pytest.mark.parametrize("window", [0, 1, 3])
+@pytest.mark.parametrize("occ_mode", [1, 2])
+def test_mc_halo_engine_launch_variants(hb, threads, window, occ_mode):
+    w = small("fcc", (4, 4, 4), [0.2, 0.2, 0.2, 0.4], 3, target_seed=5, K=24, n_steps=400)
+    st = run_both(hb, w, 5, 400, opts={"mc_engine": 2, "mc_threads": threads, "mc_window": window, "mc_occ_mode": occ_mode})
+    assert st["n_accept"].sum() > 50
+
+
+@pytest.mark.parametrize("lattice,dims", [("fcc", (7, 5, 6)), ("bcc", (5, 8, 6)), ("fcc", (3, 3, 9)), ("bcc", (3, 7, 4))])
+def test_mc_halo_engine_reject_regime_and_neighbouring_pairs(hb, lattice, dims):
+    # target 0 on small cells: converges, then long windows; small cells make (a, b) neighbours often (exclusion term)
+    w = small(lattice, dims, [0.25] * 4, 3, K=32, n_steps=2000)
+    st = run_both(hb, w, 3, 2000, log_cap=256, opts={"mc_engine": 2})
+    assert (st["n_accept"] > 10).all()
+
+
+@pytest.mark.parametrize("team", [2, 5, 9])
+@pytest.mark.parametrize("on_off", [(1, 1), (64, 32), (512, 128), (0, 0)])
+@pytest.mark.parametrize("occ_mode", [1, 2])
+def test_mc_halo_engine_teams(hb, team, on_off, occ_mode):
+    # R blocks per chain through global memory; (1, 1) = always TEAM, small thresholds = frequent SOLO <-> TEAM switches
+    w = small("fcc", (4, 4, 4), [0.2, 0.2, 0.2, 0.4], 3, target_seed=5, K=24, n_steps=600)
+    opts = {"mc_engine": 2, "mc_team": team, "mc_occ_mode": occ_mode, "mc_threads": 64}
+    if on_off[0]:
+        opts.update({"mc_team_on": on_off[0], "mc_team_off": on_off[1]})
+    st = run_both(hb, w, 5, 600, opts=opts)
+    assert st["n_accept"].sum() > 50
+
+
+@pytest.mark.parametrize("team,threads", [(4, 256), (9, 1024), (32, 32)])
+def test_mc_halo_engine_teams_reject_regime(hb, team, threads):
+    w = small("bcc", (6, 6, 6), [0.25] * 4, 3, K=32, n_steps=3000)
+    st = run_both(hb, w, 3, 3000, log_cap=256, opts={"mc_engine": 2, "mc_team": team, "mc_threads": threads})
+    assert (st["n_accept"] > 20).all()
+
+
+def test_mc_halo_engine_c3_c4_prefix(hb):
+    st = run_both(hb, wl.config(3), 4, 300, log_cap=300, opts={"mc_engine": 2})
+    assert (st["n_accept"] > 250).all()
+    st = run_both(hb, wl.config(4), 3, 300, log_cap=300, opts={"mc_engine": 2})
+    assert (st["n_accept"] > 250).all()
+
+
 def test_mc_c1_full(hb):
     w = wl.config(1)                                        # 64 chains x 10,000 steps x K=32, target 0
     st = run_both(hb, w, w.n_chains, w.n_steps, log_cap=64)
