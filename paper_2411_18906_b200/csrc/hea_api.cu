@@ -26,7 +26,7 @@ cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode,
 size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L);
 size_t mc2_team_bytes(int64_t C);
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
-                       void* team_ctl, int team_on, int team_off, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
+                       void* team_ctl, int team_on, int team_off, int accept_engine, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
                        uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches);
 }  // namespace hea
 
@@ -43,7 +43,7 @@ struct hea_ctx {
     int64_t* d_nps = nullptr;
     hea::KParams P{};
     // tuning options (0 = auto)
-    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0, opt_neighbors = 0, opt_engine = 0, opt_team = 0, opt_team_on = 0, opt_team_off = 0, opt_sro_stages = 0, opt_sro_bps = 0, opt_sro_warps = 0;
+    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0, opt_neighbors = 0, opt_engine = 0, opt_team = 0, opt_team_on = 0, opt_team_off = 0, opt_accept = 0, opt_sro_stages = 0, opt_sro_bps = 0, opt_sro_warps = 0;
     int64_t n_launches = 0;
     // internal stream and scratch for the *_host entry points
     cudaStream_t stream = nullptr;
@@ -103,6 +103,7 @@ int64_t* option_slot(hea_ctx* ctx, const char* name)
     if (!strcmp(name, "mc_neighbors")) return &ctx->opt_neighbors;
     if (!strcmp(name, "mc_engine")) return &ctx->opt_engine;
     if (!strcmp(name, "mc_team")) return &ctx->opt_team;
+    if (!strcmp(name, "mc_accept")) return &ctx->opt_accept;
     if (!strcmp(name, "mc_team_on")) return &ctx->opt_team_on;
     if (!strcmp(name, "mc_team_off")) return &ctx->opt_team_off;
     if (!strcmp(name, "sro_stages")) return &ctx->opt_sro_stages;
@@ -121,6 +122,7 @@ bool option_value_ok(const char* name, int64_t v)
     if (!strcmp(name, "mc_neighbors")) return v == 1 || v == 2;
     if (!strcmp(name, "mc_engine")) return v == 1 || v == 2;
     if (!strcmp(name, "mc_team")) return v >= 1 && v <= 32;
+    if (!strcmp(name, "mc_accept")) return v == 1 || v == 2;
     if (!strcmp(name, "mc_team_on") || !strcmp(name, "mc_team_off")) return v >= 1 && v <= (1 << 30);
     if (!strcmp(name, "sro_stages")) return v >= 1 && v <= 8;
     if (!strcmp(name, "sro_blocks_per_sm")) return v >= 1 && v <= 4;
@@ -370,7 +372,17 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
     // ---- launch configuration (results never depend on it)
     int occ_mode = (int)ctx->opt_occ_mode;
     const size_t budget = ctx->smem_optin;
-    if (ctx->opt_engine == 2) {
+    // engine: 2 = halo engine (hea_mc2.cu) whenever the padded one-hot configuration fits in shared memory and no
+    // option specific to the window engine (clusters, table neighbours, global occupancy) is set; else 1 (hea_mc.cu)
+    int engine = (int)ctx->opt_engine;
+    if (engine == 0) {
+        const bool fits = hea::mc2_shared_bytes(1, ctx->lat.type, ctx->P.L) <= budget ||
+                          (ctx->M <= 4 && hea::mc2_shared_bytes(2, ctx->lat.type, ctx->P.L) <= budget);
+        const bool fits_req = occ_mode == 0 || (occ_mode == 1 && hea::mc2_shared_bytes(1, ctx->lat.type, ctx->P.L) <= budget) ||
+                              (occ_mode == 2 && ctx->M <= 4 && hea::mc2_shared_bytes(2, ctx->lat.type, ctx->P.L) <= budget);
+        engine = (fits && fits_req && ctx->opt_cluster == 0 && ctx->opt_neighbors == 0) ? 2 : 1;
+    }
+    if (engine == 2) {
         // halo engine (hea_mc2.cu): one block per chain, padded one-hot configuration in shared memory
         int om = occ_mode;
         if (om == 0) om = hea::mc2_shared_bytes(1, ctx->lat.type, ctx->P.L) <= budget ? 1 : 2;
@@ -380,12 +392,13 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
         // chains alone would leave at least half of the SMs idle; one block per SM then
         int team = (int)ctx->opt_team;
         if (team == 0) team = (int)std::max<int64_t>(1, std::min<int64_t>(32, ctx->n_sms / C));
-        if ((int64_t)team * C > ctx->n_sms) return fail(HEA_EINVAL, "mc_team: team blocks * chains exceeds the SM count");
-        int threads = ctx->opt_threads ? (int)ctx->opt_threads : 1024;
+        if (team > 1 && (int64_t)team * C > ctx->n_sms) return fail(HEA_EINVAL, "mc_team: team blocks * chains exceeds the SM count");
+        int threads = ctx->opt_threads ? (int)ctx->opt_threads : 512;
         if (!ctx->opt_threads && team == 1) {
             const int64_t blocks_per_sm = (C + ctx->n_sms - 1) / ctx->n_sms;
-            threads = std::max(32, std::min(1024, floor_pow2(std::max<int64_t>(1, 1024 / blocks_per_sm))));
+            threads = std::max(32, std::min(512, floor_pow2(std::max<int64_t>(1, 1024 / blocks_per_sm))));
         }
+        threads = std::min(threads, 512);                   // the halo kernel is compiled for blocks of <= 512 threads
         void* team_ctl = nullptr;
         if (team > 1) {
             int rc = ensure_scratch(ctx, 5, hea::mc2_team_bytes(C));
@@ -394,7 +407,7 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
         }
         const int w_max2 = ctx->opt_window ? (int)ctx->opt_window : (1 << 20);
         cudaError_t e2 = hea::launch_mc2(ctx->P, ctx->tab_host, ctx->lat.type, om, threads, team, team_ctl,
-                                         (int)ctx->opt_team_on, (int)ctx->opt_team_off, w_max2, occ_dev, counts_dev, C,
+                                         (int)ctx->opt_team_on, (int)ctx->opt_team_off, ctx->opt_accept == 1 ? 0 : 1, w_max2, occ_dev, counts_dev, C,
                                          n_steps, K, seed, chain0, step0, stats_dev, log_dev, log_cap,
                                          (cudaStream_t)cuda_stream, &ctx->n_launches);
         return e2 == cudaSuccess ? HEA_OK : fail_cuda(e2, "hea_mc_run launch (halo engine)");

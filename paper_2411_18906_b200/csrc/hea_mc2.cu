@@ -14,7 +14,9 @@
 //  * Whether b is a neighbour of a (the exclusion of D9.2) comes from the lattice coordinates of the two sites
 //    (minimum-image displacement, squared length == shell distance), not from a compare per table entry.
 //  * Shell sizes and the basis count are template constants (fcc 12/6/24, bcc 8/6/12), so every gather is unrolled.
+#include <cstdio>
 #include <cstring>
+#include <type_traits>
 
 #include "hea_device.cuh"
 #include "hea_mc_common.cuh"
@@ -53,6 +55,10 @@ struct Sh2 {
     double bc_J;
     uint32_t bc_W, pad;
     MoveRec rec;
+    // accept engine (8 lanes per candidate)
+    MoveRec cand[32];             // improving records of the 32 groups of a round
+    int4 wdesc[24];               // accumulator word w -> (int4 index in the offset row, slot mask, shell, side)
+    double g[kSMM], t[kSMM];      // objective constants with a per-lane index
 };
 
 struct SiteC {
@@ -187,6 +193,7 @@ __device__ __forceinline__ typename Pack<M>::W pack_F(const int (&F)[M])
 //         extra blocks only add latency; the followers wait on the control block.  When the windows have grown, the
 //         leader writes the state back, posts a phase record, and the followers reload and join.
 constexpr int kMaxTeam = 32;
+constexpr int kHaloThreads = 512;            // block size cap: 128 registers per thread, no spills in the hot paths
 constexpr int kTeamRounds = 32;             // candidates per thread per TEAM window (the null mask has 64 bits)
 
 struct TeamSlot {                 // 64 bytes
@@ -222,11 +229,12 @@ struct Mc2Args {
     Geo G;
     TeamCtl* team;                // [C] control blocks, zeroed before the launch (R > 1 only)
     int team_on, team_off;        // enter TEAM when W*K >= team_on; leave it after a move with steps_done*K < team_off
+    int accept_engine;            // 1: single-step windows run on the 8-lanes-per-candidate engine
 };
 
 // Shared memory: occupancy (offset 0, so a gather address is the loaded offset itself) | Sh2 | offset table [A][ZP].
 template <int M, int OCC, bool SYM, int LAT>
-__global__ void __launch_bounds__(1024)
+__global__ void __launch_bounds__(kHaloThreads)
 mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __grid_constant__ Mc2Args AA)
 {
     extern __shared__ __align__(16) uint8_t s_raw[];
@@ -311,6 +319,21 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         }
         s_tab[i] = entry;
     }
+    for (int i = tid; i < SMM; i += T) { sh.g[i] = Kc.g[i]; sh.t[i] = Kc.t[i]; }
+    if (tid < 24) {
+        // word list of the accept engine: per shell s < S the NA_s words of site a, then the NA_s words of site b
+        int w = tid, s = 0, side = 0, g = 0, rowoff = 0;
+        bool ok = false;
+        for (int s2 = 0, w0 = 0, ro = 0; s2 < S; ++s2) {
+            const int na = s2 == 0 ? NA0 : s2 == 1 ? NA1 : NA2;
+            if (w >= w0 && w < w0 + 2 * na) { ok = true; s = s2; side = (w - w0) >= na; g = (w - w0) - side * na; rowoff = ro; }
+            w0 += 2 * na; ro += na;
+        }
+        const int zs = s == 0 ? LC::z0 : s == 1 ? LC::z1 : LC::z2;
+        const int valid = ok ? min(4, zs - 4 * g) : 0;
+        const uint32_t mask = valid >= 4 ? 0xFFFFFFFFu : ((1u << (8 * valid)) - 1u);
+        sh.wdesc[tid] = make_int4(rowoff + g, (int)mask, s, side);
+    }
     if (tid == 0) {
         sh.n_accept = g_stats[0]; sh.n_null = 0; sh.hash = g_stats[2]; sh.last_accept = g_stats[3]; sh.n_logged = 0;
         sh.best[0] = sh.best[1] = sh.best[2] = kNoKey;
@@ -342,6 +365,236 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         if (w_cap > (uint32_t)A.w_max) w_cap = (uint32_t)A.w_max;
     };
     set_mode(false);
+    const bool accept_ok = T >= 512 && AA.accept_engine != 0;   // 8 evaluating warps + null-settling warps
+
+    // D9.4: apply an accepted move in every thread of the block (counts by the first S*M*M threads, the swap with its
+    // ghost images by thread T-1, bookkeeping by thread T-2); ends with a barrier.
+    auto apply_move = [&](const MoveRec* mv, uint32_t kk, unsigned long long step) {
+        const int p = (int)(mv->pq & 0xFFu), q = (int)(mv->pq >> 8);
+        for (int idx = tid; idx < SMM; idx += T) {
+            const int s = idx / MM, rem = idx - s * MM, i = rem / M, jj = rem - i * M;
+            const PW d = (PW)mv->d[s];
+            const int ci = (i == p) - (i == q), cj = (jj == p) - (jj == q);
+            sh.cnt[idx] += ci * Pack<M>::field(d, jj) + cj * Pack<M>::field(d, i);
+        }
+        if (tid == T - 1) {
+#pragma unroll 1
+            for (int which = 0; which < 2; ++which) {
+                const SiteC sc = decode_site<LAT>(G, which ? mv->b : mv->a);
+                const uint32_t code = 1u << (which ? p : q);
+                if (sc.x >= 1 && sc.x <= Lx - 2 && sc.y >= 1 && sc.y <= Ly - 2 && sc.z >= 1 && sc.z <= Lz - 2) {
+                    occ_set<OCC>(s_occ, sc.pidx, code);       // interior cell: no ghost image
+                } else {
+                    const int px[3] = {sc.x + 1, sc.x == Lx - 1 ? 0 : -1, sc.x == 0 ? Lx + 1 : -1};
+                    const int py[3] = {sc.y + 1, sc.y == Ly - 1 ? 0 : -1, sc.y == 0 ? Ly + 1 : -1};
+                    const int pz[3] = {sc.z + 1, sc.z == Lz - 1 ? 0 : -1, sc.z == 0 ? Lz + 1 : -1};
+                    for (int ix = 0; ix < 3; ++ix)
+                        for (int iy = 0; iy < 3; ++iy)
+                            for (int iz = 0; iz < 3; ++iz) {
+                                if (px[ix] < 0 || py[iy] < 0 || pz[iz] < 0) continue;
+                                const uint32_t pi = (uint32_t)((((px[ix] * G.PLy + py[iy]) * G.PLz + pz[iz]) << LC::lgA) | sc.b);
+                                occ_set<OCC>(s_occ, pi, code);
+                            }
+                }
+            }
+        }
+        if (tid == T - 2) {
+            const uint32_t a = mv->a, b = mv->b;
+            sh.J = mv->J;
+            sh.n_accept += 1;
+            sh.last_accept = step;
+            unsigned long long h = sh.hash;
+            h = (h ^ (uint32_t)step) * 0x100000001b3ULL;
+            h = (h ^ (uint32_t)(step >> 32)) * 0x100000001b3ULL;
+            h = (h ^ kk) * 0x100000001b3ULL;
+            h = (h ^ a) * 0x100000001b3ULL;
+            h = (h ^ b) * 0x100000001b3ULL;
+            sh.hash = h;
+            const unsigned long long nl = sh.n_logged;
+            if (rank == 0 && A.log_all != nullptr && (long long)nl < A.log_cap) {
+                unsigned long long* rec = A.log_all + (chain_local * (size_t)A.log_cap + nl) * 3;
+                rec[0] = step;
+                rec[1] = (unsigned long long)kk | ((unsigned long long)a << 32);
+                rec[2] = (unsigned long long)b;
+            }
+            sh.n_logged = nl + 1;
+        }
+        __syncthreads();
+    };
+
+    // ---- accept engine: one candidate per group of 8 lanes (latency instead of throughput).  Every lane of a group
+    // draws the same proposal; the accumulator words of the 2Z gathers and the S*M rows of the objective are dealt
+    // over the lanes; species counts are combined by xor-shuffles, the rows in the D6 order by indexed shuffles.
+#ifdef HEA_MC2_TIMING
+    long long dbg_seg[6] = {0, 0, 0, 0, 0, 0};
+#endif
+    using PD = typename std::conditional<(M <= 5), uint32_t, uint64_t>::type;     // (M-1) 8-bit fields
+    constexpr int NWR = (2 * (NA0 + NA1 + NA2) + 7) / 8;                          // word rounds per lane
+    constexpr int NRR = (3 * M + 7) / 8;                                          // row rounds per lane
+    const int nw = 2 * (NA0 + (S > 1 ? NA1 : 0) + (S > 2 ? NA2 : 0));
+    auto eval_g8 = [&](unsigned long long step, uint32_t k, bool valid, int grp, int buf, double J_cur) {
+#ifdef HEA_MC2_TIMING
+        const long long dbg_e0 = clock64();
+#endif
+        const int l8 = tid & 7;
+        const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), k, chain, key0, key1);
+        uint32_t a = __umulhi(r.x, (uint32_t)N), b = __umulhi(r.y, (uint32_t)N - 1u);
+        b += (b >= a);
+        SiteC sa = decode_site<LAT>(G, a), sb = decode_site<LAT>(G, b);
+        uint32_t hp = occ_get<OCC>(s_occ, sa.pidx), hq = occ_get<OCC>(s_occ, sb.pidx);
+        if (hp == hq) {
+            a = __umulhi(r.z, (uint32_t)N); b = __umulhi(r.w, (uint32_t)N - 1u);
+            b += (b >= a);
+            sa = decode_site<LAT>(G, a); sb = decode_site<LAT>(G, b);
+            hp = occ_get<OCC>(s_occ, sa.pidx); hq = occ_get<OCC>(s_occ, sb.pidx);
+        }
+#ifdef HEA_MC2_TIMING
+        if (tid == 0) dbg_seg[0] += clock64() - dbg_e0;
+#endif
+        const bool live = valid && hp != hq;
+        const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+        int mm0 = 0, mm1 = 0, mm2 = 0;
+        if (G.distinct) {
+            const int dx = 2 * (sb.x - sa.x) + (int)((G.basis >> (3 * sb.b)) & 1u) - (int)((G.basis >> (3 * sa.b)) & 1u);
+            const int dy = 2 * (sb.y - sa.y) + (int)((G.basis >> (3 * sb.b + 1)) & 1u) - (int)((G.basis >> (3 * sa.b + 1)) & 1u);
+            const int dz = 2 * (sb.z - sa.z) + (int)((G.basis >> (3 * sb.b + 2)) & 1u) - (int)((G.basis >> (3 * sa.b + 2)) & 1u);
+            const int wx = dx > Lx ? dx - 2 * Lx : dx < -Lx ? dx + 2 * Lx : dx;
+            const int wy = dy > Ly ? dy - 2 * Ly : dy < -Ly ? dy + 2 * Ly : dy;
+            const int wz = dz > Lz ? dz - 2 * Lz : dz < -Lz ? dz + 2 * Lz : dz;
+            const int r2 = wx * wx + wy * wy + wz * wz;
+            mm0 = r2 == G.d2[0]; mm1 = r2 == G.d2[1]; mm2 = r2 == G.d2[2];
+        } else {
+            const int32_t* row = nbr + (size_t)a * P.Z;
+            for (int e = 0; e < P.Z; ++e) {
+                const int hit = (uint32_t)__ldg(row + e) == b;
+                if (e < P.zoff[1]) mm0 += hit; else if (e < P.zoff[2]) mm1 += hit; else mm2 += hit;
+            }
+            mm0 -= P.m_self[0]; mm1 -= P.m_self[1]; mm2 -= P.m_self[2];
+        }
+#ifdef HEA_MC2_TIMING
+        if (tid == 0) dbg_seg[1] += clock64() - dbg_e0;
+#endif
+        // gathers: this lane's accumulator words -> biased species counts (+ for b's neighbours, - for a's)
+        PD D0 = 0, D1 = 0, D2 = 0;
+        PD bias4 = 0;
+#pragma unroll
+        for (int r2 = 0; r2 < M - 1; ++r2) bias4 |= (PD)4 << (8 * r2);
+#pragma unroll
+        for (int rd = 0; rd < NWR; ++rd) {
+            const int w = l8 + 8 * rd;
+            if (w < nw) {
+                const int4 dsc = sh.wdesc[w];
+                const uint32_t pidx = dsc.w ? sb.pidx : sa.pidx;
+                const int bb = dsc.w ? sb.b : sa.b;
+                const int4 o = reinterpret_cast<const int4*>(s_tab + bb * ZP)[dsc.x];
+                const uint32_t base = OCC == OCC2_NIB ? (pidx & ~1u) << 2 : pidx;
+                uint32_t acc = 0;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int oj = j == 0 ? o.x : j == 1 ? o.y : j == 2 ? o.z : o.w;
+                    const uint32_t t = base + (uint32_t)oj;
+                    uint32_t x;
+                    if (OCC == OCC2_NIB) x = (uint32_t)s_occ[t >> 3] >> (t & 4u);
+                    else x = s_occ[t];
+                    acc += x << (8 * j);
+                }
+                if (OCC == OCC2_NIB) acc &= 0x0F0F0F0Fu;
+                acc &= (uint32_t)dsc.y;
+                PD pk = 0;
+#pragma unroll
+                for (int r2 = 0; r2 < M - 1; ++r2)
+                    pk |= (PD)((((acc >> r2) & 0x01010101u) * 0x01010101u) >> 24) << (8 * r2);
+                const PD v = dsc.w ? bias4 + pk : bias4 - pk;
+                D0 += dsc.z == 0 ? v : (PD)0; D1 += dsc.z == 1 ? v : (PD)0; D2 += dsc.z == 2 ? v : (PD)0;
+            }
+        }
+#ifdef HEA_MC2_TIMING
+        if (tid == 0) dbg_seg[2] += clock64() - dbg_e0;
+#endif
+#pragma unroll
+        for (int o = 1; o < 8; o <<= 1) {
+            D0 += __shfl_xor_sync(0xFFFFFFFFu, D0, o);
+            if (S > 1) D1 += __shfl_xor_sync(0xFFFFFFFFu, D1, o);
+            if (S > 2) D2 += __shfl_xor_sync(0xFFFFFFFFu, D2, o);
+        }
+        int c[M], F0[M], F1[M], F2[M];
+        {
+            int l0 = 0, l1 = 0, l2 = 0;
+#pragma unroll
+            for (int r2 = 0; r2 < M; ++r2) {
+                c[r2] = (r2 == p) - (r2 == q);
+                if (r2 < M - 1) {
+                    F0[r2] = (int)((D0 >> (8 * r2)) & 0xFFu) - 8 * NA0; l0 -= F0[r2];
+                    F1[r2] = (int)((D1 >> (8 * r2)) & 0xFFu) - 8 * NA1; l1 -= F1[r2];
+                    F2[r2] = (int)((D2 >> (8 * r2)) & 0xFFu) - 8 * NA2; l2 -= F2[r2];
+                } else {
+                    F0[r2] = l0; F1[r2] = l1; F2[r2] = l2;
+                }
+            }
+            if (S < 2) {
+#pragma unroll
+                for (int r2 = 0; r2 < M; ++r2) F1[r2] = 0;
+            }
+            if (S < 3) {
+#pragma unroll
+                for (int r2 = 0; r2 < M; ++r2) F2[r2] = 0;
+            }
+#pragma unroll
+            for (int r2 = 0; r2 < M; ++r2) { F0[r2] -= mm0 * c[r2]; F1[r2] -= mm1 * c[r2]; F2[r2] -= mm2 * c[r2]; }
+        }
+#ifdef HEA_MC2_TIMING
+        if (tid == 0) dbg_seg[3] += clock64() - dbg_e0;
+#endif
+        // rows of the objective: row rho = s*M + i on lane rho & 7
+        double rowv[NRR];
+#pragma unroll
+        for (int rr = 0; rr < NRR; ++rr) {
+            const int rho = l8 + 8 * rr;
+            double row = 0.0;
+            if (rho < S * M) {
+                const int s = rho / M, i = rho - s * M;
+                const int ci = (i == p) - (i == q);
+                int Fi = 0;
+#pragma unroll
+                for (int j = 0; j < M; ++j) { const int Fj = s == 0 ? F0[j] : s == 1 ? F1[j] : F2[j]; Fi = j == i ? Fj : Fi; }
+#pragma unroll
+                for (int j = 0; j < M; ++j) {
+                    const int Fj = s == 0 ? F0[j] : s == 1 ? F1[j] : F2[j];
+                    const int n = sh.cnt[rho * M + j] + ci * Fj + c[j] * Fi;
+                    row = __dadd_rn(row, sq_dev(n, sh.g[rho * M + j], sh.t[rho * M + j]));
+                }
+            }
+            rowv[rr] = row;
+        }
+#ifdef HEA_MC2_TIMING
+        if (tid == 0) dbg_seg[4] += clock64() - dbg_e0;
+#endif
+        // D6 combination: rows in order within a shell, shells in order
+        double Jk = 0.0;
+#pragma unroll
+        for (int s = 0; s < 3; ++s) {
+            if (s < S) {
+                double shs = 0.0;
+#pragma unroll
+                for (int i = 0; i < M; ++i) {
+                    constexpr int dummy = 0; (void)dummy;
+                    const int rho = s * M + i;
+                    const double v = __shfl_sync(0xFFFFFFFFu, rowv[rho >> 3], (tid & 24) | (rho & 7));
+                    shs = __dadd_rn(shs, v);
+                }
+                Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[s], shs));
+            }
+        }
+#ifdef HEA_MC2_TIMING
+        if (tid == 0) dbg_seg[5] += clock64() - dbg_e0;
+#endif
+        if (l8 == 0 && live && Jk < J_cur) {
+            MoveRec& m = sh.cand[grp];
+            m.key = k; m.a = a; m.b = b; m.pq = (uint32_t)p | ((uint32_t)q << 8); m.J = Jk;
+            m.d[0] = pack_F<M>(F0); m.d[1] = pack_F<M>(F1); m.d[2] = pack_F<M>(F2);
+            atomicMin(&sh.best[buf], k);
+        }
+    };
 
     unsigned long long t0 = A.step0;
     const unsigned long long t_end = A.step0 + A.n_steps;
@@ -351,6 +604,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     uint32_t tw = 0;                                         // TEAM windows so far (same in every block of the team)
     uint32_t phase = 0;                                      // phase records consumed / posted
 
+#ifdef HEA_MC2_TIMING
+    long long dbg_eval = 0, dbg_bar = 0, dbg_apply = 0, dbg_steps = 0, dbg_cd = 0, dbg_da = 0, dbg_lastC = 0, dbg_lastD = 0;
+    const long long dbg_t0 = clock64();
+#endif
     while (t0 < t_end) {
         if (R > 1 && !team && rank != 0) {
             // ---- follower in a SOLO phase: wait for the leader's phase record, reload, join the team
@@ -370,219 +627,233 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             __syncthreads();
             continue;
         }
-        const uint32_t Wc = (uint32_t)min((unsigned long long)W, t_end - t0);
-        const int buf = (int)(it % 3u);
-        volatile uint32_t* best_slot = &sh.best[buf];
-        const double J_cur = sh.J;
-        uint32_t win_key = kNoKey, win_a = 0, win_b = 0, win_pq = 0;
-        PW win_d0 = 0, win_d1 = 0, win_d2 = 0;
-        double win_J = 0.0;
-        uint64_t nullmask = 0;
-
-        uint32_t ts = ts_first, k = k_first;
-        for (int j = 0; ts < Wc; ++j) {
-            const uint32_t hint = *best_slot;
-            if ((hint >> 10) < ts) break;                       // a move at an earlier step exists: this step is void
-            const uint32_t key = (ts << 10) | k;
-            // ---- D9.1 proposal
-            const unsigned long long step = t0 + ts;
-            const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), k, chain, key0, key1);
-            uint32_t a = __umulhi(r.x, (uint32_t)N), b = __umulhi(r.y, (uint32_t)N - 1u);
-            b += (b >= a);
-            SiteC sa = decode_site<LAT>(G, a), sb = decode_site<LAT>(G, b);
-            uint32_t hp = occ_get<OCC>(s_occ, sa.pidx), hq = occ_get<OCC>(s_occ, sb.pidx);
-            if (hp == hq) {
-                a = __umulhi(r.z, (uint32_t)N); b = __umulhi(r.w, (uint32_t)N - 1u);
-                b += (b >= a);
-                sa = decode_site<LAT>(G, a); sb = decode_site<LAT>(G, b);
-                hp = occ_get<OCC>(s_occ, sa.pidx); hq = occ_get<OCC>(s_occ, sb.pidx);
-            }
-            if (hp == hq) {
-                nullmask |= 1ull << j;
-            } else if (key < hint) {                             // same step, higher k than a known move: only nullness counts
-                const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
-                int c[M];
-#pragma unroll
-                for (int r2 = 0; r2 < M; ++r2) c[r2] = (r2 == p) - (r2 == q);
-                // ---- D9.2: is b an entry of a's rows?  (excluded sum = plain sum + (m - m_self)(e_q - e_p))
-                int mm0 = 0, mm1 = 0, mm2 = 0;
-                if (G.distinct) {
-                    const int dx = 2 * (sb.x - sa.x) + (int)((G.basis >> (3 * sb.b)) & 1u) - (int)((G.basis >> (3 * sa.b)) & 1u);
-                    const int dy = 2 * (sb.y - sa.y) + (int)((G.basis >> (3 * sb.b + 1)) & 1u) - (int)((G.basis >> (3 * sa.b + 1)) & 1u);
-                    const int dz = 2 * (sb.z - sa.z) + (int)((G.basis >> (3 * sb.b + 2)) & 1u) - (int)((G.basis >> (3 * sa.b + 2)) & 1u);
-                    const int wx = dx > Lx ? dx - 2 * Lx : dx < -Lx ? dx + 2 * Lx : dx;
-                    const int wy = dy > Ly ? dy - 2 * Ly : dy < -Ly ? dy + 2 * Ly : dy;
-                    const int wz = dz > Lz ? dz - 2 * Lz : dz < -Lz ? dz + 2 * Lz : dz;
-                    const int r2 = wx * wx + wy * wy + wz * wz;
-                    mm0 = r2 == G.d2[0]; mm1 = r2 == G.d2[1]; mm2 = r2 == G.d2[2];
-                } else {
-                    const int32_t* row = nbr + (size_t)a * P.Z;
-                    for (int e = 0; e < P.Z; ++e) {
-                        const int hit = (uint32_t)__ldg(row + e) == b;
-                        if (e < P.zoff[1]) mm0 += hit; else if (e < P.zoff[2]) mm1 += hit; else mm2 += hit;
+        uint32_t key_best = kNoKey, steps_done = 1u;
+        if (accept_ok && !team && W == 1u) {
+            // ---- accept engine: this one step, 32 candidates per round on the first 8 warps; the other warps settle
+            // which candidates of the step are null (all K count, D9.1)
+            const double J_cur = sh.J;
+#ifdef HEA_MC2_TIMING
+            const long long tA = clock64();
+            if (dbg_lastD) dbg_da += tA - dbg_lastD;
+#endif
+            if (tid >= 256) {
+                for (uint32_t k = (uint32_t)tid - 256u; k < (uint32_t)K; k += (uint32_t)T - 256u) {
+                    const uint4 r = philox4x32_10((uint32_t)t0, (uint32_t)(t0 >> 32), k, chain, key0, key1);
+                    uint32_t a = __umulhi(r.x, (uint32_t)N), b = __umulhi(r.y, (uint32_t)N - 1u);
+                    b += (b >= a);
+                    uint32_t hp = occ_get<OCC>(s_occ, decode_site<LAT>(G, a).pidx), hq = occ_get<OCC>(s_occ, decode_site<LAT>(G, b).pidx);
+                    if (hp == hq) {
+                        a = __umulhi(r.z, (uint32_t)N); b = __umulhi(r.w, (uint32_t)N - 1u);
+                        b += (b >= a);
+                        hp = occ_get<OCC>(s_occ, decode_site<LAT>(G, a).pidx); hq = occ_get<OCC>(s_occ, decode_site<LAT>(G, b).pidx);
                     }
-                    mm0 -= P.m_self[0]; mm1 -= P.m_self[1]; mm2 -= P.m_self[2];
-                }
-                const int4* ta = reinterpret_cast<const int4*>(s_tab + sa.b * ZP);
-                const int4* tb = reinterpret_cast<const int4*>(s_tab + sb.b * ZP);
-                // ---- D6 objective from counts + delta, shell by shell with the exact lower-bound pruning (hea_mc.cu)
-                int F0[M], F1[M], F2[M];
-#pragma unroll
-                for (int r2 = 0; r2 < M; ++r2) { F1[r2] = 0; F2[r2] = 0; }
-                {
-                    uint32_t xa[NA0], xb[NA0];
-                    gather_shell<OCC, LC::z0>(s_occ, ta, sa.pidx, xa);
-                    gather_shell<OCC, LC::z0>(s_occ, tb, sb.pidx, xb);
-                    hist_diff<M, NA0>(xa, xb, F0);
-#pragma unroll
-                    for (int r2 = 0; r2 < M; ++r2) F0[r2] -= mm0 * c[r2];
-                }
-                double Jk = __dmul_rn(Kc.w[0], shell_sum_F<M, SYM>(sh.cnt, Kc.g, Kc.t, F0, c));
-                Jk = __dadd_rn(0.0, Jk);
-                if (S > 1 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
-                    {
-                        uint32_t xa[NA1], xb[NA1];
-                        gather_shell<OCC, LC::z1>(s_occ, ta + NA0, sa.pidx, xa);
-                        gather_shell<OCC, LC::z1>(s_occ, tb + NA0, sb.pidx, xb);
-                        hist_diff<M, NA1>(xa, xb, F1);
-#pragma unroll
-                        for (int r2 = 0; r2 < M; ++r2) F1[r2] -= mm1 * c[r2];
-                    }
-                    Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[1], shell_sum_F<M, SYM>(sh.cnt + MM, Kc.g + MM, Kc.t + MM, F1, c)));
-                    if (S > 2 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
-                        {
-                            uint32_t xa[NA2], xb[NA2];
-                            gather_shell<OCC, LC::z2>(s_occ, ta + NA0 + NA1, sa.pidx, xa);
-                            gather_shell<OCC, LC::z2>(s_occ, tb + NA0 + NA1, sb.pidx, xb);
-                            hist_diff<M, NA2>(xa, xb, F2);
-#pragma unroll
-                            for (int r2 = 0; r2 < M; ++r2) F2[r2] -= mm2 * c[r2];
-                        }
-                        Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[2], shell_sum_F<M, SYM>(sh.cnt + 2 * MM, Kc.g + 2 * MM, Kc.t + 2 * MM, F2, c)));
-                    } else if (S > 2) {
-                        Jk = J_cur;                       // pruned: not improving
-                    }
-                } else if (S > 1) {
-                    Jk = J_cur;
-                }
-                if (Jk < J_cur && win_key == kNoKey) {
-                    win_key = key; win_a = a; win_b = b; win_pq = (uint32_t)p | ((uint32_t)q << 8);
-                    win_d0 = pack_F<M>(F0); win_d1 = pack_F<M>(F1); win_d2 = pack_F<M>(F2); win_J = Jk;
-                    atomicMin(&sh.best[buf], key);
+                    my_null += hp == hq;
                 }
             }
-            k += k_inc; ts += ts_inc;
-            if (k >= (uint32_t)K) { k -= (uint32_t)K; ++ts; }
-        }
-        __syncthreads();                                        // B1: window evaluated, local minimum posted
-        uint32_t key_best = sh.best[buf];
-        if (tid == 0) sh.best[(buf + 2) % 3] = kNoKey;          // next user of that slot is two barriers away
-
-        const int lane = tid & 31;
-        if (team) {
-            // ---- TEAM exchange: post this block's best record, read all R slots, take the minimum key
-            const int par = (int)(tw & 1u);
-            TeamSlot* slots = ctl->slot[par];
-            const bool owner = key_best != kNoKey && win_key == key_best;
-            if (owner || (key_best == kNoKey && tid == 0)) {
-                TeamSlot* me = slots + rank;
-                me->key = key_best; me->a = win_a; me->b = win_b; me->pq = win_pq; me->J = win_J;
-                me->d[0] = win_d0; me->d[1] = win_d1; me->d[2] = win_d2;
-                __threadfence();
-                st_release_u32(&me->seq, tw + 1u);
-            }
-            if (tid < 32) {
-                uint32_t kk = kNoKey;
-                if (lane < R) {
-                    while (ld_acquire_u32(&slots[lane].seq) != tw + 1u) { }
-                    kk = __ldcg(&slots[lane].key);
+            uint32_t rd0 = 0;
+            for (; rd0 < (uint32_t)K; rd0 += 32u) {
+                const int buf = (int)(it % 3u);
+                if (tid < 256) {
+                    const uint32_t k = rd0 + ((uint32_t)tid >> 3);
+                    eval_g8(t0, k, k < (uint32_t)K, tid >> 3, buf, J_cur);
                 }
-                uint32_t kmin = kk;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) kmin = min(kmin, __shfl_xor_sync(0xFFFFFFFFu, kmin, o));
-                if (kmin != kNoKey && kk == kmin) {           // keys are unique: exactly one lane
-                    const TeamSlot* src = slots + lane;
-                    MoveRec& m = sh.rec;
-                    m.key = kmin; m.a = __ldcg(&src->a); m.b = __ldcg(&src->b); m.pq = __ldcg(&src->pq);
-                    m.J = __ldcg(&src->J);
-                    m.d[0] = __ldcg(&src->d[0]); m.d[1] = __ldcg(&src->d[1]); m.d[2] = __ldcg(&src->d[2]);
-                }
-                if (lane == 0) sh.team_key = kmin;
+#ifdef HEA_MC2_TIMING
+                const long long tB = clock64();
+#endif
+                __syncthreads();
+#ifdef HEA_MC2_TIMING
+                const long long tC = clock64();
+                dbg_eval += tB - tA; dbg_bar += tC - tB; dbg_lastC = tC;
+#endif
+                key_best = sh.best[buf];
+                if (tid == 0) sh.best[(buf + 2) % 3] = kNoKey;
+                ++it;
+                if (key_best != kNoKey) break;
             }
-            __syncthreads();
-            key_best = sh.team_key;
-            ++tw;
-        } else if (key_best != kNoKey) {
-            const uint32_t owner_lane_mask = __ballot_sync(0xFFFFFFFFu, win_key == key_best);
-            if (owner_lane_mask != 0u && lane == __ffs((int)owner_lane_mask) - 1) {
-                MoveRec& m = sh.rec;
-                m.key = key_best; m.a = win_a; m.b = win_b; m.pq = win_pq; m.J = win_J;
-                m.d[0] = win_d0; m.d[1] = win_d1; m.d[2] = win_d2;
+            if (key_best != kNoKey) {
+#ifdef HEA_MC2_TIMING
+                const long long tD = clock64();
+#endif
+                apply_move(&sh.cand[key_best - rd0], key_best, t0);
+#ifdef HEA_MC2_TIMING
+                dbg_apply += clock64() - tD; dbg_steps += 1; dbg_cd += tD - dbg_lastC;
+                dbg_lastD = clock64();
+#endif
+                W = 1u;
+            } else {
+                W = min(2u, w_cap);
             }
-            __syncthreads();
-        }
-        const MoveRec* mv = &sh.rec;
-
-        // ---- commit: null counts of the committed steps, then the move (D9.4)
-        const uint32_t steps_done = key_best != kNoKey ? (key_best >> 10) + 1u : Wc;
-        if (nullmask) {
-            const uint32_t lim = steps_done * (uint32_t)K;       // candidates c < lim are committed
-            const uint32_t n_comm = gtid < lim ? (lim - 1u - gtid) / GT + 1u : 0u;
-            my_null += __popcll(n_comm >= 64u ? nullmask : (nullmask & ((1ull << n_comm) - 1ull)));
-        }
-        if (key_best != kNoKey) {
-            const int p = (int)(mv->pq & 0xFFu), q = (int)(mv->pq >> 8);
-            for (int idx = tid; idx < SMM; idx += T) {
-                const int s = idx / MM, rem = idx - s * MM, i = rem / M, jj = rem - i * M;
-                const PW d = (PW)mv->d[s];
-                const int ci = (i == p) - (i == q), cj = (jj == p) - (jj == q);
-                sh.cnt[idx] += ci * Pack<M>::field(d, jj) + cj * Pack<M>::field(d, i);
-            }
-            if (tid == T - 1) {                                 // one thread (not among the count updaters when T > SMM)
-                const uint32_t a = mv->a, b = mv->b, kk = key_best & 1023u;
-                const unsigned long long step = t0 + (key_best >> 10);
-                // the swap, on the real sites and on every ghost image of them
-#pragma unroll 1
-                for (int which = 0; which < 2; ++which) {
-                    const SiteC sc = decode_site<LAT>(G, which ? b : a);
-                    const uint32_t code = 1u << (which ? p : q);
-                    const int px[3] = {sc.x + 1, sc.x == Lx - 1 ? 0 : -1, sc.x == 0 ? Lx + 1 : -1};
-                    const int py[3] = {sc.y + 1, sc.y == Ly - 1 ? 0 : -1, sc.y == 0 ? Ly + 1 : -1};
-                    const int pz[3] = {sc.z + 1, sc.z == Lz - 1 ? 0 : -1, sc.z == 0 ? Lz + 1 : -1};
-                    for (int ix = 0; ix < 3; ++ix)
-                        for (int iy = 0; iy < 3; ++iy)
-                            for (int iz = 0; iz < 3; ++iz) {
-                                if (px[ix] < 0 || py[iy] < 0 || pz[iz] < 0) continue;
-                                const uint32_t pi = (uint32_t)((((px[ix] * G.PLy + py[iy]) * G.PLz + pz[iz]) << LC::lgA) | sc.b);
-                                occ_set<OCC>(s_occ, pi, code);
-                            }
-                }
-                sh.J = mv->J;
-                sh.n_accept += 1;
-                sh.last_accept = step;
-                unsigned long long h = sh.hash;
-                h = (h ^ (uint32_t)step) * 0x100000001b3ULL;
-                h = (h ^ (uint32_t)(step >> 32)) * 0x100000001b3ULL;
-                h = (h ^ kk) * 0x100000001b3ULL;
-                h = (h ^ a) * 0x100000001b3ULL;
-                h = (h ^ b) * 0x100000001b3ULL;
-                sh.hash = h;
-                const unsigned long long nl = sh.n_logged;
-                if (rank == 0 && A.log_all != nullptr && (long long)nl < A.log_cap) {
-                    unsigned long long* rec = A.log_all + (chain_local * (size_t)A.log_cap + nl) * 3;
-                    rec[0] = step;
-                    rec[1] = (unsigned long long)kk | ((unsigned long long)a << 32);
-                    rec[2] = (unsigned long long)b;
-                }
-                sh.n_logged = nl + 1;
-            }
-            __syncthreads();
-            W = min(steps_done, w_cap);                         // the observed gap
         } else {
-            W = min(W * 2u, w_cap);
+            const uint32_t Wc = (uint32_t)min((unsigned long long)W, t_end - t0);
+            const int buf = (int)(it % 3u);
+            volatile uint32_t* best_slot = &sh.best[buf];
+            const double J_cur = sh.J;
+            uint32_t win_key = kNoKey, win_a = 0, win_b = 0, win_pq = 0;
+            PW win_d0 = 0, win_d1 = 0, win_d2 = 0;
+            double win_J = 0.0;
+            uint64_t nullmask = 0;
+
+            uint32_t ts = ts_first, k = k_first;
+            for (int j = 0; ts < Wc; ++j) {
+                const uint32_t hint = *best_slot;
+                if ((hint >> 10) < ts) break;                       // a move at an earlier step exists: this step is void
+                const uint32_t key = (ts << 10) | k;
+                // ---- D9.1 proposal
+                const unsigned long long step = t0 + ts;
+                const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), k, chain, key0, key1);
+                uint32_t a = __umulhi(r.x, (uint32_t)N), b = __umulhi(r.y, (uint32_t)N - 1u);
+                b += (b >= a);
+                SiteC sa = decode_site<LAT>(G, a), sb = decode_site<LAT>(G, b);
+                uint32_t hp = occ_get<OCC>(s_occ, sa.pidx), hq = occ_get<OCC>(s_occ, sb.pidx);
+                if (hp == hq) {
+                    a = __umulhi(r.z, (uint32_t)N); b = __umulhi(r.w, (uint32_t)N - 1u);
+                    b += (b >= a);
+                    sa = decode_site<LAT>(G, a); sb = decode_site<LAT>(G, b);
+                    hp = occ_get<OCC>(s_occ, sa.pidx); hq = occ_get<OCC>(s_occ, sb.pidx);
+                }
+                if (hp == hq) {
+                    nullmask |= 1ull << j;
+                } else if (key < hint) {                             // same step, higher k than a known move: only nullness counts
+                    const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+                    int c[M];
+    #pragma unroll
+                    for (int r2 = 0; r2 < M; ++r2) c[r2] = (r2 == p) - (r2 == q);
+                    // ---- D9.2: is b an entry of a's rows?  (excluded sum = plain sum + (m - m_self)(e_q - e_p))
+                    int mm0 = 0, mm1 = 0, mm2 = 0;
+                    if (G.distinct) {
+                        const int dx = 2 * (sb.x - sa.x) + (int)((G.basis >> (3 * sb.b)) & 1u) - (int)((G.basis >> (3 * sa.b)) & 1u);
+                        const int dy = 2 * (sb.y - sa.y) + (int)((G.basis >> (3 * sb.b + 1)) & 1u) - (int)((G.basis >> (3 * sa.b + 1)) & 1u);
+                        const int dz = 2 * (sb.z - sa.z) + (int)((G.basis >> (3 * sb.b + 2)) & 1u) - (int)((G.basis >> (3 * sa.b + 2)) & 1u);
+                        const int wx = dx > Lx ? dx - 2 * Lx : dx < -Lx ? dx + 2 * Lx : dx;
+                        const int wy = dy > Ly ? dy - 2 * Ly : dy < -Ly ? dy + 2 * Ly : dy;
+                        const int wz = dz > Lz ? dz - 2 * Lz : dz < -Lz ? dz + 2 * Lz : dz;
+                        const int r2 = wx * wx + wy * wy + wz * wz;
+                        mm0 = r2 == G.d2[0]; mm1 = r2 == G.d2[1]; mm2 = r2 == G.d2[2];
+                    } else {
+                        const int32_t* row = nbr + (size_t)a * P.Z;
+                        for (int e = 0; e < P.Z; ++e) {
+                            const int hit = (uint32_t)__ldg(row + e) == b;
+                            if (e < P.zoff[1]) mm0 += hit; else if (e < P.zoff[2]) mm1 += hit; else mm2 += hit;
+                        }
+                        mm0 -= P.m_self[0]; mm1 -= P.m_self[1]; mm2 -= P.m_self[2];
+                    }
+                    const int4* ta = reinterpret_cast<const int4*>(s_tab + sa.b * ZP);
+                    const int4* tb = reinterpret_cast<const int4*>(s_tab + sb.b * ZP);
+                    // ---- D6 objective from counts + delta, shell by shell with the exact lower-bound pruning (hea_mc.cu)
+                    int F0[M], F1[M], F2[M];
+    #pragma unroll
+                    for (int r2 = 0; r2 < M; ++r2) { F1[r2] = 0; F2[r2] = 0; }
+                    {
+                        uint32_t xa[NA0], xb[NA0];
+                        gather_shell<OCC, LC::z0>(s_occ, ta, sa.pidx, xa);
+                        gather_shell<OCC, LC::z0>(s_occ, tb, sb.pidx, xb);
+                        hist_diff<M, NA0>(xa, xb, F0);
+    #pragma unroll
+                        for (int r2 = 0; r2 < M; ++r2) F0[r2] -= mm0 * c[r2];
+                    }
+                    double Jk = __dmul_rn(Kc.w[0], shell_sum_F<M, SYM>(sh.cnt, Kc.g, Kc.t, F0, c));
+                    Jk = __dadd_rn(0.0, Jk);
+                    if (S > 1 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
+                        {
+                            uint32_t xa[NA1], xb[NA1];
+                            gather_shell<OCC, LC::z1>(s_occ, ta + NA0, sa.pidx, xa);
+                            gather_shell<OCC, LC::z1>(s_occ, tb + NA0, sb.pidx, xb);
+                            hist_diff<M, NA1>(xa, xb, F1);
+    #pragma unroll
+                            for (int r2 = 0; r2 < M; ++r2) F1[r2] -= mm1 * c[r2];
+                        }
+                        Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[1], shell_sum_F<M, SYM>(sh.cnt + MM, Kc.g + MM, Kc.t + MM, F1, c)));
+                        if (S > 2 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
+                            {
+                                uint32_t xa[NA2], xb[NA2];
+                                gather_shell<OCC, LC::z2>(s_occ, ta + NA0 + NA1, sa.pidx, xa);
+                                gather_shell<OCC, LC::z2>(s_occ, tb + NA0 + NA1, sb.pidx, xb);
+                                hist_diff<M, NA2>(xa, xb, F2);
+    #pragma unroll
+                                for (int r2 = 0; r2 < M; ++r2) F2[r2] -= mm2 * c[r2];
+                            }
+                            Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[2], shell_sum_F<M, SYM>(sh.cnt + 2 * MM, Kc.g + 2 * MM, Kc.t + 2 * MM, F2, c)));
+                        } else if (S > 2) {
+                            Jk = J_cur;                       // pruned: not improving
+                        }
+                    } else if (S > 1) {
+                        Jk = J_cur;
+                    }
+                    if (Jk < J_cur && win_key == kNoKey) {
+                        win_key = key; win_a = a; win_b = b; win_pq = (uint32_t)p | ((uint32_t)q << 8);
+                        win_d0 = pack_F<M>(F0); win_d1 = pack_F<M>(F1); win_d2 = pack_F<M>(F2); win_J = Jk;
+                        atomicMin(&sh.best[buf], key);
+                    }
+                }
+                k += k_inc; ts += ts_inc;
+                if (k >= (uint32_t)K) { k -= (uint32_t)K; ++ts; }
+            }
+            __syncthreads();                                        // B1: window evaluated, local minimum posted
+            key_best = sh.best[buf];
+            if (tid == 0) sh.best[(buf + 2) % 3] = kNoKey;          // next user of that slot is two barriers away
+
+            const int lane = tid & 31;
+            if (team) {
+                // ---- TEAM exchange: post this block's best record, read all R slots, take the minimum key
+                const int par = (int)(tw & 1u);
+                TeamSlot* slots = ctl->slot[par];
+                const bool owner = key_best != kNoKey && win_key == key_best;
+                if (owner || (key_best == kNoKey && tid == 0)) {
+                    TeamSlot* me = slots + rank;
+                    me->key = key_best; me->a = win_a; me->b = win_b; me->pq = win_pq; me->J = win_J;
+                    me->d[0] = win_d0; me->d[1] = win_d1; me->d[2] = win_d2;
+                    __threadfence();
+                    st_release_u32(&me->seq, tw + 1u);
+                }
+                if (tid < 32) {
+                    uint32_t kk = kNoKey;
+                    if (lane < R) {
+                        while (ld_acquire_u32(&slots[lane].seq) != tw + 1u) { }
+                        kk = __ldcg(&slots[lane].key);
+                    }
+                    uint32_t kmin = kk;
+    #pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) kmin = min(kmin, __shfl_xor_sync(0xFFFFFFFFu, kmin, o));
+                    if (kmin != kNoKey && kk == kmin) {           // keys are unique: exactly one lane
+                        const TeamSlot* src = slots + lane;
+                        MoveRec& m = sh.rec;
+                        m.key = kmin; m.a = __ldcg(&src->a); m.b = __ldcg(&src->b); m.pq = __ldcg(&src->pq);
+                        m.J = __ldcg(&src->J);
+                        m.d[0] = __ldcg(&src->d[0]); m.d[1] = __ldcg(&src->d[1]); m.d[2] = __ldcg(&src->d[2]);
+                    }
+                    if (lane == 0) sh.team_key = kmin;
+                }
+                __syncthreads();
+                key_best = sh.team_key;
+                ++tw;
+            } else if (key_best != kNoKey) {
+                const uint32_t owner_lane_mask = __ballot_sync(0xFFFFFFFFu, win_key == key_best);
+                if (owner_lane_mask != 0u && lane == __ffs((int)owner_lane_mask) - 1) {
+                    MoveRec& m = sh.rec;
+                    m.key = key_best; m.a = win_a; m.b = win_b; m.pq = win_pq; m.J = win_J;
+                    m.d[0] = win_d0; m.d[1] = win_d1; m.d[2] = win_d2;
+                }
+                __syncthreads();
+            }
+            const MoveRec* mv = &sh.rec;
+
+            // ---- commit: null counts of the committed steps, then the move (D9.4)
+            steps_done = key_best != kNoKey ? (key_best >> 10) + 1u : Wc;
+            if (nullmask) {
+                const uint32_t lim = steps_done * (uint32_t)K;       // candidates c < lim are committed
+                const uint32_t n_comm = gtid < lim ? (lim - 1u - gtid) / GT + 1u : 0u;
+                my_null += __popcll(n_comm >= 64u ? nullmask : (nullmask & ((1ull << n_comm) - 1ull)));
+            }
+            if (key_best != kNoKey) {
+                apply_move(mv, key_best & 1023u, t0 + (key_best >> 10));
+                W = min(steps_done, w_cap);                         // the observed gap
+            } else {
+                W = min(W * 2u, w_cap);
+            }
+            ++it;
         }
         t0 += steps_done;
-        ++it;
+
 
         // ---- mode switches (R > 1): every block of the team takes the same decision from the same history
         if (R > 1 && t0 < t_end) {
@@ -606,6 +877,14 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         }
     }
 
+#ifdef HEA_MC2_TIMING
+    if (tid == 0 && blockIdx.x == 0 && dbg_steps > 0) {
+        printf("mc2 eval segments (cumulative): proposal %lld adjacency %lld gathers %lld reduce+F %lld rows %lld combine %lld\n",
+               dbg_seg[0] / dbg_steps, dbg_seg[1] / dbg_steps, dbg_seg[2] / dbg_steps, dbg_seg[3] / dbg_steps, dbg_seg[4] / dbg_steps, dbg_seg[5] / dbg_steps);
+        printf("mc2 timing: steps %lld eval %lld bar %lld c->d %lld apply %lld d->a %lld loop-total %lld (cycles per step)\n", dbg_steps,
+               dbg_eval / dbg_steps, dbg_bar / dbg_steps, dbg_cd / dbg_steps, dbg_apply / dbg_steps, dbg_da / dbg_steps, (clock64() - dbg_t0) / dbg_steps);
+    }
+#endif
     // ---- epilogue: release waiting followers, write back (rank 0 owns the global copy; nulls are summed over blocks)
     if (R > 1 && rank == 0 && !team) {
         __syncthreads();
@@ -694,7 +973,7 @@ size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L)
 size_t mc2_team_bytes(int64_t C) { return sizeof(TeamCtl) * (size_t)C; }
 
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
-                       void* team_ctl, int team_on, int team_off, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
+                       void* team_ctl, int team_on, int team_off, int accept_engine, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
                        uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches)
 {
     Mc2Args AA;
@@ -707,6 +986,7 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
     AA.team = reinterpret_cast<TeamCtl*>(team_ctl);
     AA.team_on = team_on > 0 ? team_on : 4 * threads;
     AA.team_off = team_off > 0 ? team_off : threads;
+    AA.accept_engine = accept_engine;
     if (team > 1) {
         if (team > kMaxTeam || !team_ctl) return cudaErrorInvalidValue;
         cudaError_t em = cudaMemsetAsync(team_ctl, 0, mc2_team_bytes(C), st);

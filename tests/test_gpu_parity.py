@@ -209,6 +209,17 @@ def test_mc_halo_engine_teams_reject_regime(hb, team, threads):
     assert (st["n_accept"] > 20).all()
 
 
+@pytest.mark.parametrize("lattice,dims,conc,S,K", [("fcc", (4, 4, 4), [0.2, 0.2, 0.2, 0.4], 3, 24), ("bcc", (5, 5, 5), [0.2] * 5, 3, 70),
+                                                   ("fcc", (3, 3, 3), [0.5, 0.5], 1, 33), ("bcc", (4, 4, 4), [1 / 8] * 8, 2, 128),
+                                                   ("fcc", (2, 2, 2), [0.25] * 4, 3, 40), ("fcc", (5, 4, 3), [1 / 6] * 6, 3, 17)])
+@pytest.mark.parametrize("threads,team", [(512, 1), (1024, 1), (1024, 3)])
+def test_mc_halo_engine_accept_engine(hb, lattice, dims, conc, S, K, threads, team):
+    # single-step windows run 8 lanes per candidate (T >= 512); same trajectory as thread-per-candidate and the oracle
+    w = small(lattice, dims, conc, S, target_seed=9, K=K, n_steps=400, rng=(-0.2, 0.2))
+    st = run_both(hb, w, 3, 400, log_cap=400, opts={"mc_engine": 2, "mc_threads": threads, "mc_team": team, "mc_accept": 2})
+    assert st["n_accept"].sum() > 5
+
+
 def test_mc_halo_engine_c3_c4_prefix(hb):
     st = run_both(hb, wl.config(3), 4, 300, log_cap=300, opts={"mc_engine": 2})
     assert (st["n_accept"] > 250).all()
