@@ -5,10 +5,11 @@
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
 Workload (BASELINE.json:configs[3], "c4"): fcc 40x40x40 = 256,000 atoms, 4 species at 0.25, shells 1-2, non-zero
-first-shell target (seed 11), 16 chains per GPU, K = 128 candidates per MC step.  One bench "step" is one pass of the
-whole hot path over that batch: `hea_sro_full` of the 16 configurations (counts, alpha, J) followed by
-`hea_mc_run` for --mc-steps MC steps of every chain (default 50,000; the 1e7-step trajectory of the config is
-cut into such segments -- split-run invariance, D9, makes the result identical to one long call).
+first-shell target (seed 11), 16 chains per GPU x 1e7 MC steps, K = 128 candidates per step, chain seed 4.
+One bench "step" is one pass of the whole hot path over that batch, exactly the config: `hea_sro_full` of the 16 seeded
+random start configurations (counts, alpha, J) followed by ONE `hea_mc_run` of the whole 1e7-step trajectory of every
+chain (about 70,000 steps in the accept regime, the rest in the reject regime; `regimes` reports both separately).
+--mc-steps n shortens the trajectory (exploration; stated in `config`).
 `value` = swap trials/s = chains * mc-steps * K / device time of the whole step, inputs resident in HBM.
 `e2e` = the same metric through the host-buffer C-ABI call `hea_mc_run_host` (H2D of the occupancies from pinned
 memory, recount, MC, D2H of occupancies + counts + stats inside the timed region).
@@ -17,7 +18,8 @@ Multi-GPU: chains are independent, so rank r runs chains [16 r, 16 r + 16) with 
 `roofline` is for the dominant kernel of the step (the MC kernel; ALU-issue bound, model in DESIGN.md section 6);
 `recount_roofline` is for the recount kernel on the sweep point of configs[4] where the neighbour table exceeds L2
 (fcc 100^3 = 4,000,000 atoms, 3 shells, batch 1; HBM bound, 4*Z+1 = 169 B/atom).
-`cpu_baseline` / `--impl reference`: the CPU oracle (oracle/hea_oracle.c), as it stands, on the host cores.
+`cpu_baseline` / `--impl reference`: the CPU oracle (oracle/hea_oracle.c), as it stands, on the host cores, on a
+bounded sample (the first steps of the same trajectory).
 """
 import argparse
 import json
@@ -33,7 +35,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "delta-SRO swap trials/sec (c4: fcc 40^3, 256,000 atoms, 16 chains, K=128) incl. full-SRO recount per step"
+METRIC = "delta-SRO swap trials/sec (c4: fcc 40^3, 256,000 atoms, 16 chains x 1e7 steps, K=128) incl. the full-SRO recount of the start"
 UNIT = "swap-trials/s"
 
 
@@ -168,7 +170,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--mc-steps", type=int, default=50_000, help="MC steps per chain per bench step")
+    ap.add_argument("--mc-steps", type=int, default=0, help="MC steps per chain per bench step (0 = the whole trajectory of the config: 1e7 for c4)")
     ap.add_argument("--ref-mc-steps", type=int, default=2_000, help="MC steps per bench step of the reference arm")
     ap.add_argument("--recount-L", type=int, default=100, help="fcc L^3 cells of the recount roofline point")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -202,22 +204,26 @@ def main():
     for kv in args.opt:
         k, v = kv.split("=")
         h.set_option(k, int(v))
-    C, K, N, n_mc = w.n_chains, w.K, w.n_sites, args.mc_steps
+    C, K, N = w.n_chains, w.K, w.n_sites
+    n_mc = args.mc_steps if args.mc_steps > 0 else w.n_steps
     SMM = h.S * h.M * h.M
     chain0, _ = sharding.weak_chain_range(rank, C)
-    occ = h.init_random(C, w.seed, chain0)
+    occ_init = h.init_random(C, w.seed, chain0)                           # the seeded random start of the config
+    occ = occ_init.clone()
     counts = torch.empty((C, h.S, h.M, h.M), dtype=torch.int32, device=dev)
     stats = h.new_stats(C)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
-    state = {"step0": 0}
 
     def one_step(ev=None):
+        # one pass of the whole hot path over the batch: recount of the C start configurations, then the whole MC
+        # trajectory of every chain from step 0.  Restoring the start and resetting the stats is not part of the path.
+        occ.copy_(occ_init)
+        h.reset_stats(stats)
         if ev: ev[0].record()
         h.sro_full(occ, counts=counts)
         if ev: ev[1].record()
-        h.mc_run(occ, counts, n_mc, K, w.seed, chain0=chain0, step0=state["step0"], stats=stats)
+        h.mc_run(occ, counts, n_mc, K, w.seed, chain0=chain0, step0=0, stats=stats)
         if ev: ev[2].record()
-        state["step0"] += n_mc
 
     def barrier():
         torch.cuda.synchronize()
@@ -228,7 +234,6 @@ def main():
     for _ in range(args.warmup):
         one_step()
     barrier()
-    st0 = binding.stats_to_numpy(stats).copy()
     sampler = ClockSampler(local_rank)
     sampler.start()
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
@@ -240,7 +245,7 @@ def main():
         one_step(evs[i])
     barrier()
     t_wall = time.perf_counter() - t_wall0
-    launches = h.launch_count() - l0
+    launches = h.launch_count() - l0 - args.steps          # minus the stats resets (outside the events)
     t_rc = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
     t_mc = sum(e[1].elapsed_time(e[2]) for e in evs) * 1e-3
     t_dev = t_rc + t_mc
@@ -250,23 +255,47 @@ def main():
     chk, _, _ = h.sro_full(occ)
     assert bool((chk == counts).all()), "incremental counts diverged from the recount"
 
+    # ---- the two regimes of the trajectory, timed separately (information, not the metric): the first steps from the
+    # random start (accept regime: nearly every step applies a move) and steps after the whole trajectory (reject regime)
+    def timed_mc(n, step0):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        h.mc_run(occ, counts, n, K, w.seed, chain0=chain0, step0=step0, stats=stats)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3
+    n_tail = min(1_000_000, max(1000, n_mc // 10))
+    a0 = int(st1["n_accept"].sum())
+    t_tail = timed_mc(n_tail, n_mc)
+    a1 = int(binding.stats_to_numpy(stats)["n_accept"].sum())
+    n_head = min(20_000, n_mc)
+    occ.copy_(occ_init); h.reset_stats(stats); h.sro_full(occ, counts=counts)
+    t_head = timed_mc(n_head, 0)
+    a2 = int(binding.stats_to_numpy(stats)["n_accept"].sum())
+    regimes = {"first_steps": {"mc_steps": n_head, "trials_per_s": world * C * n_head * K / t_head,
+                               "us_per_step": 1e6 * t_head / n_head, "accept_rate": a2 / (C * n_head)},
+               "after_trajectory": {"mc_steps": n_tail, "trials_per_s": world * C * n_tail * K / t_tail,
+                                    "us_per_step": 1e6 * t_tail / n_tail, "accept_rate": (a1 - a0) / (C * n_tail)}}
+
     # ---- e2e: host buffers through hea_mc_run_host, copies inside the timed region
+    occ_host0 = occ_init.cpu()
     occ_host = torch.empty((C, N), dtype=torch.uint8).pin_memory()
-    occ_host.copy_(occ.cpu())
     occ_np = occ_host.numpy()
-    st_host = binding.stats_to_numpy(stats).copy()
     cnt_host = np.empty((C, h.S, h.M, h.M), dtype=np.int32)
-    e2e_step0 = state["step0"]
-    for _ in range(2):
-        h.mc_run_host(occ_np, n_mc, K, w.seed, chain0=chain0, step0=e2e_step0, stats=st_host, counts_out=cnt_host)
-        e2e_step0 += n_mc
+    for _ in range(1):
+        occ_host.copy_(occ_host0)
+        st_host = binding.fresh_stats_host(C)
+        h.mc_run_host(occ_np, n_mc, K, w.seed, chain0=chain0, step0=0, stats=st_host, counts_out=cnt_host)
     barrier()
-    t0 = time.perf_counter()
+    t_e2e = 0.0
     for _ in range(args.steps):
-        h.mc_run_host(occ_np, n_mc, K, w.seed, chain0=chain0, step0=e2e_step0, stats=st_host, counts_out=cnt_host)
-        e2e_step0 += n_mc
-    torch.cuda.synchronize()
-    t_e2e = time.perf_counter() - t0
+        occ_host.copy_(occ_host0)
+        st_host = binding.fresh_stats_host(C)
+        t0 = time.perf_counter()
+        h.mc_run_host(occ_np, n_mc, K, w.seed, chain0=chain0, step0=0, stats=st_host, counts_out=cnt_host)
+        torch.cuda.synchronize()
+        t_e2e += time.perf_counter() - t0
+    assert (st_host["hash"] == st1["hash"]).all(), "host-buffer path and device path disagree"
     clocks = sampler.stop()
     h2d = C * N + 40 * C
     d2h = C * N + 4 * SMM * C + 40 * C
@@ -319,8 +348,9 @@ def main():
                    "(256 MB fill, outside the events)", "parallelism": f"chains sharded, {world} rank(s), no collective"},
         "recount_atoms_per_s": world * C * N * args.steps / t_rc,
         "mc_trials_per_s": world * mc_rate_1gpu,
-        "accept_rate": float((st1["n_accept"] - st0["n_accept"]).sum()) / (C * n_mc * args.steps),
-        "null_rate": float((st1["n_null"] - st0["n_null"]).sum()) / (C * n_mc * args.steps * K),
+        "accept_rate": float(st1["n_accept"].sum()) / (C * n_mc),
+        "null_rate": float(st1["n_null"].sum()) / (C * n_mc * K),
+        "regimes": regimes,
         "J_mean": float(st1["J"].mean()),
         "wall_ms_per_step_incl_flush": 1e3 * t_wall / args.steps,
         "clocks": clocks,
@@ -329,7 +359,7 @@ def main():
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "achieved": mc_rate_1gpu * ops / 1e12, "peak": alu_peak,
                      "unit": "T thread-instr/s", "frac": mc_rate_1gpu * ops / 1e12 / alu_peak, "traffic": None,
-                     "kernel": "mc_window_kernel", "ops_per_trial": ops, "ms_per_launch": 1e3 * t_mc / args.steps,
+                     "kernel": "mc_halo_kernel", "ops_per_trial": ops, "ms_per_launch": 1e3 * t_mc / args.steps,
                      "peak_source": f"{n_sms} SMs x 128 lanes/clk x {sm_max_mhz:.0f} MHz (DESIGN.md section 6)"},
     }
     if args.workload != 4 or args.chains:

@@ -148,6 +148,10 @@ class Hea:
         _check(lib().hea_mc_stats_reset(self._h, C.c_void_p(st.data_ptr()), n_chains, _stream()))
         return st
 
+    def reset_stats(self, stats):
+        _check(lib().hea_mc_stats_reset(self._h, C.c_void_p(stats.data_ptr()), stats.shape[0], _stream()))
+        return stats
+
     def mc_run(self, occ, counts, n_steps, K, seed, chain0=0, step0=0, stats=None, log_cap=0):
         """In place on occ [C][N] and counts [C][S][M][M]; returns (stats tensor [C][5] int64 view, log or None)."""
         assert occ.dtype == torch.uint8 and occ.is_cuda and occ.is_contiguous() and occ.dim() == 2
