@@ -250,6 +250,20 @@ def test_mc_c4_prefix(hb):
     assert (st["n_accept"] > 250).all()
 
 
+def test_mc_c4_bench_launch_configuration_through_convergence(hb):
+    # exactly what bench.py launches (16 chains -> teams of 9 blocks, 512 threads, accept engine, then TEAM windows),
+    # through the accept regime (~70,000 steps), the transition and into the reject regime
+    w = wl.config(4)
+    st = run_both(hb, w, w.n_chains, 300_000, log_cap=64, threads=16)
+    assert (st["n_accept"] > 60_000).all() and (st["last_accept_step"] < 90_000).all()
+
+
+def test_mc_c3_many_chains_through_convergence(hb):
+    w = wl.config(3)
+    st = run_both(hb, w, 64, 6000, log_cap=64, threads=16)
+    assert (st["n_accept"] > 1000).all()
+
+
 def test_mc_c4_global_occupancy_path(hb):
     w = wl.config(4)
     run_both(hb, w, 2, 100, opts={"mc_occ_mode": 3, "mc_cluster": 8})
