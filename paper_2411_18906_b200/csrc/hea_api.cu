@@ -25,6 +25,7 @@ cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode,
                       int* query_max_clusters);
 size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L);
 size_t mc2_team_bytes(int64_t C);
+constexpr int kMc2MaxThreads = 512;
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
                        void* team_ctl, int team_on, int team_off, int accept_engine, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
                        uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches);
@@ -393,12 +394,12 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
         int team = (int)ctx->opt_team;
         if (team == 0) team = (int)std::max<int64_t>(1, std::min<int64_t>(32, ctx->n_sms / C));
         if (team > 1 && (int64_t)team * C > ctx->n_sms) return fail(HEA_EINVAL, "mc_team: team blocks * chains exceeds the SM count");
-        int threads = ctx->opt_threads ? (int)ctx->opt_threads : 512;
+        int threads = ctx->opt_threads ? (int)ctx->opt_threads : hea::kMc2MaxThreads;
         if (!ctx->opt_threads && team == 1) {
             const int64_t blocks_per_sm = (C + ctx->n_sms - 1) / ctx->n_sms;
-            threads = std::max(32, std::min(512, floor_pow2(std::max<int64_t>(1, 1024 / blocks_per_sm))));
+            if (blocks_per_sm > 1) threads = std::max(32, std::min(512, floor_pow2(std::max<int64_t>(1, 1024 / blocks_per_sm))));
         }
-        threads = std::min(threads, 512);                   // the halo kernel is compiled for blocks of <= 512 threads
+        threads = std::min(threads, hea::kMc2MaxThreads);   // the halo kernel is compiled for blocks of at most this size
         void* team_ctl = nullptr;
         if (team > 1) {
             int rc = ensure_scratch(ctx, 5, hea::mc2_team_bytes(C));

@@ -14,7 +14,6 @@
 //  * Whether b is a neighbour of a (the exclusion of D9.2) comes from the lattice coordinates of the two sites
 //    (minimum-image displacement, squared length == shell distance), not from a compare per table entry.
 //  * Shell sizes and the basis count are template constants (fcc 12/6/24, bcc 8/6/12), so every gather is unrolled.
-#include <cstdio>
 #include <cstring>
 #include <type_traits>
 
@@ -45,6 +44,8 @@ struct Geo {
     int distinct;                 // every L >= 3: a site pair is joined by at most one lattice vector of a shell
 };
 
+constexpr int kQueueCap = 2048;
+
 struct Sh2 {
     int cnt[kSMM];
     double J;
@@ -59,6 +60,12 @@ struct Sh2 {
     MoveRec cand[32];             // improving records of the 32 groups of a round
     int4 wdesc[24];               // accumulator word w -> (int4 index in the offset row, slot mask, shell, side)
     double g[kSMM], t[kSMM];      // objective constants with a per-lane index
+    // two-stage evaluation of long windows: integer pre-filter on shell 1, survivors queued for the full evaluation
+    float fb2[64];                // first-shell cell (i, j): 2 (N_ij - n*_ij), n* = the count at which alpha = target
+    float fwg[64];                //                          w_1 g_ij^2
+    uint32_t q_n[3];              // queue fill, triple-buffered like best[]
+    uint32_t q_pad;
+    uint32_t queue[kQueueCap];    // keys of the candidates that passed the pre-filter
 };
 
 struct SiteC {
@@ -337,6 +344,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     if (tid == 0) {
         sh.n_accept = g_stats[0]; sh.n_null = 0; sh.hash = g_stats[2]; sh.last_accept = g_stats[3]; sh.n_logged = 0;
         sh.best[0] = sh.best[1] = sh.best[2] = kNoKey;
+        sh.q_n[0] = sh.q_n[1] = sh.q_n[2] = 0u;
         sh.rec.key = kNoKey;
     }
     __syncthreads();
@@ -422,47 +430,40 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         __syncthreads();
     };
 
-    // ---- accept engine: one candidate per group of 8 lanes (latency instead of throughput).  Every lane of a group
-    // draws the same proposal; the accumulator words of the 2Z gathers and the S*M rows of the objective are dealt
-    // over the lanes; species counts are combined by xor-shuffles, the rows in the D6 order by indexed shuffles.
-#ifdef HEA_MC2_TIMING
-    long long dbg_seg[6] = {0, 0, 0, 0, 0, 0};
-#endif
-    using PD = typename std::conditional<(M <= 5), uint32_t, uint64_t>::type;     // (M-1) 8-bit fields
-    constexpr int NWR = (2 * (NA0 + NA1 + NA2) + 7) / 8;                          // word rounds per lane
-    constexpr int NRR = (3 * M + 7) / 8;                                          // row rounds per lane
-    const int nw = 2 * (NA0 + (S > 1 ? NA1 : 0) + (S > 2 ? NA2 : 0));
-    auto eval_g8 = [&](unsigned long long step, uint32_t k, bool valid, int grp, int buf, double J_cur) {
-#ifdef HEA_MC2_TIMING
-        const long long dbg_e0 = clock64();
-#endif
-        const int l8 = tid & 7;
+    // D9.1: the proposal of candidate (step, k): sites, their decoded positions and one-hot species (equal codes = null)
+    auto propose = [&](unsigned long long step, uint32_t k, uint32_t& a, uint32_t& b, SiteC& sa, SiteC& sb, uint32_t& hp,
+                       uint32_t& hq) {
         const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), k, chain, key0, key1);
-        uint32_t a = __umulhi(r.x, (uint32_t)N), b = __umulhi(r.y, (uint32_t)N - 1u);
+        a = __umulhi(r.x, (uint32_t)N); b = __umulhi(r.y, (uint32_t)N - 1u);
         b += (b >= a);
-        SiteC sa = decode_site<LAT>(G, a), sb = decode_site<LAT>(G, b);
-        uint32_t hp = occ_get<OCC>(s_occ, sa.pidx), hq = occ_get<OCC>(s_occ, sb.pidx);
+        sa = decode_site<LAT>(G, a); sb = decode_site<LAT>(G, b);
+        hp = occ_get<OCC>(s_occ, sa.pidx); hq = occ_get<OCC>(s_occ, sb.pidx);
         if (hp == hq) {
             a = __umulhi(r.z, (uint32_t)N); b = __umulhi(r.w, (uint32_t)N - 1u);
             b += (b >= a);
             sa = decode_site<LAT>(G, a); sb = decode_site<LAT>(G, b);
             hp = occ_get<OCC>(s_occ, sa.pidx); hq = occ_get<OCC>(s_occ, sb.pidx);
         }
-#ifdef HEA_MC2_TIMING
-        if (tid == 0) dbg_seg[0] += clock64() - dbg_e0;
-#endif
-        const bool live = valid && hp != hq;
-        const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
-        int mm0 = 0, mm1 = 0, mm2 = 0;
+    };
+    // D9.2: per shell, (entries of a's row equal to b) - (entries of a row equal to its own site)
+    auto adjacency = [&](uint32_t a, uint32_t b, const SiteC& sa, const SiteC& sb, int& mm0, int& mm1, int& mm2) {
+        mm0 = 0; mm1 = 0; mm2 = 0;
         if (G.distinct) {
-            const int dx = 2 * (sb.x - sa.x) + (int)((G.basis >> (3 * sb.b)) & 1u) - (int)((G.basis >> (3 * sa.b)) & 1u);
-            const int dy = 2 * (sb.y - sa.y) + (int)((G.basis >> (3 * sb.b + 1)) & 1u) - (int)((G.basis >> (3 * sa.b + 1)) & 1u);
-            const int dz = 2 * (sb.z - sa.z) + (int)((G.basis >> (3 * sb.b + 2)) & 1u) - (int)((G.basis >> (3 * sa.b + 2)) & 1u);
-            const int wx = dx > Lx ? dx - 2 * Lx : dx < -Lx ? dx + 2 * Lx : dx;
-            const int wy = dy > Ly ? dy - 2 * Ly : dy < -Ly ? dy + 2 * Ly : dy;
-            const int wz = dz > Lz ? dz - 2 * Lz : dz < -Lz ? dz + 2 * Lz : dz;
-            const int r2 = wx * wx + wy * wy + wz * wz;
-            mm0 = r2 == G.d2[0]; mm1 = r2 == G.d2[1]; mm2 = r2 == G.d2[2];
+            // neighbours of any shell sit in cells at most one apart (periodically): almost every pair fails this test
+            const int cx = sb.x - sa.x, cy = sb.y - sa.y, cz = sb.z - sa.z;
+            const bool nx = (uint32_t)(cx + 1) <= 2u || cx == Lx - 1 || cx == 1 - Lx;
+            const bool ny = (uint32_t)(cy + 1) <= 2u || cy == Ly - 1 || cy == 1 - Ly;
+            const bool nz = (uint32_t)(cz + 1) <= 2u || cz == Lz - 1 || cz == 1 - Lz;
+            if (nx && ny && nz) {
+                const int dx = 2 * cx + (int)((G.basis >> (3 * sb.b)) & 1u) - (int)((G.basis >> (3 * sa.b)) & 1u);
+                const int dy = 2 * cy + (int)((G.basis >> (3 * sb.b + 1)) & 1u) - (int)((G.basis >> (3 * sa.b + 1)) & 1u);
+                const int dz = 2 * cz + (int)((G.basis >> (3 * sb.b + 2)) & 1u) - (int)((G.basis >> (3 * sa.b + 2)) & 1u);
+                const int wx = dx > Lx ? dx - 2 * Lx : dx < -Lx ? dx + 2 * Lx : dx;
+                const int wy = dy > Ly ? dy - 2 * Ly : dy < -Ly ? dy + 2 * Ly : dy;
+                const int wz = dz > Lz ? dz - 2 * Lz : dz < -Lz ? dz + 2 * Lz : dz;
+                const int r2 = wx * wx + wy * wy + wz * wz;
+                mm0 = r2 == G.d2[0]; mm1 = r2 == G.d2[1]; mm2 = r2 == G.d2[2];
+            }
         } else {
             const int32_t* row = nbr + (size_t)a * P.Z;
             for (int e = 0; e < P.Z; ++e) {
@@ -471,9 +472,24 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             }
             mm0 -= P.m_self[0]; mm1 -= P.m_self[1]; mm2 -= P.m_self[2];
         }
-#ifdef HEA_MC2_TIMING
-        if (tid == 0) dbg_seg[1] += clock64() - dbg_e0;
-#endif
+    };
+
+    // ---- accept engine: one candidate per group of 8 lanes (latency instead of throughput).  Every lane of a group
+    // draws the same proposal; the accumulator words of the 2Z gathers and the S*M rows of the objective are dealt
+    // over the lanes; species counts are combined by xor-shuffles, the rows in the D6 order by indexed shuffles.
+    using PD = typename std::conditional<(M <= 5), uint32_t, uint64_t>::type;     // (M-1) 8-bit fields
+    constexpr int NWR = (2 * (NA0 + NA1 + NA2) + 7) / 8;                          // word rounds per lane
+    constexpr int NRR = (3 * M + 7) / 8;                                          // row rounds per lane
+    const int nw = 2 * (NA0 + (S > 1 ? NA1 : 0) + (S > 2 ? NA2 : 0));
+    auto eval_g8 = [&](unsigned long long step, uint32_t k, bool valid, int grp, int buf, double J_cur) {
+        const int l8 = tid & 7;
+        uint32_t a, b, hp, hq;
+        SiteC sa, sb;
+        propose(step, k, a, b, sa, sb, hp, hq);
+        const bool live = valid && hp != hq;
+        const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+        int mm0, mm1, mm2;
+        adjacency(a, b, sa, sb, mm0, mm1, mm2);
         // gathers: this lane's accumulator words -> biased species counts (+ for b's neighbours, - for a's)
         PD D0 = 0, D1 = 0, D2 = 0;
         PD bias4 = 0;
@@ -508,9 +524,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 D0 += dsc.z == 0 ? v : (PD)0; D1 += dsc.z == 1 ? v : (PD)0; D2 += dsc.z == 2 ? v : (PD)0;
             }
         }
-#ifdef HEA_MC2_TIMING
-        if (tid == 0) dbg_seg[2] += clock64() - dbg_e0;
-#endif
 #pragma unroll
         for (int o = 1; o < 8; o <<= 1) {
             D0 += __shfl_xor_sync(0xFFFFFFFFu, D0, o);
@@ -542,9 +555,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
 #pragma unroll
             for (int r2 = 0; r2 < M; ++r2) { F0[r2] -= mm0 * c[r2]; F1[r2] -= mm1 * c[r2]; F2[r2] -= mm2 * c[r2]; }
         }
-#ifdef HEA_MC2_TIMING
-        if (tid == 0) dbg_seg[3] += clock64() - dbg_e0;
-#endif
         // rows of the objective: row rho = s*M + i on lane rho & 7
         double rowv[NRR];
 #pragma unroll
@@ -566,9 +576,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             }
             rowv[rr] = row;
         }
-#ifdef HEA_MC2_TIMING
-        if (tid == 0) dbg_seg[4] += clock64() - dbg_e0;
-#endif
         // D6 combination: rows in order within a shell, shells in order
         double Jk = 0.0;
 #pragma unroll
@@ -585,9 +592,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[s], shs));
             }
         }
-#ifdef HEA_MC2_TIMING
-        if (tid == 0) dbg_seg[5] += clock64() - dbg_e0;
-#endif
         if (l8 == 0 && live && Jk < J_cur) {
             MoveRec& m = sh.cand[grp];
             m.key = k; m.a = a; m.b = b; m.pq = (uint32_t)p | ((uint32_t)q << 8); m.J = Jk;
@@ -603,11 +607,8 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     uint32_t it = 0;                                         // windows evaluated by this block
     uint32_t tw = 0;                                         // TEAM windows so far (same in every block of the team)
     uint32_t phase = 0;                                      // phase records consumed / posted
+    double slack_J = -1.0;                                   // J the pre-filter intervals were computed for (J >= 0 always)
 
-#ifdef HEA_MC2_TIMING
-    long long dbg_eval = 0, dbg_bar = 0, dbg_apply = 0, dbg_steps = 0, dbg_cd = 0, dbg_da = 0, dbg_lastC = 0, dbg_lastD = 0;
-    const long long dbg_t0 = clock64();
-#endif
     while (t0 < t_end) {
         if (R > 1 && !team && rank != 0) {
             // ---- follower in a SOLO phase: wait for the leader's phase record, reload, join the team
@@ -632,10 +633,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             // ---- accept engine: this one step, 32 candidates per round on the first 8 warps; the other warps settle
             // which candidates of the step are null (all K count, D9.1)
             const double J_cur = sh.J;
-#ifdef HEA_MC2_TIMING
-            const long long tA = clock64();
-            if (dbg_lastD) dbg_da += tA - dbg_lastD;
-#endif
             if (tid >= 256) {
                 for (uint32_t k = (uint32_t)tid - 256u; k < (uint32_t)K; k += (uint32_t)T - 256u) {
                     const uint4 r = philox4x32_10((uint32_t)t0, (uint32_t)(t0 >> 32), k, chain, key0, key1);
@@ -657,28 +654,14 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     const uint32_t k = rd0 + ((uint32_t)tid >> 3);
                     eval_g8(t0, k, k < (uint32_t)K, tid >> 3, buf, J_cur);
                 }
-#ifdef HEA_MC2_TIMING
-                const long long tB = clock64();
-#endif
                 __syncthreads();
-#ifdef HEA_MC2_TIMING
-                const long long tC = clock64();
-                dbg_eval += tB - tA; dbg_bar += tC - tB; dbg_lastC = tC;
-#endif
                 key_best = sh.best[buf];
-                if (tid == 0) sh.best[(buf + 2) % 3] = kNoKey;
+                if (tid == 0) { sh.best[(buf + 2) % 3] = kNoKey; sh.q_n[(buf + 2) % 3] = 0u; }
                 ++it;
                 if (key_best != kNoKey) break;
             }
             if (key_best != kNoKey) {
-#ifdef HEA_MC2_TIMING
-                const long long tD = clock64();
-#endif
                 apply_move(&sh.cand[key_best - rd0], key_best, t0);
-#ifdef HEA_MC2_TIMING
-                dbg_apply += clock64() - tD; dbg_steps += 1; dbg_cd += tD - dbg_lastC;
-                dbg_lastD = clock64();
-#endif
                 W = 1u;
             } else {
                 W = min(2u, w_cap);
@@ -693,104 +676,149 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             double win_J = 0.0;
             uint64_t nullmask = 0;
 
+            // ---- long windows run in two stages: an integer pre-filter on the first shell (a candidate can only
+            // improve if w_1 e_ij(N_ij + dN_ij) < J_cur for every cell, i.e. dN_ij inside a precomputed interval),
+            // survivors queued and evaluated in full afterwards -- so that a few survivors do not hold whole warps
+            const bool use_filter = SYM && prune && Kc.w[0] > 0.0 && (unsigned long long)Wc * (unsigned)K >= 2ull * GT;
+            float filt_T0 = 0.0f, filt_thr = 0.0f;
+            if (use_filter) {
+                if (!(slack_J == J_cur)) {
+                    for (int idx = tid; idx < MM; idx += T) {
+                        const double gi = sh.g[idx];
+                        sh.fb2[idx] = (float)(2.0 * ((double)sh.cnt[idx] - (1.0 - sh.t[idx]) / gi));
+                        sh.fwg[idx] = (float)(Kc.w[0] * gi * gi);
+                    }
+                    slack_J = J_cur;
+                    __syncthreads();
+                }
+                for (int idx = 0; idx < MM; ++idx) { const float hb = 0.5f * sh.fb2[idx]; filt_T0 = fmaf(sh.fwg[idx] * hb, hb, filt_T0); }
+                filt_thr = fmaxf((float)J_cur * 1.002f, 1.0e-30f);
+            }
+            // the part of an evaluation after the first shell's F: D6 objective shell by shell with the exact pruning
+            auto eval_rest = [&](uint32_t key, uint32_t a, uint32_t b, const SiteC& sa, const SiteC& sb, int p, int q,
+                                 const int (&c)[M], int mm1, int mm2, const int (&F0)[M]) {
+                const int4* ta = reinterpret_cast<const int4*>(s_tab + sa.b * ZP);
+                const int4* tb = reinterpret_cast<const int4*>(s_tab + sb.b * ZP);
+                int F1[M], F2[M];
+#pragma unroll
+                for (int r2 = 0; r2 < M; ++r2) { F1[r2] = 0; F2[r2] = 0; }
+                double Jk = __dmul_rn(Kc.w[0], shell_sum_F<M, SYM>(sh.cnt, Kc.g, Kc.t, F0, c));
+                Jk = __dadd_rn(0.0, Jk);
+                if (S > 1 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
+                    {
+                        uint32_t xa[NA1], xb[NA1];
+                        gather_shell<OCC, LC::z1>(s_occ, ta + NA0, sa.pidx, xa);
+                        gather_shell<OCC, LC::z1>(s_occ, tb + NA0, sb.pidx, xb);
+                        hist_diff<M, NA1>(xa, xb, F1);
+#pragma unroll
+                        for (int r2 = 0; r2 < M; ++r2) F1[r2] -= mm1 * c[r2];
+                    }
+                    Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[1], shell_sum_F<M, SYM>(sh.cnt + MM, Kc.g + MM, Kc.t + MM, F1, c)));
+                    if (S > 2 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
+                        {
+                            uint32_t xa[NA2], xb[NA2];
+                            gather_shell<OCC, LC::z2>(s_occ, ta + NA0 + NA1, sa.pidx, xa);
+                            gather_shell<OCC, LC::z2>(s_occ, tb + NA0 + NA1, sb.pidx, xb);
+                            hist_diff<M, NA2>(xa, xb, F2);
+#pragma unroll
+                            for (int r2 = 0; r2 < M; ++r2) F2[r2] -= mm2 * c[r2];
+                        }
+                        Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[2], shell_sum_F<M, SYM>(sh.cnt + 2 * MM, Kc.g + 2 * MM, Kc.t + 2 * MM, F2, c)));
+                    } else if (S > 2) {
+                        Jk = J_cur;                       // pruned: not improving
+                    }
+                } else if (S > 1) {
+                    Jk = J_cur;
+                }
+                if (Jk < J_cur && key < win_key) {
+                    win_key = key; win_a = a; win_b = b; win_pq = (uint32_t)p | ((uint32_t)q << 8);
+                    win_d0 = pack_F<M>(F0); win_d1 = pack_F<M>(F1); win_d2 = pack_F<M>(F2); win_J = Jk;
+                    atomicMin(&sh.best[buf], key);
+                }
+            };
+            // first-shell species-count differences of a non-null candidate
+            auto first_shell = [&](const SiteC& sa, const SiteC& sb, int mm0, const int (&c)[M], int (&F0)[M]) {
+                uint32_t xa[NA0], xb[NA0];
+                gather_shell<OCC, LC::z0>(s_occ, reinterpret_cast<const int4*>(s_tab + sa.b * ZP), sa.pidx, xa);
+                gather_shell<OCC, LC::z0>(s_occ, reinterpret_cast<const int4*>(s_tab + sb.b * ZP), sb.pidx, xb);
+                hist_diff<M, NA0>(xa, xb, F0);
+#pragma unroll
+                for (int r2 = 0; r2 < M; ++r2) F0[r2] -= mm0 * c[r2];
+            };
+
             uint32_t ts = ts_first, k = k_first;
             for (int j = 0; ts < Wc; ++j) {
                 const uint32_t hint = *best_slot;
                 if ((hint >> 10) < ts) break;                       // a move at an earlier step exists: this step is void
                 const uint32_t key = (ts << 10) | k;
-                // ---- D9.1 proposal
-                const unsigned long long step = t0 + ts;
-                const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), k, chain, key0, key1);
-                uint32_t a = __umulhi(r.x, (uint32_t)N), b = __umulhi(r.y, (uint32_t)N - 1u);
-                b += (b >= a);
-                SiteC sa = decode_site<LAT>(G, a), sb = decode_site<LAT>(G, b);
-                uint32_t hp = occ_get<OCC>(s_occ, sa.pidx), hq = occ_get<OCC>(s_occ, sb.pidx);
-                if (hp == hq) {
-                    a = __umulhi(r.z, (uint32_t)N); b = __umulhi(r.w, (uint32_t)N - 1u);
-                    b += (b >= a);
-                    sa = decode_site<LAT>(G, a); sb = decode_site<LAT>(G, b);
-                    hp = occ_get<OCC>(s_occ, sa.pidx); hq = occ_get<OCC>(s_occ, sb.pidx);
-                }
+                uint32_t a, b, hp, hq;
+                SiteC sa, sb;
+                propose(t0 + ts, k, a, b, sa, sb, hp, hq);
                 if (hp == hq) {
                     nullmask |= 1ull << j;
                 } else if (key < hint) {                             // same step, higher k than a known move: only nullness counts
                     const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
-                    int c[M];
-    #pragma unroll
+                    int c[M], F0[M];
+#pragma unroll
                     for (int r2 = 0; r2 < M; ++r2) c[r2] = (r2 == p) - (r2 == q);
-                    // ---- D9.2: is b an entry of a's rows?  (excluded sum = plain sum + (m - m_self)(e_q - e_p))
-                    int mm0 = 0, mm1 = 0, mm2 = 0;
-                    if (G.distinct) {
-                        const int dx = 2 * (sb.x - sa.x) + (int)((G.basis >> (3 * sb.b)) & 1u) - (int)((G.basis >> (3 * sa.b)) & 1u);
-                        const int dy = 2 * (sb.y - sa.y) + (int)((G.basis >> (3 * sb.b + 1)) & 1u) - (int)((G.basis >> (3 * sa.b + 1)) & 1u);
-                        const int dz = 2 * (sb.z - sa.z) + (int)((G.basis >> (3 * sb.b + 2)) & 1u) - (int)((G.basis >> (3 * sa.b + 2)) & 1u);
-                        const int wx = dx > Lx ? dx - 2 * Lx : dx < -Lx ? dx + 2 * Lx : dx;
-                        const int wy = dy > Ly ? dy - 2 * Ly : dy < -Ly ? dy + 2 * Ly : dy;
-                        const int wz = dz > Lz ? dz - 2 * Lz : dz < -Lz ? dz + 2 * Lz : dz;
-                        const int r2 = wx * wx + wy * wy + wz * wz;
-                        mm0 = r2 == G.d2[0]; mm1 = r2 == G.d2[1]; mm2 = r2 == G.d2[2];
-                    } else {
-                        const int32_t* row = nbr + (size_t)a * P.Z;
-                        for (int e = 0; e < P.Z; ++e) {
-                            const int hit = (uint32_t)__ldg(row + e) == b;
-                            if (e < P.zoff[1]) mm0 += hit; else if (e < P.zoff[2]) mm1 += hit; else mm2 += hit;
+                    int mm0, mm1, mm2;
+                    adjacency(a, b, sa, sb, mm0, mm1, mm2);
+                    first_shell(sa, sb, mm0, c, F0);
+                    bool full = true;
+                    if (use_filter) {
+                        // fp32 model of w_1 sh_1 after the move: T0 + sum over the changed cells of w g^2 dN (2 b + dN),
+                        // rows p and q (dN_pj = F_j + c_j F_p, dN_qj = -F_j + c_j F_q), the mirrored cells (j, p), (j, q)
+                        // through the weight 2 - |c_j|.  Relative error ~1e-6; the threshold carries a 2e-3 margin.
+                        int Fp = 0, Fq = 0;
+#pragma unroll
+                        for (int r2 = 0; r2 < M; ++r2) { Fp = c[r2] > 0 ? F0[r2] : Fp; Fq = c[r2] < 0 ? F0[r2] : Fq; }
+                        const float* b2p = sh.fb2 + p * M; const float* wgp = sh.fwg + p * M;
+                        const float* b2q = sh.fb2 + q * M; const float* wgq = sh.fwg + q * M;
+                        float lb = filt_T0;
+#pragma unroll
+                        for (int r2 = 0; r2 < M; ++r2) {
+                            const float cw = c[r2] != 0 ? 1.0f : 2.0f;
+                            const float dp = __int_as_float(0x4B400000 + (F0[r2] + c[r2] * Fp)) - 12582912.0f;
+                            const float dq = __int_as_float(0x4B400000 + (c[r2] * Fq - F0[r2])) - 12582912.0f;
+                            lb = fmaf(dp * (b2p[r2] + dp) * wgp[r2], cw, lb);
+                            lb = fmaf(dq * (b2q[r2] + dq) * wgq[r2], cw, lb);
                         }
-                        mm0 -= P.m_self[0]; mm1 -= P.m_self[1]; mm2 -= P.m_self[2];
-                    }
-                    const int4* ta = reinterpret_cast<const int4*>(s_tab + sa.b * ZP);
-                    const int4* tb = reinterpret_cast<const int4*>(s_tab + sb.b * ZP);
-                    // ---- D6 objective from counts + delta, shell by shell with the exact lower-bound pruning (hea_mc.cu)
-                    int F0[M], F1[M], F2[M];
-    #pragma unroll
-                    for (int r2 = 0; r2 < M; ++r2) { F1[r2] = 0; F2[r2] = 0; }
-                    {
-                        uint32_t xa[NA0], xb[NA0];
-                        gather_shell<OCC, LC::z0>(s_occ, ta, sa.pidx, xa);
-                        gather_shell<OCC, LC::z0>(s_occ, tb, sb.pidx, xb);
-                        hist_diff<M, NA0>(xa, xb, F0);
-    #pragma unroll
-                        for (int r2 = 0; r2 < M; ++r2) F0[r2] -= mm0 * c[r2];
-                    }
-                    double Jk = __dmul_rn(Kc.w[0], shell_sum_F<M, SYM>(sh.cnt, Kc.g, Kc.t, F0, c));
-                    Jk = __dadd_rn(0.0, Jk);
-                    if (S > 1 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
-                        {
-                            uint32_t xa[NA1], xb[NA1];
-                            gather_shell<OCC, LC::z1>(s_occ, ta + NA0, sa.pidx, xa);
-                            gather_shell<OCC, LC::z1>(s_occ, tb + NA0, sb.pidx, xb);
-                            hist_diff<M, NA1>(xa, xb, F1);
-    #pragma unroll
-                            for (int r2 = 0; r2 < M; ++r2) F1[r2] -= mm1 * c[r2];
+                        const bool out = lb > filt_thr;
+                        full = !out;
+                        if (full) {
+                            const uint32_t slot = atomicAdd(&sh.q_n[buf], 1u);
+                            if (slot < (uint32_t)kQueueCap) { sh.queue[slot] = key; full = false; }
                         }
-                        Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[1], shell_sum_F<M, SYM>(sh.cnt + MM, Kc.g + MM, Kc.t + MM, F1, c)));
-                        if (S > 2 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
-                            {
-                                uint32_t xa[NA2], xb[NA2];
-                                gather_shell<OCC, LC::z2>(s_occ, ta + NA0 + NA1, sa.pidx, xa);
-                                gather_shell<OCC, LC::z2>(s_occ, tb + NA0 + NA1, sb.pidx, xb);
-                                hist_diff<M, NA2>(xa, xb, F2);
-    #pragma unroll
-                                for (int r2 = 0; r2 < M; ++r2) F2[r2] -= mm2 * c[r2];
-                            }
-                            Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[2], shell_sum_F<M, SYM>(sh.cnt + 2 * MM, Kc.g + 2 * MM, Kc.t + 2 * MM, F2, c)));
-                        } else if (S > 2) {
-                            Jk = J_cur;                       // pruned: not improving
-                        }
-                    } else if (S > 1) {
-                        Jk = J_cur;
                     }
-                    if (Jk < J_cur && win_key == kNoKey) {
-                        win_key = key; win_a = a; win_b = b; win_pq = (uint32_t)p | ((uint32_t)q << 8);
-                        win_d0 = pack_F<M>(F0); win_d1 = pack_F<M>(F1); win_d2 = pack_F<M>(F2); win_J = Jk;
-                        atomicMin(&sh.best[buf], key);
-                    }
+                    if (full) eval_rest(key, a, b, sa, sb, p, q, c, mm1, mm2, F0);
                 }
                 k += k_inc; ts += ts_inc;
                 if (k >= (uint32_t)K) { k -= (uint32_t)K; ++ts; }
             }
+            if (use_filter) {
+                // ---- second stage: the queued survivors, one per thread
+                __syncthreads();
+                const uint32_t nq = min(sh.q_n[buf], (uint32_t)kQueueCap);
+                for (uint32_t i = (uint32_t)tid; i < nq; i += (uint32_t)T) {
+                    const uint32_t key = sh.queue[i];
+                    const uint32_t hint = *best_slot;
+                    if (!(key < hint)) continue;
+                    uint32_t a, b, hp, hq;
+                    SiteC sa, sb;
+                    propose(t0 + (key >> 10), key & 1023u, a, b, sa, sb, hp, hq);
+                    const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+                    int c[M], F0[M];
+#pragma unroll
+                    for (int r2 = 0; r2 < M; ++r2) c[r2] = (r2 == p) - (r2 == q);
+                    int mm0, mm1, mm2;
+                    adjacency(a, b, sa, sb, mm0, mm1, mm2);
+                    first_shell(sa, sb, mm0, c, F0);
+                    eval_rest(key, a, b, sa, sb, p, q, c, mm1, mm2, F0);
+                }
+            }
             __syncthreads();                                        // B1: window evaluated, local minimum posted
             key_best = sh.best[buf];
-            if (tid == 0) sh.best[(buf + 2) % 3] = kNoKey;          // next user of that slot is two barriers away
+            if (tid == 0) { sh.best[(buf + 2) % 3] = kNoKey; sh.q_n[(buf + 2) % 3] = 0u; }   // next user of these slots is two barriers away
 
             const int lane = tid & 31;
             if (team) {
@@ -877,14 +905,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         }
     }
 
-#ifdef HEA_MC2_TIMING
-    if (tid == 0 && blockIdx.x == 0 && dbg_steps > 0) {
-        printf("mc2 eval segments (cumulative): proposal %lld adjacency %lld gathers %lld reduce+F %lld rows %lld combine %lld\n",
-               dbg_seg[0] / dbg_steps, dbg_seg[1] / dbg_steps, dbg_seg[2] / dbg_steps, dbg_seg[3] / dbg_steps, dbg_seg[4] / dbg_steps, dbg_seg[5] / dbg_steps);
-        printf("mc2 timing: steps %lld eval %lld bar %lld c->d %lld apply %lld d->a %lld loop-total %lld (cycles per step)\n", dbg_steps,
-               dbg_eval / dbg_steps, dbg_bar / dbg_steps, dbg_cd / dbg_steps, dbg_apply / dbg_steps, dbg_da / dbg_steps, (clock64() - dbg_t0) / dbg_steps);
-    }
-#endif
     // ---- epilogue: release waiting followers, write back (rank 0 owns the global copy; nulls are summed over blocks)
     if (R > 1 && rank == 0 && !team) {
         __syncthreads();
