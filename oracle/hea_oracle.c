@@ -400,6 +400,77 @@ static void mc_chain(const ora_sys *sy, uint8_t *occ, int32_t *counts, uint64_t 
     st->J = J_cur;
 }
 
+/* ---- the paper's own selection and termination, as options (Eq. 6: F_best = min over the
+ * candidates; Alg. 3 P:244-250 and section 4.6.4: a search-depth counter, reset when a better solution is
+ * found, incremented otherwise, the search ending when it reaches its threshold or after the maximum number of steps).
+ * Reading (A23): select_best != 0 -> the candidate with the smallest J_k is taken (ties -> lowest k) and
+ * applied iff J_k < J_cur (tolerance 0, as in D9); depth = consecutive steps without an applied move; with
+ * depth_limit > 0 a chain stops as soon as depth == depth_limit (a chain entering with depth >= depth_limit does nothing).
+ * depth is in/out so that split runs continue exactly; *steps_done = steps executed by this call.
+ * Every K candidates are evaluated in best mode (the minimum needs all of them). */
+static void mc_chain_ex(const ora_sys *sy, uint8_t *occ, int32_t *counts, uint64_t n_steps, int K, uint64_t seed,
+                        uint64_t chain, uint64_t step0, ora_stats *st, ora_move *log, int64_t log_cap,
+                        int select_best, uint64_t depth_limit, uint64_t *depth_io, uint64_t *steps_done)
+{
+    int sz = sy->S * sy->M * sy->M;
+    int32_t trial[ORA_MAX_SHELLS*ORA_MAX_SPECIES*ORA_MAX_SPECIES];
+    int32_t chosen[ORA_MAX_SHELLS*ORA_MAX_SPECIES*ORA_MAX_SPECIES];
+    double J_cur = ora_objective(sy, counts);
+    int64_t n_logged = 0;
+    uint64_t depth = depth_io ? *depth_io : 0;
+    uint64_t t = 0;
+    for (; t < n_steps; t++) {
+        if (depth_limit > 0 && depth >= depth_limit) break;
+        uint64_t step = step0 + t;
+        int found = 0; uint32_t ks = 0, as = 0, bs = 0; double Js = 0.0;
+        for (int k = 0; k < K; k++) {
+            uint32_t a, b;
+            if (!ora_propose(sy, occ, seed, chain, step, (uint32_t)k, &a, &b)) { st->n_null++; continue; }
+            if (found && !select_best) continue;
+            memcpy(trial, counts, sizeof(int32_t)*sz);
+            ora_delta_counts(sy, occ, a, b, trial);
+            double Jk = ora_objective(sy, trial);
+            int take = select_best ? (Jk < J_cur && (!found || Jk < Js))      /* strict: ties keep the lower k */
+                                   : (!found && Jk < J_cur);
+            if (take) {
+                found = 1; ks = (uint32_t)k; as = a; bs = b; Js = Jk;
+                memcpy(chosen, trial, sizeof(int32_t)*sz);
+            }
+        }
+        if (found) {
+            uint8_t tmp = occ[as]; occ[as] = occ[bs]; occ[bs] = tmp;
+            memcpy(counts, chosen, sizeof(int32_t)*sz);
+            J_cur = Js;
+            st->n_accept++;
+            st->last_accept_step = step;
+            uint64_t h = st->hash;
+            h = hash_word(h, (uint32_t)step); h = hash_word(h, (uint32_t)(step >> 32));
+            h = hash_word(h, ks); h = hash_word(h, as); h = hash_word(h, bs);
+            st->hash = h;
+            if (log && n_logged < log_cap) { ora_move m = { step, ks, as, bs }; log[n_logged++] = m; }
+            depth = 0;
+        } else {
+            depth++;
+        }
+    }
+    st->J = J_cur;
+    if (depth_io) *depth_io = depth;
+    if (steps_done) *steps_done = t;
+}
+
+/* single-threaded over the chains (a test oracle, not the timed baseline) */
+int ora_mc_run_ex(const ora_sys *sy, uint8_t *occ, int32_t *counts, int64_t C, uint64_t n_steps, int K,
+                  uint64_t seed, uint64_t chain0, uint64_t step0, ora_stats *stats, ora_move *log, int64_t log_cap,
+                  int select_best, uint64_t depth_limit, uint64_t *depth_io, uint64_t *steps_done)
+{
+    int sz = sy->S * sy->M * sy->M;
+    for (int64_t c = 0; c < C; c++)
+        mc_chain_ex(sy, occ + c*sy->N, counts + c*sz, n_steps, K, seed, chain0 + (uint64_t)c, step0, stats + c,
+                    log ? log + c*log_cap : NULL, log_cap, select_best, depth_limit,
+                    depth_io ? depth_io + c : NULL, steps_done ? steps_done + c : NULL);
+    return 1;
+}
+
 typedef struct {
     const ora_sys *sy; uint8_t *occ; int32_t *counts; int64_t c_begin, c_end; uint64_t n_steps; int K;
     uint64_t seed, chain0, step0; ora_stats *stats; ora_move *log; int64_t log_cap; int eval_all;

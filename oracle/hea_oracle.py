@@ -56,6 +56,8 @@ def lib():
         L.ora_delta_counts.argtypes = [vp, vp, u32, u32, vp]
         L.ora_mc_run.restype = i32
         L.ora_mc_run.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp, vp, i64, i32, i32]
+        L.ora_mc_run_ex.restype = i32
+        L.ora_mc_run_ex.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp, vp, i64, i32, u64, vp, vp]
         _lib = L
     return _lib
 
@@ -166,3 +168,17 @@ class Oracle:
                                 _p(log), log_cap, n_threads, 1 if eval_all else 0)
         self.threads_used = used
         return stats, log
+
+    def mc_run_ex(self, occ, counts, n_steps, K, seed, chain0=0, step0=0, stats=None, log_cap=0, select_best=False,
+                  depth_limit=0, depth=None):
+        """SURVEY 8f-1 options: best-of-K selection, search-depth termination.  Returns (stats, log, depth, steps_done)."""
+        n = occ.shape[0]
+        if stats is None:
+            stats = fresh_stats(n)
+        if depth is None:
+            depth = np.zeros(n, dtype=np.uint64)
+        steps_done = np.zeros(n, dtype=np.uint64)
+        log = np.zeros((n, log_cap), dtype=MOVE_DTYPE) if log_cap > 0 else None
+        lib().ora_mc_run_ex(self._h, _p(occ), _p(counts), n, n_steps, K, seed, chain0, step0, _p(stats), _p(log),
+                            log_cap, 1 if select_best else 0, depth_limit, _p(depth), _p(steps_done))
+        return stats, log, depth, steps_done

@@ -264,6 +264,30 @@ def test_mc_c3_many_chains_through_convergence(hb):
     assert (st["n_accept"] > 1000).all()
 
 
+def test_fig3_workflow_non_equiatomic_target_from_small_cell(hb):
+    # SURVEY 8f-3 / PAPER.md Fig. 3: a 500-atom Fe40Mn40Cr10Co10 cell is refined, its measured alpha becomes the target
+    # of the 256,000-atom cell; every stage GPU == oracle (exercises c_j != 1/M in g_ij and in the sum rule)
+    ws = wl.fig3_small_workload(2000)
+    h, o = pair(hb, ws)
+    st = run_both(hb, ws, 1, 2000, log_cap=0)
+    occ = h.init_random(1, seed=ws.seed)
+    cnt, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    h.mc_run(occ, cnt, 2000, ws.K, ws.seed)
+    _, alpha, _ = h.sro_full(occ, want_alpha=True)
+    o_occ = o.init_random(1, ws.seed)
+    o_cnt, _, _ = o.sro_full(o_occ)
+    o.mc_run(o_occ, o_cnt, 2000, ws.K, ws.seed, eval_all=False)
+    _, o_alpha, _ = o.sro_full(o_occ)
+    a = alpha.cpu().numpy()
+    np.testing.assert_array_equal(a, o_alpha)
+    conc = np.asarray(ws.conc)
+    np.testing.assert_allclose((a[0] * conc[None, None, :]).sum(-1), 0.0, atol=1e-12)       # sum_j c_j alpha_ij = 0
+    np.testing.assert_array_equal(a[0], np.swapaxes(a[0], -1, -2))                            # alpha symmetric (A17)
+    wlg = wl.fig3_large_workload(a[0], n_chains=4)
+    st = run_both(hb, wlg, 4, 3000, log_cap=64, threads=4)
+    assert (st["n_accept"] > 2000).all()
+
+
 def test_mc_c4_global_occupancy_path(hb):
     w = wl.config(4)
     run_both(hb, w, 2, 100, opts={"mc_occ_mode": 3, "mc_cluster": 8})

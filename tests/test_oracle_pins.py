@@ -432,3 +432,94 @@ def test_survey_crosscheck_trajectories(rec):
         s, k, a, b = (int(x) for x in mv.split(":"))
         m = log[0][i]
         assert (int(m["step"]), int(m["k"]), int(m["a"]), int(m["b"])) == (s, k, a, b)
+
+
+# ---- best-of-K selection (Eq. 6) and search-depth termination (Alg. 3)
+@pytest.mark.parametrize("lattice,dims,conc,S,K", [("bcc", (2, 2, 3), [0.5, 0.5], 2, 6), ("fcc", (2, 2, 2), [0.25] * 4, 3, 8),
+                                                   ("bcc", (3, 3, 3), [0.5, 0.25, 0.25], 2, 5)])
+@pytest.mark.parametrize("depth_limit", [0, 3])
+def test_mc_ex_best_of_K_and_depth_by_full_recount(lattice, dims, conc, S, K, depth_limit):
+    """Every step re-derived in Python: proposals from the pinned Philox, every candidate's J from a FULL recount, the
+    minimum J (ties -> lowest k) applied iff it improves; depth = consecutive steps without a move; stop at the limit."""
+    M = len(conc)
+    rng = np.random.default_rng(2)
+    tgt = rng.uniform(-0.2, 0.2, size=(S, M, M))
+    o = make(lattice, dims, conc, S, target=tgt)
+    seed, chain0, step0, n_steps = 91, 5, 17, 60
+    occ = o.init_random(2, seed=seed, chain0=chain0)
+    counts = np.stack([o.pair_counts(occ[c]) for c in range(2)])
+    ref_occ = occ.copy()
+    stats, log, depth, steps_done = o.mc_run_ex(occ, counts, n_steps, K, seed, chain0=chain0, step0=step0, log_cap=64,
+                                                select_best=True, depth_limit=depth_limit)
+    for c in range(2):
+        x = ref_occ[c].copy()
+        J_cur = o.objective(o.pair_counts(x))
+        n_acc = n_null = d = t_done = 0
+        h, moves = ho.HASH0, []
+        for t in range(n_steps):
+            if depth_limit and d >= depth_limit:
+                break
+            step = step0 + t
+            best = None
+            for k in range(K):
+                ok, a, b = py_propose(o, x, seed, chain0 + c, step, k)
+                if not ok:
+                    n_null += 1
+                    continue
+                y = x.copy()
+                y[a], y[b] = x[b], x[a]
+                Jk = o.objective(o.pair_counts(y))
+                if Jk < J_cur and (best is None or Jk < best[3]):
+                    best = (k, a, b, Jk)
+            if best is not None:
+                k, a, b, Jk = best
+                x[a], x[b] = x[b], x[a]
+                J_cur = Jk
+                n_acc += 1
+                d = 0
+                for word in (step & 0xFFFFFFFF, step >> 32, k, a, b):
+                    h = ((h ^ word) * 0x100000001B3) & 0xFFFFFFFFFFFFFFFF
+                moves.append((step, k, a, b))
+            else:
+                d += 1
+            t_done = t + 1
+        np.testing.assert_array_equal(occ[c], x)
+        np.testing.assert_array_equal(counts[c], o.pair_counts(x))
+        st = stats[c]
+        assert (int(st["n_accept"]), int(st["n_null"]), int(st["hash"])) == (n_acc, n_null, h)
+        assert float(st["J"]) == J_cur
+        assert (int(depth[c]), int(steps_done[c])) == (d, t_done)
+        got = [(int(m["step"]), int(m["k"]), int(m["a"]), int(m["b"])) for m in log[c][:n_acc]]
+        assert got == moves[:64]
+        if depth_limit:
+            assert t_done < n_steps and d == depth_limit          # these small cells do stall within 60 steps
+
+
+def test_mc_ex_reduces_to_the_north_star_rule_and_continues_exactly():
+    o = make("fcc", (3, 3, 3), [0.5, 0.25, 0.25], 2, target=None)
+    seed, K = 5, 12
+    occ0 = o.init_random(3, seed=seed)
+    cnt0 = np.stack([o.pair_counts(occ0[c]) for c in range(3)])
+    # select_best = False, no depth limit == ora_mc_run
+    a_occ, a_cnt = occ0.copy(), cnt0.copy()
+    st_a, _ = o.mc_run(a_occ, a_cnt, 200, K, seed, eval_all=False)
+    b_occ, b_cnt = occ0.copy(), cnt0.copy()
+    st_b, _, _, done = o.mc_run_ex(b_occ, b_cnt, 200, K, seed)
+    np.testing.assert_array_equal(a_occ, b_occ)
+    assert (st_a["hash"] == st_b["hash"]).all() and (done == 200).all()
+    # a split run with the depth carried over equals one run (best-of-K, depth limit 25)
+    c_occ, c_cnt = occ0.copy(), cnt0.copy()
+    st_c, _, d_c, done_c = o.mc_run_ex(c_occ, c_cnt, 400, K, seed, select_best=True, depth_limit=25)
+    d_occ, d_cnt = occ0.copy(), cnt0.copy()
+    st_d, _, d_d, done_1 = o.mc_run_ex(d_occ, d_cnt, 150, K, seed, select_best=True, depth_limit=25)
+    st_d, _, d_d, done_2 = o.mc_run_ex(d_occ, d_cnt, 250, K, seed, step0=150, stats=st_d, select_best=True, depth_limit=25, depth=d_d)
+    np.testing.assert_array_equal(c_occ, d_occ)
+    assert (st_c["hash"] == st_d["hash"]).all() and (st_c["J"] == st_d["J"]).all()
+    # a chain that stopped in the first part does nothing in the second; the others add up
+    assert ((done_1 + done_2 == done_c) | (done_1 < 150)).all() and (d_c == d_d).all()
+    # best-of-K never does worse in one step than lowest-index from the same state
+    e_occ, e_cnt = occ0.copy(), cnt0.copy()
+    st_e, _, _, _ = o.mc_run_ex(e_occ, e_cnt, 1, K, seed, select_best=True)
+    f_occ, f_cnt = occ0.copy(), cnt0.copy()
+    st_f, _ = o.mc_run(f_occ, f_cnt, 1, K, seed, eval_all=False)
+    assert (st_e["J"] <= st_f["J"]).all()
