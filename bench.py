@@ -47,6 +47,12 @@ def load_peaks():
     return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
 
 
+# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed `ncu --set full` captures:
+# profiles/r1_mc_halo_c4_full.md (whole c4 trajectory, one launch) and profiles/r1_sro_count_v3.md (fcc 100^3, batch 1).
+NCU_TRAFFIC_MC_C4_FULL = 4_412_160 + 26_112
+NCU_TRAFFIC_RECOUNT_L100 = 680_663_040
+
+
 # ALU-issue model of one swap trial: thread-instructions the method needs per candidate.
 def mc_ops_per_trial(Z, S, M):
     philox = 10 * 4 + 4                 # 10 rounds x (2 wide multiplies + 2 three-input xors) + 4 bounded draws
@@ -321,7 +327,8 @@ def main():
         Zr = sum(hr.z)
         bytes_r = (4 * Zr + 1) * hr.N
         recount = {"bound": "hbm", "achieved": bytes_r / t_r / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                   "frac": bytes_r / t_r / 1e9 / hbm_peak, "traffic": None, "peak_source": peak_src,
+                   "frac": bytes_r / t_r / 1e9 / hbm_peak,
+                   "traffic": NCU_TRAFFIC_RECOUNT_L100 if args.recount_L == 100 else None, "peak_source": peak_src,
                    "kernel": "sro_count_kernel", "workload": f"fcc {args.recount_L}^3 ({hr.N} atoms), 5 species, "
                    f"3 shells (Z={Zr}), batch 1; table {4 * Zr * hr.N / 1e6:.0f} MB > L2",
                    "bytes_per_atom": 4 * Zr + 1, "atoms_per_s": hr.N / t_r, "ms_per_launch": t_r * 1e3}
@@ -358,7 +365,8 @@ def main():
                 "d2h_bytes_per_step": d2h, "api": "hea_mc_run_host (pinned host occupancies)"},
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "achieved": mc_rate_1gpu * ops / 1e12, "peak": alu_peak,
-                     "unit": "T thread-instr/s", "frac": mc_rate_1gpu * ops / 1e12 / alu_peak, "traffic": None,
+                     "unit": "T thread-instr/s", "frac": mc_rate_1gpu * ops / 1e12 / alu_peak,
+                     "traffic": NCU_TRAFFIC_MC_C4_FULL if (args.workload == 4 and not args.chains and n_mc == w.n_steps) else None,
                      "kernel": "mc_halo_kernel", "ops_per_trial": ops, "ms_per_launch": 1e3 * t_mc / args.steps,
                      "peak_source": f"{n_sms} SMs x 128 lanes/clk x {sm_max_mhz:.0f} MHz (DESIGN.md section 6)"},
     }
