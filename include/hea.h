@@ -145,6 +145,27 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
                hea_mc_stats* stats_dev, hea_move* log_dev, int64_t log_cap, void* cuda_stream);
 
 /*
+ * hea_mc_run_ex -- hea_mc_run with the paper's own selection and termination as options.
+ *   select_best != 0: per step the candidate with the smallest J_k is taken (Eq. 6: F_best = min over the
+ *                     updates; ties -> lowest k) and applied iff J_k < J_cur; 0: lowest improving k (hea_mc_run).
+ *   depth_limit > 0:  search-depth termination (Alg. 3, section 4.6.4): depth = consecutive steps
+ *                     without an applied move, reset by every applied move; a chain stops as soon as
+ *                     depth == depth_limit (a chain entering with depth >= depth_limit does nothing), else after
+ *                     n_steps steps.  0: no depth termination.
+ *   depth_dev      [C] uint64 in/out: the depth counters (carry them over for split runs); may be NULL when
+ *                  depth_limit == 0
+ *   steps_done_dev [C] uint64 out: steps executed by this call (n_steps unless the depth limit stopped the chain);
+ *                  may be NULL
+ * Everything else as hea_mc_run; hea_mc_run == hea_mc_run_ex(select_best 0, depth_limit 0, NULL, NULL).
+ * Returns HEA_EUNSUPPORTED for a non-default option when the configuration does not fit the shared-memory engine.
+ */
+int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, uint64_t n_steps, int K,
+                  uint64_t seed, uint64_t chain0, uint64_t step0,
+                  hea_mc_stats* stats_dev, hea_move* log_dev, int64_t log_cap,
+                  int select_best, uint64_t depth_limit, uint64_t* depth_dev, uint64_t* steps_done_dev,
+                  void* cuda_stream);
+
+/*
  * Host-buffer (end-to-end) forms: the same kernels, with host<->device copies done by the library on an internal
  * stream, synchronous.  Host buffers may be pageable or pinned.
  *   hea_sro_full_host: occ_host [B][N] -> counts_host (required), alpha_host / obj_host (optional).

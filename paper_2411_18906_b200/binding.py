@@ -23,7 +23,7 @@ MOVE_DTYPE = np.dtype([("step", "<u8"), ("k", "<u4"), ("a", "<u4"), ("b", "<u4")
 
 EXPORTS = ["hea_version", "hea_last_error", "hea_create", "hea_destroy", "hea_info", "hea_neighbor_table",
            "hea_set_option", "hea_get_option", "hea_init_random", "hea_sro_full", "hea_mc_stats_reset",
-           "hea_mc_run", "hea_sro_full_host", "hea_mc_run_host", "hea_launch_count"]
+           "hea_mc_run", "hea_mc_run_ex", "hea_sro_full_host", "hea_mc_run_host", "hea_launch_count"]
 
 
 class HeaError(RuntimeError):
@@ -56,6 +56,7 @@ def lib():
         L.hea_sro_full.argtypes = [vp, vp, i64, vp, vp, vp, vp]
         L.hea_mc_stats_reset.argtypes = [vp, vp, i64, vp]
         L.hea_mc_run.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp, vp, i64, vp]
+        L.hea_mc_run_ex.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp, vp, i64, i32, u64, vp, vp, vp]
         L.hea_sro_full_host.argtypes = [vp, vp, i64, vp, vp, vp]
         L.hea_mc_run_host.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp]
         L.hea_launch_count.argtypes = [vp, vp]
@@ -164,6 +165,23 @@ class Hea:
                                 seed, chain0, step0, C.c_void_p(stats.data_ptr()),
                                 C.c_void_p(log.data_ptr()) if log is not None else None, log_cap, _stream()))
         return stats, log
+
+    def mc_run_ex(self, occ, counts, n_steps, K, seed, chain0=0, step0=0, stats=None, log_cap=0, select_best=False,
+                  depth_limit=0, depth=None):
+        """hea_mc_run_ex: best-of-K selection and search-depth termination.  Returns (stats, log, depth, steps_done)."""
+        n = occ.shape[0]
+        if stats is None:
+            stats = self.new_stats(n)
+        if depth is None:
+            depth = torch.zeros((n,), dtype=torch.int64, device=self.device)
+        steps_done = torch.zeros((n,), dtype=torch.int64, device=self.device)
+        log = torch.zeros((n, max(log_cap, 1), MOVE_WORDS), dtype=torch.int64, device=self.device) if log_cap > 0 else None
+        _check(lib().hea_mc_run_ex(self._h, C.c_void_p(occ.data_ptr()), C.c_void_p(counts.data_ptr()), n, n_steps, K,
+                                   seed, chain0, step0, C.c_void_p(stats.data_ptr()),
+                                   C.c_void_p(log.data_ptr()) if log is not None else None, log_cap,
+                                   1 if select_best else 0, depth_limit, C.c_void_p(depth.data_ptr()),
+                                   C.c_void_p(steps_done.data_ptr()), _stream()))
+        return stats, log, depth, steps_done
 
     # ---- host-buffer (end-to-end) calls: numpy arrays in, synchronous
     def sro_full_host(self, occ, want_alpha=False, want_obj=True):

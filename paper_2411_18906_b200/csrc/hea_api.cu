@@ -28,7 +28,8 @@ size_t mc2_team_bytes(int64_t C);
 constexpr int kMc2MaxThreads = 512;
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
                        void* team_ctl, int team_on, int team_off, int accept_engine, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
-                       uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches);
+                       uint64_t step0, void* stats, void* log, int64_t log_cap, int select_best, uint64_t depth_limit,
+                       uint64_t* depth, uint64_t* steps_done, cudaStream_t st, int64_t* n_launches);
 }  // namespace hea
 
 struct hea_ctx {
@@ -358,6 +359,16 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
                uint64_t chain0, uint64_t step0, hea_mc_stats* stats_dev, hea_move* log_dev, int64_t log_cap,
                void* cuda_stream)
 {
+    return hea_mc_run_ex(ctx, occ_dev, counts_dev, C, n_steps, K, seed, chain0, step0, stats_dev, log_dev, log_cap, 0, 0,
+                         nullptr, nullptr, cuda_stream);
+}
+
+int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, uint64_t n_steps, int K, uint64_t seed,
+                  uint64_t chain0, uint64_t step0, hea_mc_stats* stats_dev, hea_move* log_dev, int64_t log_cap,
+                  int select_best, uint64_t depth_limit, uint64_t* depth_dev, uint64_t* steps_done_dev, void* cuda_stream)
+{
+    if (depth_limit > 0 && C != 0 && !depth_dev) return fail(HEA_EINVAL, "depth_limit > 0 needs depth_dev");
+    const bool ex_mode = select_best != 0 || depth_limit > 0 || steps_done_dev != nullptr;
     static_assert(sizeof(hea_mc_stats) == 40, "hea_mc_stats layout");
     static_assert(sizeof(hea_move) == 24, "hea_move layout");
     if (!ctx) return fail(HEA_EINVAL, "ctx is NULL");
@@ -383,6 +394,8 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
                               (occ_mode == 2 && ctx->M <= 4 && hea::mc2_shared_bytes(2, ctx->lat.type, ctx->P.L) <= budget);
         engine = (fits && fits_req && ctx->opt_cluster == 0 && ctx->opt_neighbors == 0) ? 2 : 1;
     }
+    if (ex_mode && engine != 2)
+        return fail(HEA_EUNSUPPORTED, "hea_mc_run_ex options need the shared-memory (halo) engine: configuration too large or engine forced");
     if (engine == 2) {
         // halo engine (hea_mc2.cu): one block per chain, padded one-hot configuration in shared memory
         int om = occ_mode;
@@ -409,8 +422,9 @@ int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, u
         const int w_max2 = ctx->opt_window ? (int)ctx->opt_window : (1 << 20);
         cudaError_t e2 = hea::launch_mc2(ctx->P, ctx->tab_host, ctx->lat.type, om, threads, team, team_ctl,
                                          (int)ctx->opt_team_on, (int)ctx->opt_team_off, ctx->opt_accept == 1 ? 0 : 1, w_max2, occ_dev, counts_dev, C,
-                                         n_steps, K, seed, chain0, step0, stats_dev, log_dev, log_cap,
-                                         (cudaStream_t)cuda_stream, &ctx->n_launches);
+                                         n_steps, K, seed, chain0, step0, stats_dev, log_dev, log_cap, select_best,
+                                         depth_limit, depth_dev, steps_done_dev, (cudaStream_t)cuda_stream,
+                                         &ctx->n_launches);
         return e2 == cudaSuccess ? HEA_OK : fail_cuda(e2, "hea_mc_run launch (halo engine)");
     }
     const int AZ = ctx->P.A * ctx->P.Z;

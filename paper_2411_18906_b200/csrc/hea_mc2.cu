@@ -53,6 +53,7 @@ struct Sh2 {
     uint32_t best[3];
     uint32_t team_key;            // minimum key over the team (TEAM windows)
     unsigned long long bc_t0;     // follower: broadcast of the leader's phase record
+    unsigned long long bc_depth;
     double bc_J;
     uint32_t bc_W, pad;
     MoveRec rec;
@@ -64,7 +65,8 @@ struct Sh2 {
     float fb2[64];                // first-shell cell (i, j): 2 (N_ij - n*_ij), n* = the count at which alpha = target
     float fwg[64];                //                          w_1 g_ij^2
     uint32_t q_n[3];              // queue fill, triple-buffered like best[]
-    uint32_t q_pad;
+    uint32_t bestk;               // best-of-K: lowest key among the minimum-J candidates of the deciding step
+    unsigned long long bestJ;     // best-of-K: minimum J (as ordered bits) among the candidates of the deciding step
     uint32_t queue[kQueueCap];    // keys of the candidates that passed the pre-filter
 };
 
@@ -215,7 +217,8 @@ struct TeamCtl {
     uint32_t W;                   // window length (steps) to continue with
     unsigned long long t0;        // next step
     double J;
-    uint32_t pad[10];
+    unsigned long long depth;     // search-depth counter (hea_mc_run_ex)
+    uint32_t pad[8];
     TeamSlot slot[2][kMaxTeam];   // [team-window parity][rank]
 };
 
@@ -237,6 +240,11 @@ struct Mc2Args {
     TeamCtl* team;                // [C] control blocks, zeroed before the launch (R > 1 only)
     int team_on, team_off;        // enter TEAM when W*K >= team_on; leave it after a move with steps_done*K < team_off
     int accept_engine;            // 1: single-step windows run on the 8-lanes-per-candidate engine
+    // hea_mc_run_ex
+    int select_best;              // 1: the minimum J_k of a step is taken (ties -> lowest k) instead of the lowest improving k
+    unsigned long long depth_limit;        // > 0: a chain stops after this many consecutive steps without a move
+    unsigned long long* depth_all;         // [C] in/out, or nullptr
+    unsigned long long* steps_done_all;    // [C] out, or nullptr
 };
 
 // Shared memory: occupancy (offset 0, so a gather address is the loaded offset itself) | Sh2 | offset table [A][ZP].
@@ -345,6 +353,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         sh.n_accept = g_stats[0]; sh.n_null = 0; sh.hash = g_stats[2]; sh.last_accept = g_stats[3]; sh.n_logged = 0;
         sh.best[0] = sh.best[1] = sh.best[2] = kNoKey;
         sh.q_n[0] = sh.q_n[1] = sh.q_n[2] = 0u;
+        sh.bestk = kNoKey; sh.bestJ = ~0ull;
         sh.rec.key = kNoKey;
     }
     __syncthreads();
@@ -373,7 +382,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         if (w_cap > (uint32_t)A.w_max) w_cap = (uint32_t)A.w_max;
     };
     set_mode(false);
-    const bool accept_ok = T >= 512 && AA.accept_engine != 0;   // 8 evaluating warps + null-settling warps
+    const bool best_mode = AA.select_best != 0;
+    const unsigned long long depth_limit = AA.depth_limit;
+    unsigned long long depth = (depth_limit && AA.depth_all) ? AA.depth_all[chain_local] : 0ull;
+    const bool accept_ok = T >= 512 && AA.accept_engine != 0 && !best_mode;   // 8 evaluating warps + null-settling warps
 
     // D9.4: apply an accepted move in every thread of the block (counts by the first S*M*M threads, the swap with its
     // ghost images by thread T-1, bookkeeping by thread T-2); ends with a barrier.
@@ -409,6 +421,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         if (tid == T - 2) {
             const uint32_t a = mv->a, b = mv->b;
             sh.J = mv->J;
+            sh.bestk = kNoKey; sh.bestJ = ~0ull;
             sh.n_accept += 1;
             sh.last_accept = step;
             unsigned long long h = sh.hash;
@@ -609,19 +622,21 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     uint32_t phase = 0;                                      // phase records consumed / posted
     double slack_J = -1.0;                                   // J the pre-filter intervals were computed for (J >= 0 always)
 
-    while (t0 < t_end) {
+    while (t0 < t_end && !(depth_limit && depth >= depth_limit)) {
         if (R > 1 && !team && rank != 0) {
             // ---- follower in a SOLO phase: wait for the leader's phase record, reload, join the team
             if (tid == 0) {
                 while (ld_acquire_u32(&ctl->phase_seq) != phase + 1u) __nanosleep(256);
                 sh.bc_W = __ldcg(&ctl->W);                   // broadcast through shared memory
                 sh.bc_t0 = __ldcg(&ctl->t0);
+                sh.bc_depth = __ldcg(&ctl->depth);
                 sh.J = __ldcg(&ctl->J);
             }
             __syncthreads();
             ++phase;
             W = sh.bc_W;
             t0 = sh.bc_t0;
+            depth = sh.bc_depth;
             if (t0 >= t_end) break;
             load_state();
             set_mode(true);
@@ -663,11 +678,13 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             if (key_best != kNoKey) {
                 apply_move(&sh.cand[key_best - rd0], key_best, t0);
                 W = 1u;
+                depth = 0;
             } else {
                 W = min(2u, w_cap);
+                depth += 1;
             }
         } else {
-            const uint32_t Wc = (uint32_t)min((unsigned long long)W, t_end - t0);
+            const uint32_t Wc = (uint32_t)min(min((unsigned long long)W, t_end - t0), depth_limit ? depth_limit - depth : ~0ull);
             const int buf = (int)(it % 3u);
             volatile uint32_t* best_slot = &sh.best[buf];
             const double J_cur = sh.J;
@@ -730,10 +747,14 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 } else if (S > 1) {
                     Jk = J_cur;
                 }
-                if (Jk < J_cur && key < win_key) {
+                // this thread keeps its best candidate: the lowest key, or in best-of-K mode the lowest (step, J, k)
+                const uint32_t kts = key >> 10, wts = win_key >> 10;
+                const bool better = best_mode ? (kts < wts || (kts == wts && (Jk < win_J || (Jk == win_J && key < win_key))))
+                                              : key < win_key;
+                if (Jk < J_cur && better) {
                     win_key = key; win_a = a; win_b = b; win_pq = (uint32_t)p | ((uint32_t)q << 8);
                     win_d0 = pack_F<M>(F0); win_d1 = pack_F<M>(F1); win_d2 = pack_F<M>(F2); win_J = Jk;
-                    atomicMin(&sh.best[buf], key);
+                    atomicMin(&sh.best[buf], best_mode ? (key & ~1023u) : key);
                 }
             };
             // first-shell species-count differences of a non-null candidate
@@ -756,7 +777,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 propose(t0 + ts, k, a, b, sa, sb, hp, hq);
                 if (hp == hq) {
                     nullmask |= 1ull << j;
-                } else if (key < hint) {                             // same step, higher k than a known move: only nullness counts
+                } else if (best_mode || key < hint) {               // same step, higher k than a known move: only nullness counts
                     const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
                     int c[M], F0[M];
 #pragma unroll
@@ -802,7 +823,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 for (uint32_t i = (uint32_t)tid; i < nq; i += (uint32_t)T) {
                     const uint32_t key = sh.queue[i];
                     const uint32_t hint = *best_slot;
-                    if (!(key < hint)) continue;
+                    if (best_mode ? (hint >> 10) < (key >> 10) : !(key < hint)) continue;
                     uint32_t a, b, hp, hq;
                     SiteC sa, sb;
                     propose(t0 + (key >> 10), key & 1023u, a, b, sa, sb, hp, hq);
@@ -819,6 +840,16 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             __syncthreads();                                        // B1: window evaluated, local minimum posted
             key_best = sh.best[buf];
             if (tid == 0) { sh.best[(buf + 2) % 3] = kNoKey; sh.q_n[(buf + 2) % 3] = 0u; }   // next user of these slots is two barriers away
+            if (best_mode && key_best != kNoKey) {
+                // best-of-K: among this block's improving candidates of the deciding step, the minimum J, then the
+                // lowest k (bestJ / bestk are reset by apply_move, which always follows)
+                const bool mine = win_key != kNoKey && (win_key >> 10) == (key_best >> 10);
+                if (mine) atomicMin(&sh.bestJ, (unsigned long long)__double_as_longlong(win_J));
+                __syncthreads();
+                if (mine && (unsigned long long)__double_as_longlong(win_J) == sh.bestJ) atomicMin(&sh.bestk, win_key);
+                __syncthreads();
+                key_best = sh.bestk;
+            }
 
             const int lane = tid & 31;
             if (team) {
@@ -835,11 +866,21 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 }
                 if (tid < 32) {
                     uint32_t kk = kNoKey;
+                    unsigned long long jb = 0ull;
                     if (lane < R) {
                         while (ld_acquire_u32(&slots[lane].seq) != tw + 1u) { }
                         kk = __ldcg(&slots[lane].key);
+                        if (best_mode) jb = (unsigned long long)__double_as_longlong(__ldcg(&slots[lane].J));
                     }
-                    uint32_t kmin = kk;
+                    // minimum over the team: by key, or in best-of-K mode by (step, J, k)
+                    const uint32_t ka = best_mode ? (kk == kNoKey ? kNoKey : kk >> 10) : kk;
+                    uint32_t amin = ka;
+    #pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) amin = min(amin, __shfl_xor_sync(0xFFFFFFFFu, amin, o));
+                    unsigned long long jmin = ka == amin ? jb : ~0ull;
+    #pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) jmin = min(jmin, __shfl_xor_sync(0xFFFFFFFFu, jmin, o));
+                    uint32_t kmin = (ka == amin && jb == jmin) ? kk : kNoKey;
     #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) kmin = min(kmin, __shfl_xor_sync(0xFFFFFFFFu, kmin, o));
                     if (kmin != kNoKey && kk == kmin) {           // keys are unique: exactly one lane
@@ -875,8 +916,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             if (key_best != kNoKey) {
                 apply_move(mv, key_best & 1023u, t0 + (key_best >> 10));
                 W = min(steps_done, w_cap);                         // the observed gap
+                depth = 0;
             } else {
                 W = min(W * 2u, w_cap);
+                depth += steps_done;
             }
             ++it;
         }
@@ -895,7 +938,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 store_state();
                 __syncthreads();
                 if (tid == 0) {
-                    ctl->W = W; ctl->t0 = t0; ctl->J = sh.J;
+                    ctl->W = W; ctl->t0 = t0; ctl->J = sh.J; ctl->depth = depth;
                     __threadfence();
                     st_release_u32(&ctl->phase_seq, phase + 1u);
                 }
@@ -909,7 +952,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     if (R > 1 && rank == 0 && !team) {
         __syncthreads();
         if (tid == 0) {
-            ctl->W = 1; ctl->t0 = t_end; ctl->J = sh.J;
+            ctl->W = 1; ctl->t0 = t_end; ctl->J = sh.J; ctl->depth = depth;
             __threadfence();
             st_release_u32(&ctl->phase_seq, phase + 1u);
         }
@@ -923,6 +966,8 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             g_stats[2] = sh.hash;
             g_stats[3] = sh.last_accept;
             g_stats[4] = (unsigned long long)__double_as_longlong(sh.J);
+            if (AA.depth_all) AA.depth_all[chain_local] = depth;
+            if (AA.steps_done_all) AA.steps_done_all[chain_local] = t0 - A.step0;
         }
     }
     if (tid == 0 && sh.n_null) atomicAdd(&g_stats[1], sh.n_null);
@@ -994,7 +1039,8 @@ size_t mc2_team_bytes(int64_t C) { return sizeof(TeamCtl) * (size_t)C; }
 
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
                        void* team_ctl, int team_on, int team_off, int accept_engine, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
-                       uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches)
+                       uint64_t step0, void* stats, void* log, int64_t log_cap, int select_best, uint64_t depth_limit,
+                       uint64_t* depth, uint64_t* steps_done, cudaStream_t st, int64_t* n_launches)
 {
     Mc2Args AA;
     McArgs& A = AA.a;
@@ -1007,6 +1053,10 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
     AA.team_on = team_on > 0 ? team_on : 4 * threads;
     AA.team_off = team_off > 0 ? team_off : threads;
     AA.accept_engine = accept_engine;
+    AA.select_best = select_best ? 1 : 0;
+    AA.depth_limit = depth_limit;
+    AA.depth_all = reinterpret_cast<unsigned long long*>(depth);
+    AA.steps_done_all = reinterpret_cast<unsigned long long*>(steps_done);
     if (team > 1) {
         if (team > kMaxTeam || !team_ctl) return cudaErrorInvalidValue;
         cudaError_t em = cudaMemsetAsync(team_ctl, 0, mc2_team_bytes(C), st);

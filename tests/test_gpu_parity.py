@@ -369,3 +369,76 @@ def test_host_buffer_entry_points(hb):
     np.testing.assert_array_equal(g_occ, occ)
     np.testing.assert_array_equal(g_counts, o_cnt)
     assert_stats_equal(g_stats, o_stats)
+
+
+# ---- hea_mc_run_ex (best-of-K selection, search-depth termination) against ora_mc_run_ex
+def run_both_ex(hb, w, n_chains, n_steps, select_best, depth_limit, opts=None, log_cap=64, split=None):
+    h, o = pair(hb, w)
+    for k, v in (opts or {}).items():
+        h.set_option(k, v)
+    occ = h.init_random(n_chains, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    o_occ, o_cnt = occ.cpu().numpy().copy(), counts.cpu().numpy().copy()
+    o_stats, o_log, o_depth, o_done = o.mc_run_ex(o_occ, o_cnt, n_steps, w.K, w.seed, log_cap=log_cap,
+                                                  select_best=select_best, depth_limit=depth_limit)
+    if split is None:
+        stats, log, depth, done = h.mc_run_ex(occ, counts, n_steps, w.K, w.seed, log_cap=log_cap,
+                                              select_best=select_best, depth_limit=depth_limit)
+        done = done.cpu().numpy().astype(np.uint64)
+    else:                                                       # two calls, depth and stats carried over
+        stats, log, depth, d1 = h.mc_run_ex(occ, counts, split, w.K, w.seed, log_cap=log_cap,
+                                            select_best=select_best, depth_limit=depth_limit)
+        stats, _, depth, d2 = h.mc_run_ex(occ, counts, n_steps - split, w.K, w.seed, step0=split, stats=stats,
+                                          select_best=select_best, depth_limit=depth_limit, depth=depth)
+        d1, d2 = d1.cpu().numpy().astype(np.uint64), d2.cpu().numpy().astype(np.uint64)
+        # a chain stopped by the depth limit in the first call does nothing in the second
+        assert ((d1 == split) | (d2 == 0)).all()
+        done = d1 + d2
+    np.testing.assert_array_equal(occ.cpu().numpy(), o_occ)
+    np.testing.assert_array_equal(counts.cpu().numpy(), o_cnt)
+    assert_stats_equal(hb.stats_to_numpy(stats), o_stats)
+    np.testing.assert_array_equal(depth.cpu().numpy().astype(np.uint64), o_depth)
+    np.testing.assert_array_equal(done, o_done)
+    if split is None and log_cap:
+        got = hb.log_to_numpy(log)
+        for c in range(n_chains):
+            n = min(int(o_stats["n_accept"][c]), log_cap)
+            for f in ("step", "k", "a", "b"):
+                np.testing.assert_array_equal(got[c][:n][f], o_log[c][:n][f])
+    return o_stats, o_done
+
+
+@pytest.mark.parametrize("select_best", [False, True])
+@pytest.mark.parametrize("depth_limit", [0, 7, 150])
+@pytest.mark.parametrize("team,threads", [(1, 64), (1, 512), (3, 128), (9, 512)])
+def test_mc_run_ex_selection_and_depth(hb, select_best, depth_limit, team, threads):
+    w = small("fcc", (4, 4, 4), [0.2, 0.2, 0.2, 0.4], 3, target_seed=5, K=24, n_steps=1500)
+    st, done = run_both_ex(hb, w, 5, 1500, select_best, depth_limit,
+                           opts={"mc_team": team, "mc_threads": threads, "mc_team_on": 256, "mc_team_off": 64})
+    assert st["n_accept"].sum() > 50
+    if depth_limit == 7:
+        assert (done < 1500).all()                          # the depth limit stopped every chain early
+
+
+@pytest.mark.parametrize("select_best", [False, True])
+def test_mc_run_ex_split_run_carries_depth(hb, select_best):
+    w = small("bcc", (5, 5, 5), [0.25] * 4, 3, K=32, n_steps=3000)
+    run_both_ex(hb, w, 6, 3000, select_best, 400, split=1100, log_cap=0)
+
+
+@pytest.mark.parametrize("lattice,dims,conc,S", LATTICES[:9])
+def test_mc_run_ex_best_of_K_lattices(hb, lattice, dims, conc, S):
+    w = small(lattice, dims, conc, S, target_seed=11, K=16)
+    run_both_ex(hb, w, 3, 120, True, 0)
+
+
+def test_mc_run_ex_c4_best_of_K_prefix_and_errors(hb):
+    w = wl.config(4)
+    st, _ = run_both_ex(hb, w, 4, 400, True, 0, log_cap=400)
+    assert (st["n_accept"] > 300).all()
+    h, _ = pair(hb, small("fcc", (3, 3, 3), [0.5, 0.5], 2))
+    occ = h.init_random(2, seed=1)
+    cnt, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    h.set_option("mc_engine", 1)
+    with pytest.raises(hb.HeaError):                        # the window engine has no ex options
+        h.mc_run_ex(occ, cnt, 10, 8, 1, select_best=True)
