@@ -410,6 +410,8 @@ int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C
         int threads = ctx->opt_threads ? (int)ctx->opt_threads : hea::kMc2MaxThreads;
         if (!ctx->opt_threads && team == 1) {
             const int64_t blocks_per_sm = (C + ctx->n_sms - 1) / ctx->n_sms;
+            // 128 registers per thread: 512 threads are resident per SM; measured on c2 (7 blocks per SM) and c3 (2 per
+            // SM), blocks of 1024 / blocks_per_sm threads running in waves beat smaller blocks that are all resident
             if (blocks_per_sm > 1) threads = std::max(32, std::min(512, floor_pow2(std::max<int64_t>(1, 1024 / blocks_per_sm))));
         }
         threads = std::min(threads, hea::kMc2MaxThreads);   // the halo kernel is compiled for blocks of at most this size

@@ -377,7 +377,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         gtid = tm ? (uint32_t)tid * (uint32_t)R + rank : (uint32_t)tid;
         ts_first = gtid / (uint32_t)K; k_first = gtid - ts_first * (uint32_t)K;
         ts_inc = GT / (uint32_t)K; k_inc = GT - ts_inc * (uint32_t)K;
-        w_cap = (uint32_t)min((uint64_t)(1u << 20), ((uint64_t)(tm ? kTeamRounds : kMaxRounds) * GT) / (uint32_t)K);
+        w_cap = (uint32_t)min((uint64_t)(1u << 20), ((uint64_t)kTeamRounds * GT) / (uint32_t)K);
         if (w_cap < 1u) w_cap = 1u;
         if (w_cap > (uint32_t)A.w_max) w_cap = (uint32_t)A.w_max;
     };
