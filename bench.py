@@ -169,6 +169,68 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+
+# ------------------------------------------------------------------------------------------ configs[4]: throughput sweeps
+def run_sweep(args):
+    """BASELINE.json:configs[4]: full-SRO recount on fcc L^3 (L = 10..100) x batch 1..1024, and the MC chain-count sweep
+    1..65,536 chains on the 2,000-atom bcc cell (steady state after a warm-up run).  Prints one JSON object; not the
+    driver's bench line."""
+    import torch
+    from paper_2411_18906_b200 import binding, workloads
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    hbm_peak, _, _ = load_peaks()
+    out = {"sweep": "configs[4]", "recount": [], "mc_chains": []}
+    for L in workloads.RECOUNT_SWEEP_L:
+        wr = workloads.recount_sweep_workload(L, 1)
+        hr = binding.Hea(*wr.create_args(), device=0)
+        Z = sum(hr.z)
+        for B in workloads.RECOUNT_SWEEP_B:
+            if B * hr.N > (6 << 30):
+                continue
+            occ = hr.init_random(B, wr.seed)
+            cnt = torch.empty((B, hr.S, hr.M, hr.M), dtype=torch.int32, device=dev)
+            for _ in range(2):
+                hr.sro_full(occ, counts=cnt, want_alpha=False, want_obj=False)
+            reps = max(3, min(50, int(2e9 // (B * hr.N)) or 3))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps):
+                hr.sro_full(occ, counts=cnt, want_alpha=False, want_obj=False)
+            e1.record()
+            torch.cuda.synchronize()
+            t = e0.elapsed_time(e1) * 1e-3 / reps
+            table_bytes, occ_bytes = 4 * Z * hr.N, B * hr.N
+            out["recount"].append({"L": L, "atoms": hr.N, "batch": B, "us": 1e6 * t, "atoms_per_s": B * hr.N / t,
+                                   "model_GBps_table_once": (table_bytes + occ_bytes) / t / 1e9,
+                                   "frac_hbm_table_once": (table_bytes + occ_bytes) / t / 1e9 / hbm_peak,
+                                   "table_MB": table_bytes / 1e6})
+            del occ, cnt
+        hr.close()
+    for C in workloads.CHAIN_SWEEP_C:
+        wm = workloads.chain_sweep_workload(C)
+        hm = binding.Hea(*wm.create_args(), device=0)
+        occ = hm.init_random(C, wm.seed)
+        cnt, _, _ = hm.sro_full(occ, want_alpha=False, want_obj=False)
+        st = hm.new_stats(C)
+        n_warm, n_time = 20_000, 20_000
+        hm.mc_run(occ, cnt, n_warm, wm.K, wm.seed, stats=st)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a0 = int(binding.stats_to_numpy(st)["n_accept"].sum())
+        e0.record()
+        hm.mc_run(occ, cnt, n_time, wm.K, wm.seed, step0=n_warm, stats=st)
+        e1.record()
+        torch.cuda.synchronize()
+        t = e0.elapsed_time(e1) * 1e-3
+        a1 = int(binding.stats_to_numpy(st)["n_accept"].sum())
+        out["mc_chains"].append({"chains": C, "mc_steps": n_time, "K": wm.K, "ms": 1e3 * t,
+                                 "trials_per_s": C * n_time * wm.K / t, "us_per_step": 1e6 * t / n_time,
+                                 "accept_rate": (a1 - a0) / (C * n_time)})
+        hm.close()
+    print(json.dumps(out))
+
 # ------------------------------------------------------------------------------------------ GPU arm
 def main():
     ap = argparse.ArgumentParser()
@@ -184,11 +246,14 @@ def main():
     ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config 1..4 (default 4 = the metric's)")
     ap.add_argument("--chains", type=int, default=0, help="override the chain count (exploration only)")
     ap.add_argument("--opt", action="append", default=[], help="tuning option name=value (hea_set_option)")
+    ap.add_argument("--sweep", action="store_true", help="run the configs[4] throughput sweeps instead of the bench step")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3                                   # timing rule: W >= 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
 
     import torch
     import torch.distributed as dist
