@@ -166,6 +166,20 @@ int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C
                   void* cuda_stream);
 
 /*
+ * hea_pool_select -- the selection step of the global search (Alg. 1; retained top solutions seed the
+ * next iteration, the others are generated entirely randomly) over a pool of C chains.
+ * The chains are ranked by J of counts_dev (D6), ascending, ties -> lower index.  The n_keep best move to positions
+ * 0..n_keep-1 in rank order with their counts and stats; every position r >= n_keep receives a fresh seeded random
+ * configuration (hea_init_random, chain id new_chain0 + r - n_keep), its recount, and reset stats.  The paper gives no
+ * value for the retained fraction ("at most half") or the discarded fraction p_a: n_keep is the caller's.
+ *   occ_dev [C][N], counts_dev [C][S][M][M], stats_dev [C]: in/out; counts_dev must be the recount of occ_dev
+ *   order_dev [n_keep] int32 out (optional, may be NULL): previous index of the chain now at each kept position
+ * A chain at position r continues with RNG chain id chain0 + r of the next hea_mc_run.  C <= 65,536.
+ */
+int hea_pool_select(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, hea_mc_stats* stats_dev, int64_t C,
+                    int64_t n_keep, uint64_t seed, uint64_t new_chain0, int32_t* order_dev, void* cuda_stream);
+
+/*
  * Host-buffer (end-to-end) forms: the same kernels, with host<->device copies done by the library on an internal
  * stream, synchronous.  Host buffers may be pageable or pinned.
  *   hea_sro_full_host: occ_host [B][N] -> counts_host (required), alpha_host / obj_host (optional).

@@ -169,6 +169,24 @@ class Oracle:
         self.threads_used = used
         return stats, log
 
+    def pool_select(self, occ, counts, stats, n_keep, seed, new_chain0):
+        """SURVEY 8f-2, the selection step of the global search (Alg. 1; the retained top
+        solutions seed the next iteration, the others are generated entirely randomly).  Reading (A24):
+        the pool is ranked by J of the supplied counts, ascending, ties -> lower index; the n_keep best move to the front
+        in rank order with their counts and stats; every other slot r >= n_keep gets a fresh seeded random configuration
+        (D8, chain id new_chain0 + r - n_keep), its recount, and reset stats.  In place; returns `order`, the previous
+        index of the chain now at each kept position.  Plain numpy over the pinned pieces (objective, init, recount)."""
+        n = occ.shape[0]
+        J = np.array([self.objective(counts[c]) for c in range(n)])
+        order = sorted(range(n), key=lambda c: (J[c], c))[:n_keep]
+        occ[:n_keep], counts[:n_keep], stats[:n_keep] = occ[order].copy(), counts[order].copy(), stats[order].copy()
+        if n > n_keep:
+            occ[n_keep:] = self.init_random(n - n_keep, seed, new_chain0)
+            for c in range(n_keep, n):
+                counts[c] = self.pair_counts(occ[c])
+            stats[n_keep:] = fresh_stats(n - n_keep)
+        return np.asarray(order, dtype=np.int32)
+
     def mc_run_ex(self, occ, counts, n_steps, K, seed, chain0=0, step0=0, stats=None, log_cap=0, select_best=False,
                   depth_limit=0, depth=None):
         """SURVEY 8f-1 options: best-of-K selection, search-depth termination.  Returns (stats, log, depth, steps_done)."""

@@ -23,7 +23,7 @@ MOVE_DTYPE = np.dtype([("step", "<u8"), ("k", "<u4"), ("a", "<u4"), ("b", "<u4")
 
 EXPORTS = ["hea_version", "hea_last_error", "hea_create", "hea_destroy", "hea_info", "hea_neighbor_table",
            "hea_set_option", "hea_get_option", "hea_init_random", "hea_sro_full", "hea_mc_stats_reset",
-           "hea_mc_run", "hea_mc_run_ex", "hea_sro_full_host", "hea_mc_run_host", "hea_launch_count"]
+           "hea_mc_run", "hea_mc_run_ex", "hea_pool_select", "hea_sro_full_host", "hea_mc_run_host", "hea_launch_count"]
 
 
 class HeaError(RuntimeError):
@@ -57,6 +57,7 @@ def lib():
         L.hea_mc_stats_reset.argtypes = [vp, vp, i64, vp]
         L.hea_mc_run.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp, vp, i64, vp]
         L.hea_mc_run_ex.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp, vp, i64, i32, u64, vp, vp, vp]
+        L.hea_pool_select.argtypes = [vp, vp, vp, vp, i64, i64, u64, u64, vp, vp]
         L.hea_sro_full_host.argtypes = [vp, vp, i64, vp, vp, vp]
         L.hea_mc_run_host.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp]
         L.hea_launch_count.argtypes = [vp, vp]
@@ -182,6 +183,15 @@ class Hea:
                                    1 if select_best else 0, depth_limit, C.c_void_p(depth.data_ptr()),
                                    C.c_void_p(steps_done.data_ptr()), _stream()))
         return stats, log, depth, steps_done
+
+    def pool_select(self, occ, counts, stats, n_keep, seed, new_chain0):
+        """hea_pool_select, in place; returns order [n_keep] int32 (previous index of each kept chain)."""
+        n = occ.shape[0]
+        order = torch.empty((max(n_keep, 1),), dtype=torch.int32, device=self.device)
+        _check(lib().hea_pool_select(self._h, C.c_void_p(occ.data_ptr()), C.c_void_p(counts.data_ptr()),
+                                     C.c_void_p(stats.data_ptr()), n, n_keep, seed, new_chain0,
+                                     C.c_void_p(order.data_ptr()), _stream()))
+        return order[:n_keep]
 
     # ---- host-buffer (end-to-end) calls: numpy arrays in, synchronous
     def sro_full_host(self, occ, want_alpha=False, want_obj=True):

@@ -24,6 +24,9 @@ cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode,
                       uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches,
                       int* query_max_clusters);
 size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L);
+cudaError_t launch_pool_rank(const double* J, int64_t C, int64_t n_keep, int32_t* order, cudaStream_t st, int64_t* n_launches);
+cudaError_t launch_pool_gather(const void* src, void* dst, const int32_t* order, int64_t n_keep, size_t item,
+                               cudaStream_t st, int64_t* n_launches);
 size_t mc2_team_bytes(int64_t C);
 constexpr int kMc2MaxThreads = 512;
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
@@ -466,6 +469,47 @@ int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C
                                    counts_dev, C, n_steps, K, seed, chain0, step0, stats_dev, log_dev, log_cap, st,
                                    &ctx->n_launches, nullptr);
     return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_mc_run launch");
+}
+
+int hea_pool_select(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, hea_mc_stats* stats_dev, int64_t C, int64_t n_keep,
+                    uint64_t seed, uint64_t new_chain0, int32_t* order_dev, void* cuda_stream)
+{
+    if (!ctx) return fail(HEA_EINVAL, "ctx is NULL");
+    if (C < 0 || n_keep < 0 || n_keep > C) return fail(HEA_EINVAL, "need 0 <= n_keep <= C");
+    if (C > 65536) return fail(HEA_EUNSUPPORTED, "hea_pool_select ranks at most 65,536 chains");
+    if (new_chain0 + (uint64_t)(C - n_keep) > (1ull << 32)) return fail(HEA_EINVAL, "chain ids must be < 2^32");
+    if (C == 0) return HEA_OK;
+    if (!occ_dev || !counts_dev || !stats_dev) return fail(HEA_EINVAL, "occ_dev / counts_dev / stats_dev is NULL");
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t N = (size_t)ctx->P.N, SMM = (size_t)ctx->S * ctx->M * ctx->M;
+    int rc;
+    if ((rc = ensure_scratch(ctx, 0, N * (size_t)std::max<int64_t>(n_keep, 1))) != HEA_OK) return rc;
+    if ((rc = ensure_scratch(ctx, 1, sizeof(int32_t) * SMM * (size_t)std::max<int64_t>(n_keep, 1))) != HEA_OK) return rc;
+    if ((rc = ensure_scratch(ctx, 2, sizeof(double) * (size_t)C)) != HEA_OK) return rc;
+    if ((rc = ensure_scratch(ctx, 3, sizeof(int32_t) * (size_t)C)) != HEA_OK) return rc;
+    if ((rc = ensure_scratch(ctx, 4, sizeof(hea_mc_stats) * (size_t)std::max<int64_t>(n_keep, 1))) != HEA_OK) return rc;
+    double* J = (double*)ctx->scratch[2];
+    int32_t* order = (int32_t*)ctx->scratch[3];
+    cudaError_t e = hea::launch_sro_epilogue(ctx->P, counts_dev, C, nullptr, J, st, &ctx->n_launches);
+    if (e == cudaSuccess) e = hea::launch_pool_rank(J, C, n_keep, order, st, &ctx->n_launches);
+    if (e == cudaSuccess) e = hea::launch_pool_gather(occ_dev, ctx->scratch[0], order, n_keep, N, st, &ctx->n_launches);
+    if (e == cudaSuccess) e = hea::launch_pool_gather(counts_dev, ctx->scratch[1], order, n_keep, sizeof(int32_t) * SMM, st, &ctx->n_launches);
+    if (e == cudaSuccess) e = hea::launch_pool_gather(stats_dev, ctx->scratch[4], order, n_keep, sizeof(hea_mc_stats), st, &ctx->n_launches);
+    if (e == cudaSuccess && n_keep > 0) {
+        e = cudaMemcpyAsync(occ_dev, ctx->scratch[0], N * (size_t)n_keep, cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(counts_dev, ctx->scratch[1], sizeof(int32_t) * SMM * (size_t)n_keep, cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(stats_dev, ctx->scratch[4], sizeof(hea_mc_stats) * (size_t)n_keep, cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess && order_dev) e = cudaMemcpyAsync(order_dev, order, sizeof(int32_t) * (size_t)n_keep, cudaMemcpyDeviceToDevice, st);
+    }
+    if (e != cudaSuccess) return fail_cuda(e, "hea_pool_select");
+    const int64_t n_new = C - n_keep;
+    if (n_new > 0) {
+        if ((rc = hea_init_random(ctx, occ_dev + N * (size_t)n_keep, n_new, seed, new_chain0, cuda_stream)) != HEA_OK) return rc;
+        if ((rc = hea_sro_full(ctx, occ_dev + N * (size_t)n_keep, n_new, counts_dev + SMM * (size_t)n_keep, nullptr, nullptr, cuda_stream)) != HEA_OK) return rc;
+        if ((rc = hea_mc_stats_reset(ctx, stats_dev + n_keep, n_new, cuda_stream)) != HEA_OK) return rc;
+    }
+    return HEA_OK;
 }
 
 int hea_sro_full_host(hea_ctx* ctx, const uint8_t* occ_host, int64_t B, int32_t* counts_host, double* alpha_host,

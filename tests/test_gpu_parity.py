@@ -442,3 +442,28 @@ def test_mc_run_ex_c4_best_of_K_prefix_and_errors(hb):
     h.set_option("mc_engine", 1)
     with pytest.raises(hb.HeaError):                        # the window engine has no ex options
         h.mc_run_ex(occ, cnt, 10, 8, 1, select_best=True)
+
+
+# ---- hea_pool_select (selection step of the global search) against the oracle's pool_select
+@pytest.mark.parametrize("C,n_keep", [(12, 5), (9, 0), (7, 7), (300, 150)])
+def test_pool_select_and_global_iterations(hb, C, n_keep):
+    w = small("bcc", (4, 4, 4), [0.5, 0.25, 0.25], 2, target_seed=3, K=16)
+    h, o = pair(hb, w)
+    occ = h.init_random(C, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    o_occ, o_cnt = occ.cpu().numpy().copy(), counts.cpu().numpy().copy()
+    stats = h.new_stats(C)
+    o_stats = ho.fresh_stats(C)
+    for it in range(3):                                      # local search, then selection: three global iterations
+        h.mc_run(occ, counts, 40, w.K, w.seed, step0=40 * it, stats=stats)
+        o.mc_run(o_occ, o_cnt, 40, w.K, w.seed, step0=40 * it, stats=o_stats, eval_all=False, n_threads=8)
+        if it == 0 and C >= 8:                               # an exact tie: two identical chains
+            occ[C - 1], counts[C - 1], stats[C - 1] = occ[1].clone(), counts[1].clone(), stats[1].clone()
+            o_occ[C - 1], o_cnt[C - 1], o_stats[C - 1] = o_occ[1], o_cnt[1], o_stats[1]
+        order = h.pool_select(occ, counts, stats, n_keep, seed=1234 + it, new_chain0=10_000 * (it + 1))
+        o_order = o.pool_select(o_occ, o_cnt, o_stats, n_keep, seed=1234 + it, new_chain0=10_000 * (it + 1))
+        np.testing.assert_array_equal(order.cpu().numpy(), o_order)
+        np.testing.assert_array_equal(occ.cpu().numpy(), o_occ)
+        np.testing.assert_array_equal(counts.cpu().numpy(), o_cnt)
+        assert_stats_equal(hb.stats_to_numpy(stats), o_stats)
+        np.testing.assert_array_equal(hb.stats_to_numpy(stats)["last_accept_step"], o_stats["last_accept_step"])

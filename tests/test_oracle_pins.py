@@ -523,3 +523,36 @@ def test_mc_ex_reduces_to_the_north_star_rule_and_continues_exactly():
     f_occ, f_cnt = occ0.copy(), cnt0.copy()
     st_f, _ = o.mc_run(f_occ, f_cnt, 1, K, seed, eval_all=False)
     assert (st_e["J"] <= st_f["J"]).all()
+
+
+# ---- the selection step of the global search (Alg. 1)
+def test_pool_select_keeps_the_best_and_reseeds_the_rest():
+    o = make("bcc", (3, 3, 3), [0.5, 0.25, 0.25], 2, target=None)
+    seed, C, K, n_keep = 8, 12, 8, 5
+    occ = o.init_random(C, seed=seed)
+    counts = np.stack([o.pair_counts(occ[c]) for c in range(C)])
+    stats, _ = o.mc_run(occ, counts, 30, K, seed, eval_all=False)
+    occ[7], counts[7], stats[7] = occ[2], counts[2], stats[2]              # an exact tie between slots 2 and 7
+    J = np.array([o.objective(counts[c]) for c in range(C)])
+    occ0, cnt0, st0 = occ.copy(), counts.copy(), stats.copy()
+    order = o.pool_select(occ, counts, stats, n_keep, seed=99, new_chain0=1000)
+    # kept = the n_keep smallest J, ascending, ties by index; nothing kept is worse than anything dropped
+    assert len(set(order.tolist())) == n_keep
+    kept_J = J[order]
+    assert (np.diff(kept_J) >= 0).all()
+    dropped = [c for c in range(C) if c not in set(order.tolist())]
+    assert kept_J.max() <= J[dropped].min()
+    for r in range(n_keep - 1):
+        if kept_J[r] == kept_J[r + 1]:
+            assert order[r] < order[r + 1]
+    if 2 in order.tolist() and 7 in order.tolist():
+        assert order.tolist().index(2) + 1 == order.tolist().index(7)
+    for r, c in enumerate(order):
+        np.testing.assert_array_equal(occ[r], occ0[c])
+        np.testing.assert_array_equal(counts[r], cnt0[c])
+        assert stats[r] == st0[c]
+    # the rest: fresh D8 configurations with the new chain ids, recounted, stats reset
+    np.testing.assert_array_equal(occ[n_keep:], o.init_random(C - n_keep, 99, 1000))
+    for c in range(n_keep, C):
+        np.testing.assert_array_equal(counts[c], o.pair_counts(occ[c]))
+    assert (stats[n_keep:] == ho.fresh_stats(C - n_keep)).all()
