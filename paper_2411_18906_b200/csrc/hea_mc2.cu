@@ -20,6 +20,13 @@
 #include "hea_device.cuh"
 #include "hea_mc_common.cuh"
 
+// The kernel is instantiated for 2 lattices x 2 selection rules x 8 species counts x 2 layouts x 2 target symmetries.
+// To keep the build parallel, this file is compiled four times: HEA_MC2_PART = lattice + 2 * best-of-K (hea_mc2_p1..3.cu
+// include it with the macro set); part 0 also holds the host-side dispatcher.
+#ifndef HEA_MC2_PART
+#define HEA_MC2_PART 0
+#endif
+
 namespace hea {
 
 namespace {
@@ -248,7 +255,7 @@ struct Mc2Args {
 };
 
 // Shared memory: occupancy (offset 0, so a gather address is the loaded offset itself) | Sh2 | offset table [A][ZP].
-template <int M, int OCC, bool SYM, int LAT>
+template <int M, int OCC, bool SYM, int LAT, bool BEST>
 __global__ void __launch_bounds__(kHaloThreads)
 mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __grid_constant__ Mc2Args AA)
 {
@@ -382,7 +389,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         if (w_cap > (uint32_t)A.w_max) w_cap = (uint32_t)A.w_max;
     };
     set_mode(false);
-    const bool best_mode = AA.select_best != 0;
+    constexpr bool best_mode = BEST;
     const unsigned long long depth_limit = AA.depth_limit;
     unsigned long long depth = (depth_limit && AA.depth_all) ? AA.depth_all[chain_local] : 0ull;
     const bool accept_ok = T >= 512 && AA.accept_engine != 0 && !best_mode;   // 8 evaluating warps + null-settling warps
@@ -973,7 +980,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     if (tid == 0 && sh.n_null) atomicAdd(&g_stats[1], sh.n_null);
 }
 
-template <int M, int OCC, bool SYM, int LAT>
+constexpr int kPartLat = HEA_MC2_PART & 1;
+constexpr bool kPartBest = (HEA_MC2_PART >> 1) != 0;
+
+template <int M, int OCC, bool SYM>
 cudaError_t launch2_one(const KParams& P, const DevTables& host_tab, const Mc2Args& AA, int64_t C, int threads, size_t smem,
                         cudaStream_t st)
 {
@@ -984,7 +994,7 @@ cudaError_t launch2_one(const KParams& P, const DevTables& host_tab, const Mc2Ar
             Kc.t[s * M * M + i] = s < P.S ? host_tab.t[s * M * M + i] : 0.0;
         }
     for (int s = 0; s < 4; ++s) Kc.w[s] = host_tab.w[s];
-    auto kern = mc_halo_kernel<M, OCC, SYM, LAT>;
+    auto kern = mc_halo_kernel<M, OCC, SYM, kPartLat, kPartBest>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
@@ -1000,29 +1010,45 @@ cudaError_t launch2_one(const KParams& P, const DevTables& host_tab, const Mc2Ar
     return cudaLaunchKernelEx(&cfg, kern, P, Kc, AA);
 }
 
-template <int M, int OCC, bool SYM>
-cudaError_t launch2_lat(int lat, const KParams& P, const DevTables& host_tab, const Mc2Args& AA, int64_t C, int threads,
-                        size_t smem, cudaStream_t st)
-{
-    return lat == 0 ? launch2_one<M, OCC, SYM, 0>(P, host_tab, AA, C, threads, smem, st)
-                    : launch2_one<M, OCC, SYM, 1>(P, host_tab, AA, C, threads, smem, st);
-}
-
 template <int M>
-cudaError_t launch2_m(bool sym, int occ_mode, int lat, const KParams& P, const DevTables& host_tab, const Mc2Args& AA,
-                      int64_t C, int threads, size_t smem, cudaStream_t st)
+cudaError_t launch2_m(bool sym, int occ_mode, const KParams& P, const DevTables& host_tab, const Mc2Args& AA, int64_t C,
+                      int threads, size_t smem, cudaStream_t st)
 {
     if (occ_mode == OCC2_NIB) {
         if (M > 4) return cudaErrorInvalidValue;            // a nibble holds a one-hot code of at most 4 species
         constexpr int MN = M > 4 ? 4 : M;
-        return sym ? launch2_lat<MN, OCC2_NIB, true>(lat, P, host_tab, AA, C, threads, smem, st)
-                   : launch2_lat<MN, OCC2_NIB, false>(lat, P, host_tab, AA, C, threads, smem, st);
+        return sym ? launch2_one<MN, OCC2_NIB, true>(P, host_tab, AA, C, threads, smem, st)
+                   : launch2_one<MN, OCC2_NIB, false>(P, host_tab, AA, C, threads, smem, st);
     }
-    return sym ? launch2_lat<M, OCC2_U8, true>(lat, P, host_tab, AA, C, threads, smem, st)
-               : launch2_lat<M, OCC2_U8, false>(lat, P, host_tab, AA, C, threads, smem, st);
+    return sym ? launch2_one<M, OCC2_U8, true>(P, host_tab, AA, C, threads, smem, st)
+               : launch2_one<M, OCC2_U8, false>(P, host_tab, AA, C, threads, smem, st);
 }
 
 }  // namespace
+
+#define HEA_MC2_CAT2(a, b) a##b
+#define HEA_MC2_CAT(a, b) HEA_MC2_CAT2(a, b)
+// this part's entry: AA points to an Mc2Args (same layout in every part)
+cudaError_t HEA_MC2_CAT(launch_mc2_part, HEA_MC2_PART)(bool sym, int occ_mode, const KParams& P, const DevTables& host_tab,
+                                                       const void* AA_, int64_t C, int threads, size_t smem, cudaStream_t st)
+{
+    const Mc2Args& AA = *reinterpret_cast<const Mc2Args*>(AA_);
+    switch (P.M) {
+        case 1: return launch2_m<1>(sym, occ_mode, P, host_tab, AA, C, threads, smem, st);
+        case 2: return launch2_m<2>(sym, occ_mode, P, host_tab, AA, C, threads, smem, st);
+        case 3: return launch2_m<3>(sym, occ_mode, P, host_tab, AA, C, threads, smem, st);
+        case 4: return launch2_m<4>(sym, occ_mode, P, host_tab, AA, C, threads, smem, st);
+        case 5: return launch2_m<5>(sym, occ_mode, P, host_tab, AA, C, threads, smem, st);
+        case 6: return launch2_m<6>(sym, occ_mode, P, host_tab, AA, C, threads, smem, st);
+        case 7: return launch2_m<7>(sym, occ_mode, P, host_tab, AA, C, threads, smem, st);
+        default: return launch2_m<8>(sym, occ_mode, P, host_tab, AA, C, threads, smem, st);
+    }
+}
+
+#if HEA_MC2_PART == 0
+cudaError_t launch_mc2_part1(bool, int, const KParams&, const DevTables&, const void*, int64_t, int, size_t, cudaStream_t);
+cudaError_t launch_mc2_part2(bool, int, const KParams&, const DevTables&, const void*, int64_t, int, size_t, cudaStream_t);
+cudaError_t launch_mc2_part3(bool, int, const KParams&, const DevTables&, const void*, int64_t, int, size_t, cudaStream_t);
 
 // Shared-memory bytes of the halo engine (occ_mode 1 = one-hot bytes, 2 = one-hot nibbles).
 size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L)
@@ -1083,19 +1109,15 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
     else { G.basis = (1u << 3) | (1u << 4) | (1u << 5); G.d2[0] = 3; G.d2[1] = 4; G.d2[2] = 8; }
     G.distinct = P.L[0] >= 3 && P.L[1] >= 3 && P.L[2] >= 3;
     const size_t smem = mc2_shared_bytes(occ_mode, lattice, P.L);
-    cudaError_t e;
-    switch (P.M) {
-        case 1: e = launch2_m<1>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
-        case 2: e = launch2_m<2>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
-        case 3: e = launch2_m<3>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
-        case 4: e = launch2_m<4>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
-        case 5: e = launch2_m<5>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
-        case 6: e = launch2_m<6>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
-        case 7: e = launch2_m<7>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
-        default: e = launch2_m<8>(sym, occ_mode, lattice, P, host_tab, AA, C, threads, smem, st); break;
-    }
+    const int part = (lattice != 0 ? 1 : 0) + (select_best ? 2 : 0);
+    cudaError_t e = part == 0 ? launch_mc2_part0(sym, occ_mode, P, host_tab, &AA, C, threads, smem, st)
+                  : part == 1 ? launch_mc2_part1(sym, occ_mode, P, host_tab, &AA, C, threads, smem, st)
+                  : part == 2 ? launch_mc2_part2(sym, occ_mode, P, host_tab, &AA, C, threads, smem, st)
+                              : launch_mc2_part3(sym, occ_mode, P, host_tab, &AA, C, threads, smem, st);
     if (e == cudaSuccess) ++*n_launches;
     return e;
 }
+
+#endif  // HEA_MC2_PART == 0
 
 }  // namespace hea
