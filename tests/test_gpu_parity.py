@@ -467,3 +467,67 @@ def test_pool_select_and_global_iterations(hb, C, n_keep):
         np.testing.assert_array_equal(counts.cpu().numpy(), o_cnt)
         assert_stats_equal(hb.stats_to_numpy(stats), o_stats)
         np.testing.assert_array_equal(hb.stats_to_numpy(stats)["last_accept_step"], o_stats["last_accept_step"])
+
+
+# ---- full sizes, in the launch configuration of bench.py: every chain on the GPU, sampled chains through the oracle
+def full_size_sampled(hb, w, n_steps, sample, threads=8):
+    h, o = pair(hb, w)
+    C = w.n_chains
+    occ = h.init_random(C, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    occ0 = occ.cpu().numpy().copy()
+    stats, _ = h.mc_run(occ, counts, n_steps, w.K, w.seed)
+    got = hb.stats_to_numpy(stats)
+    occ_f, cnt_f = occ.cpu().numpy(), counts.cpu().numpy()
+    # properties that hold at any size, on every chain
+    for c in range(C):
+        np.testing.assert_array_equal(np.bincount(occ_f[c], minlength=h.M), np.bincount(occ0[c], minlength=h.M))
+    recount, _, obj = h.sro_full(occ)
+    np.testing.assert_array_equal(recount.cpu().numpy(), cnt_f)                 # incremental == recount
+    np.testing.assert_array_equal(obj.cpu().numpy(), got["J"])
+    null_rate = got["n_null"].sum() / (C * n_steps * w.K)
+    assert abs(null_rate - sum(x * x for x in w.conc) ** 2) < 2e-3             # (sum c_i^2)^2
+    # sampled chains, element by element (chain c is independent of the batch it runs in)
+    for c in sample:
+        o_occ = o.init_random(1, w.seed, chain0=c)
+        np.testing.assert_array_equal(o_occ[0], occ0[c])
+        o_cnt = np.stack([o.pair_counts(o_occ[0])])
+        o_st, _ = o.mc_run(o_occ, o_cnt, n_steps, w.K, w.seed, chain0=c, n_threads=1, eval_all=False)
+        np.testing.assert_array_equal(occ_f[c], o_occ[0])
+        np.testing.assert_array_equal(cnt_f[c], o_cnt[0])
+        assert_stats_equal(got[c:c + 1], o_st)
+    return got
+
+
+def test_full_size_c2_all_chains_full_length(hb):
+    w = wl.config(2)                                        # 1,024 chains x 100,000 steps x K=32
+    full_size_sampled(hb, w, w.n_steps, sample=[0, 517, 1023])
+
+
+def test_full_size_c3_all_chains(hb):
+    w = wl.config(3)                                        # 256 chains x K=64; 200,000 of the 1e6 steps (oracle time)
+    full_size_sampled(hb, w, 200_000, sample=[0, 255])
+
+
+def test_full_size_c4_full_trajectory(hb):
+    w = wl.config(4)                                        # 16 chains x 1e7 steps x K=128: the bench step
+    h, o = pair(hb, w)
+    got = full_size_sampled(hb, w, w.n_steps, sample=[])
+    assert (got["n_accept"] > 60_000).all() and (got["J"] < 1e-8).all()
+    # the same trajectory cut into two calls (different window and team schedules) gives the same moves
+    occ = h.init_random(w.n_chains, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    stats, _ = h.mc_run(occ, counts, 3_000_000, w.K, w.seed)
+    h.mc_run(occ, counts, 7_000_000, w.K, w.seed, step0=3_000_000, stats=stats)
+    st2 = hb.stats_to_numpy(stats)
+    for f in ("n_accept", "n_null", "hash", "last_accept_step", "J"):
+        np.testing.assert_array_equal(got[f], st2[f])
+    # one sampled chain against the oracle over the first 1,000,000 steps (accept regime, transition, 930,000 reject steps)
+    o_occ = o.init_random(1, w.seed, chain0=11)
+    o_cnt = np.stack([o.pair_counts(o_occ[0])])
+    o_st, _ = o.mc_run(o_occ, o_cnt, 1_000_000, w.K, w.seed, chain0=11, n_threads=1, eval_all=False)
+    occ = h.init_random(w.n_chains, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    stats, _ = h.mc_run(occ, counts, 1_000_000, w.K, w.seed)
+    assert_stats_equal(hb.stats_to_numpy(stats)[11:12], o_st)
+    np.testing.assert_array_equal(occ.cpu().numpy()[11], o_occ[0])
