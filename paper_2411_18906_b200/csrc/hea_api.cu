@@ -30,7 +30,7 @@ cudaError_t launch_pool_gather(const void* src, void* dst, const int32_t* order,
 size_t mc2_team_bytes(int64_t C);
 constexpr int kMc2MaxThreads = 512;
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
-                       void* team_ctl, int team_on, int team_off, int accept_engine, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
+                       void* team_ctl, int team_on, int team_off, int accept_engine, size_t smem_budget, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
                        uint64_t step0, void* stats, void* log, int64_t log_cap, int select_best, uint64_t depth_limit,
                        uint64_t* depth, uint64_t* steps_done, cudaStream_t st, int64_t* n_launches);
 }  // namespace hea
@@ -127,7 +127,7 @@ bool option_value_ok(const char* name, int64_t v)
     if (!strcmp(name, "mc_neighbors")) return v == 1 || v == 2;
     if (!strcmp(name, "mc_engine")) return v == 1 || v == 2;
     if (!strcmp(name, "mc_team")) return v >= 1 && v <= 32;
-    if (!strcmp(name, "mc_accept")) return v == 1 || v == 2;
+    if (!strcmp(name, "mc_accept")) return v >= 1 && v <= 3;      // 1 off, 2 single-step engine, 3 (= default) pipelined
     if (!strcmp(name, "mc_team_on") || !strcmp(name, "mc_team_off")) return v >= 1 && v <= (1 << 30);
     if (!strcmp(name, "sro_stages")) return v >= 1 && v <= 8;
     if (!strcmp(name, "sro_blocks_per_sm")) return v >= 1 && v <= 4;
@@ -426,7 +426,8 @@ int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C
         }
         const int w_max2 = ctx->opt_window ? (int)ctx->opt_window : (1 << 20);
         cudaError_t e2 = hea::launch_mc2(ctx->P, ctx->tab_host, ctx->lat.type, om, threads, team, team_ctl,
-                                         (int)ctx->opt_team_on, (int)ctx->opt_team_off, ctx->opt_accept == 1 ? 0 : 1, w_max2, occ_dev, counts_dev, C,
+                                         (int)ctx->opt_team_on, (int)ctx->opt_team_off,
+                                         ctx->opt_accept == 1 ? 0 : ctx->opt_accept == 2 ? 1 : 2, budget, w_max2, occ_dev, counts_dev, C,
                                          n_steps, K, seed, chain0, step0, stats_dev, log_dev, log_cap, select_best,
                                          depth_limit, depth_dev, steps_done_dev, (cudaStream_t)cuda_stream,
                                          &ctx->n_launches);

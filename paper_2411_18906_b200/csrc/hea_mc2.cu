@@ -52,6 +52,18 @@ struct Geo {
 };
 
 constexpr int kQueueCap = 2048;
+constexpr int kPaeK = 16;                   // pipelined accept engine: candidates per step evaluated ahead
+constexpr int kPaeRecs = 512;               // records per epoch (= block threads): kPaeRecs / kPaeK steps
+
+// A candidate evaluated ahead of its step (pipelined accept engine): everything that depends on the configuration but
+// not on the pair counts.  Valid as long as none of its drawn sites was touched (or had a neighbour touched) since.
+struct PRec {
+    uint32_t a, b;                // the proposal after the redraw rule
+    uint32_t a1, b1;              // the first draw (decides the redraw)
+    uint32_t pqn;                 // p | q << 8 | null << 16 | absent << 17
+    uint32_t pad;
+    unsigned long long d0, d1, d2;   // Pack<M> species-count differences per shell, adjacency-corrected
+};
 
 struct Sh2 {
     int cnt[kSMM];
@@ -247,6 +259,7 @@ struct Mc2Args {
     TeamCtl* team;                // [C] control blocks, zeroed before the launch (R > 1 only)
     int team_on, team_off;        // enter TEAM when W*K >= team_on; leave it after a move with steps_done*K < team_off
     int accept_engine;            // 1: single-step windows run on the 8-lanes-per-candidate engine
+    int pae;                      // 1: ... pipelined over epochs of steps (record, dirty-bitmap and offset buffers present)
     // hea_mc_run_ex
     int select_best;              // 1: the minimum J_k of a step is taken (ties -> lowest k) instead of the lowest improving k
     unsigned long long depth_limit;        // > 0: a chain stops after this many consecutive steps without a move
@@ -271,6 +284,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     uint8_t* s_occ = s_raw;
     Sh2& sh = *reinterpret_cast<Sh2*>(s_raw + occ_bytes);
     int* s_tab = reinterpret_cast<int*>(s_raw + occ_bytes + ((sizeof(Sh2) + 15) & ~(size_t)15));
+    // pipelined accept engine buffers (only when AA.pae): records | dirty bitmap over logical sites | logical offsets [A][Z]
+    PRec* s_prec = reinterpret_cast<PRec*>(s_tab + LC::A * ZP);
+    uint32_t* s_dirty = reinterpret_cast<uint32_t*>(s_prec + kPaeRecs);
+    int* s_loff = reinterpret_cast<int*>(s_dirty + ((P.N + 31) >> 5));
 
     const int tid = threadIdx.x, T = blockDim.x;
     const int S = P.S, N = P.N, K = A.K, R = A.R;
@@ -342,6 +359,14 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         s_tab[i] = entry;
     }
     for (int i = tid; i < SMM; i += T) { sh.g[i] = Kc.g[i]; sh.t[i] = Kc.t[i]; }
+    if (AA.pae) {
+        for (int i = tid; i < ((P.N + 31) >> 5); i += T) s_dirty[i] = 0u;
+        for (int i = tid; i < LC::A * P.Z; i += T) {      // neighbour e of a site of basis b without periodic wrap
+            const int8_t* st = P.tab->stencil + i * 4;
+            const int b = i / P.Z;
+            s_loff[i] = ((((int)st[1] * Ly + (int)st[2]) * Lz + (int)st[3]) << LC::lgA) + ((int)st[0] - b);
+        }
+    }
     if (tid < 24) {
         // word list of the accept engine: per shell s < S the NA_s words of site a, then the NA_s words of site b
         int w = tid, s = 0, side = 0, g = 0, rowoff = 0;
@@ -425,6 +450,21 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 }
             }
         }
+        if (AA.pae && tid >= 32 && tid < 64) {
+            // pipelined accept engine: the two sites and all their neighbours are now "touched"
+            const int lane = tid - 32;
+#pragma unroll 1
+            for (int which = 0; which < 2; ++which) {
+                const uint32_t u = which ? mv->b : mv->a;
+                const SiteC sc = decode_site<LAT>(G, u);
+                const bool interior = sc.x >= 1 && sc.x <= Lx - 2 && sc.y >= 1 && sc.y <= Ly - 2 && sc.z >= 1 && sc.z <= Lz - 2;
+                for (int e = lane; e < P.Z; e += 32) {
+                    const uint32_t v = interior ? u + (uint32_t)s_loff[sc.b * P.Z + e] : (uint32_t)__ldg(nbr + (size_t)u * P.Z + e);
+                    atomicOr(&s_dirty[v >> 5], 1u << (v & 31u));
+                }
+                if (lane == 0) atomicOr(&s_dirty[u >> 5], 1u << (u & 31u));
+            }
+        }
         if (tid == T - 2) {
             const uint32_t a = mv->a, b = mv->b;
             sh.J = mv->J;
@@ -451,11 +491,12 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     };
 
     // D9.1: the proposal of candidate (step, k): sites, their decoded positions and one-hot species (equal codes = null)
-    auto propose = [&](unsigned long long step, uint32_t k, uint32_t& a, uint32_t& b, SiteC& sa, SiteC& sb, uint32_t& hp,
-                       uint32_t& hq) {
+    auto propose2 = [&](unsigned long long step, uint32_t k, uint32_t& a, uint32_t& b, SiteC& sa, SiteC& sb, uint32_t& hp,
+                        uint32_t& hq, uint32_t& a1, uint32_t& b1) {
         const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), k, chain, key0, key1);
         a = __umulhi(r.x, (uint32_t)N); b = __umulhi(r.y, (uint32_t)N - 1u);
         b += (b >= a);
+        a1 = a; b1 = b;
         sa = decode_site<LAT>(G, a); sb = decode_site<LAT>(G, b);
         hp = occ_get<OCC>(s_occ, sa.pidx); hq = occ_get<OCC>(s_occ, sb.pidx);
         if (hp == hq) {
@@ -464,6 +505,11 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             sa = decode_site<LAT>(G, a); sb = decode_site<LAT>(G, b);
             hp = occ_get<OCC>(s_occ, sa.pidx); hq = occ_get<OCC>(s_occ, sb.pidx);
         }
+    };
+    auto propose = [&](unsigned long long step, uint32_t k, uint32_t& a, uint32_t& b, SiteC& sa, SiteC& sb, uint32_t& hp,
+                       uint32_t& hq) {
+        uint32_t a1, b1;
+        propose2(step, k, a, b, sa, sb, hp, hq, a1, b1);
     };
     // D9.2: per shell, (entries of a's row equal to b) - (entries of a row equal to its own site)
     auto adjacency = [&](uint32_t a, uint32_t b, const SiteC& sa, const SiteC& sb, int& mm0, int& mm1, int& mm2) {
@@ -501,15 +547,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     constexpr int NWR = (2 * (NA0 + NA1 + NA2) + 7) / 8;                          // word rounds per lane
     constexpr int NRR = (3 * M + 7) / 8;                                          // row rounds per lane
     const int nw = 2 * (NA0 + (S > 1 ? NA1 : 0) + (S > 2 ? NA2 : 0));
-    auto eval_g8 = [&](unsigned long long step, uint32_t k, bool valid, int grp, int buf, double J_cur) {
+    // species-count differences of all shells for the candidate (sa, sb), the 8 lanes of a group sharing the gathers
+    auto g8_F = [&](const SiteC& sa, const SiteC& sb, int mm0, int mm1, int mm2, int p, int q, int (&c)[M], int (&F0)[M],
+                    int (&F1)[M], int (&F2)[M]) {
         const int l8 = tid & 7;
-        uint32_t a, b, hp, hq;
-        SiteC sa, sb;
-        propose(step, k, a, b, sa, sb, hp, hq);
-        const bool live = valid && hp != hq;
-        const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
-        int mm0, mm1, mm2;
-        adjacency(a, b, sa, sb, mm0, mm1, mm2);
         // gathers: this lane's accumulator words -> biased species counts (+ for b's neighbours, - for a's)
         PD D0 = 0, D1 = 0, D2 = 0;
         PD bias4 = 0;
@@ -550,7 +591,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             if (S > 1) D1 += __shfl_xor_sync(0xFFFFFFFFu, D1, o);
             if (S > 2) D2 += __shfl_xor_sync(0xFFFFFFFFu, D2, o);
         }
-        int c[M], F0[M], F1[M], F2[M];
         {
             int l0 = 0, l1 = 0, l2 = 0;
 #pragma unroll
@@ -575,6 +615,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
 #pragma unroll
             for (int r2 = 0; r2 < M; ++r2) { F0[r2] -= mm0 * c[r2]; F1[r2] -= mm1 * c[r2]; F2[r2] -= mm2 * c[r2]; }
         }
+    };
+    // J of the candidate from the current counts and its F, rows dealt over the 8 lanes, combined in the D6 order
+    auto g8_J = [&](const int (&c)[M], int p, int q, const int (&F0)[M], const int (&F1)[M], const int (&F2)[M]) -> double {
+        const int l8 = tid & 7;
         // rows of the objective: row rho = s*M + i on lane rho & 7
         double rowv[NRR];
 #pragma unroll
@@ -612,12 +656,30 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[s], shs));
             }
         }
+        return Jk;
+    };
+    auto g8_post = [&](bool live, double Jk, double J_cur, uint32_t k, uint32_t a, uint32_t b, int p, int q,
+                       const int (&F0)[M], const int (&F1)[M], const int (&F2)[M], int grp, int buf) {
+        const int l8 = tid & 7;
         if (l8 == 0 && live && Jk < J_cur) {
             MoveRec& m = sh.cand[grp];
             m.key = k; m.a = a; m.b = b; m.pq = (uint32_t)p | ((uint32_t)q << 8); m.J = Jk;
             m.d[0] = pack_F<M>(F0); m.d[1] = pack_F<M>(F1); m.d[2] = pack_F<M>(F2);
             atomicMin(&sh.best[buf], k);
         }
+    };
+    auto eval_g8 = [&](unsigned long long step, uint32_t k, bool valid, int grp, int buf, double J_cur) {
+        uint32_t a, b, hp, hq;
+        SiteC sa, sb;
+        propose(step, k, a, b, sa, sb, hp, hq);
+        const bool live = valid && hp != hq;
+        const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+        int mm0, mm1, mm2;
+        adjacency(a, b, sa, sb, mm0, mm1, mm2);
+        int c[M], F0[M], F1[M], F2[M];
+        g8_F(sa, sb, mm0, mm1, mm2, p, q, c, F0, F1, F2);
+        const double Jk = g8_J(c, p, q, F0, F1, F2);
+        g8_post(live, Jk, J_cur, k, a, b, p, q, F0, F1, F2, grp, buf);
     };
 
     unsigned long long t0 = A.step0;
@@ -651,7 +713,147 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             continue;
         }
         uint32_t key_best = kNoKey, steps_done = 1u;
-        if (accept_ok && !team && W == 1u) {
+        if (accept_ok && !team && W == 1u && AA.pae) {
+            // ---- pipelined accept engine.  In the accept regime nearly every step applies a move found among its first
+            // few candidates, and a step is one candidate evaluation long.  What depends only on the configuration
+            // (proposal, adjacency, the 2Z gathers) is therefore computed AHEAD for an epoch of T / 16 steps x 16
+            // candidates, one record per thread; the serial part of a step is the objective of those records against
+            // the current counts (8 lanes per record), the selection, and the move.  A record is stale once a move has
+            // touched one of its drawn sites or one of their neighbours: every move marks its two sites and their
+            // neighbours in a bitmap, and a warp that meets a stale record recomputes its records from the current
+            // configuration.  Steps whose first 16 candidates do not improve fall back to rounds of 32 candidates.
+            const uint32_t n_ep = (uint32_t)min((unsigned long long)(T / kPaeK), t_end - t0);
+            {
+                const uint32_t es = (uint32_t)tid / (uint32_t)kPaeK, k = (uint32_t)tid % (uint32_t)kPaeK;
+                if ((uint32_t)tid < n_ep * (uint32_t)kPaeK) {
+                    PRec rec;
+                    rec.pad = 0; rec.d0 = rec.d1 = rec.d2 = 0ull; rec.a = rec.b = rec.a1 = rec.b1 = 0u;
+                    rec.pqn = 1u << 17;                                   // absent (k >= K)
+                    if (k < (uint32_t)K) {
+                        uint32_t a, b, hp, hq, a1, b1;
+                        SiteC sa, sb;
+                        propose2(t0 + es, k, a, b, sa, sb, hp, hq, a1, b1);
+                        rec.a = a; rec.b = b; rec.a1 = a1; rec.b1 = b1;
+                        if (hp == hq) {
+                            rec.pqn = 1u << 16;                           // null
+                        } else {
+                            const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+                            int c[M], F0[M], F1[M], F2[M];
+#pragma unroll
+                            for (int r2 = 0; r2 < M; ++r2) { c[r2] = (r2 == p) - (r2 == q); F1[r2] = 0; F2[r2] = 0; }
+                            int mm0, mm1, mm2;
+                            adjacency(a, b, sa, sb, mm0, mm1, mm2);
+                            const int4* ta = reinterpret_cast<const int4*>(s_tab + sa.b * ZP);
+                            const int4* tb = reinterpret_cast<const int4*>(s_tab + sb.b * ZP);
+                            {
+                                uint32_t xa[NA0], xb[NA0];
+                                gather_shell<OCC, LC::z0>(s_occ, ta, sa.pidx, xa);
+                                gather_shell<OCC, LC::z0>(s_occ, tb, sb.pidx, xb);
+                                hist_diff<M, NA0>(xa, xb, F0);
+                            }
+                            if (S > 1) {
+                                uint32_t xa[NA1], xb[NA1];
+                                gather_shell<OCC, LC::z1>(s_occ, ta + NA0, sa.pidx, xa);
+                                gather_shell<OCC, LC::z1>(s_occ, tb + NA0, sb.pidx, xb);
+                                hist_diff<M, NA1>(xa, xb, F1);
+                            }
+                            if (S > 2) {
+                                uint32_t xa[NA2], xb[NA2];
+                                gather_shell<OCC, LC::z2>(s_occ, ta + NA0 + NA1, sa.pidx, xa);
+                                gather_shell<OCC, LC::z2>(s_occ, tb + NA0 + NA1, sb.pidx, xb);
+                                hist_diff<M, NA2>(xa, xb, F2);
+                            }
+#pragma unroll
+                            for (int r2 = 0; r2 < M; ++r2) { F0[r2] -= mm0 * c[r2]; F1[r2] -= mm1 * c[r2]; F2[r2] -= mm2 * c[r2]; }
+                            rec.pqn = (uint32_t)p | ((uint32_t)q << 8);
+                            rec.d0 = (unsigned long long)pack_F<M>(F0); rec.d1 = (unsigned long long)pack_F<M>(F1);
+                            rec.d2 = (unsigned long long)pack_F<M>(F2);
+                        }
+                    }
+                    s_prec[tid] = rec;
+                }
+            }
+            __syncthreads();
+            bool any_move = false;
+            for (uint32_t es = 0; es < n_ep; ++es) {
+                const double J_cur = sh.J;
+                if (tid >= 256) {                                        // which of the K candidates of this step are null
+                    for (uint32_t k = (uint32_t)tid - 256u; k < (uint32_t)K; k += (uint32_t)T - 256u) {
+                        uint32_t a, b, hp, hq;
+                        SiteC sa, sb;
+                        propose(t0, k, a, b, sa, sb, hp, hq);
+                        my_null += hp == hq;
+                    }
+                }
+                int buf = (int)(it % 3u);
+                if (tid < kPaeK * 8) {
+                    const int grp = tid >> 3;
+                    const PRec rec = s_prec[es * kPaeK + grp];
+                    auto dirty = [&](uint32_t v) { return (s_dirty[v >> 5] >> (v & 31u)) & 1u; };
+                    const bool absent = (rec.pqn >> 17) & 1u;
+                    const bool stale = !absent && (dirty(rec.a) | dirty(rec.b) | dirty(rec.a1) | dirty(rec.b1));
+                    uint32_t a = rec.a, b = rec.b;
+                    bool live = !absent && !((rec.pqn >> 16) & 1u);
+                    int p = (int)(rec.pqn & 0xFFu), q = (int)((rec.pqn >> 8) & 0xFFu);
+                    int c[M], F0[M], F1[M], F2[M];
+                    if (__any_sync(0xFFFFFFFFu, stale)) {                // recompute this warp's four records
+                        uint32_t hp, hq;
+                        SiteC sa, sb;
+                        propose(t0, (uint32_t)grp, a, b, sa, sb, hp, hq);
+                        live = !absent && hp != hq;
+                        p = 31 - __clz((int)hp); q = 31 - __clz((int)hq);
+                        int mm0, mm1, mm2;
+                        adjacency(a, b, sa, sb, mm0, mm1, mm2);
+                        g8_F(sa, sb, mm0, mm1, mm2, p, q, c, F0, F1, F2);
+                    } else {
+#pragma unroll
+                        for (int r2 = 0; r2 < M; ++r2) {
+                            c[r2] = live ? (r2 == p) - (r2 == q) : 0;
+                            F0[r2] = Pack<M>::field((PW)rec.d0, r2); F1[r2] = Pack<M>::field((PW)rec.d1, r2);
+                            F2[r2] = Pack<M>::field((PW)rec.d2, r2);
+                        }
+                    }
+                    const double Jk = g8_J(c, p, q, F0, F1, F2);
+                    g8_post(live, Jk, J_cur, (uint32_t)grp, a, b, p, q, F0, F1, F2, grp, buf);
+                }
+                __syncthreads();
+                key_best = sh.best[buf];
+                if (tid == 0) { sh.best[(buf + 2) % 3] = kNoKey; sh.q_n[(buf + 2) % 3] = 0u; }
+                ++it;
+                uint32_t rd0 = 0;
+                if (key_best == kNoKey) {                                // none of the first 16: the other candidates
+                    for (rd0 = (uint32_t)kPaeK; rd0 < (uint32_t)K; rd0 += 32u) {
+                        buf = (int)(it % 3u);
+                        if (tid < 256) {
+                            const uint32_t k = rd0 + ((uint32_t)tid >> 3);
+                            eval_g8(t0, k, k < (uint32_t)K, tid >> 3, buf, J_cur);
+                        }
+                        __syncthreads();
+                        key_best = sh.best[buf];
+                        if (tid == 0) { sh.best[(buf + 2) % 3] = kNoKey; sh.q_n[(buf + 2) % 3] = 0u; }
+                        ++it;
+                        if (key_best != kNoKey) break;
+                    }
+                }
+                if (key_best != kNoKey) {
+                    apply_move(&sh.cand[key_best - rd0], key_best, t0);
+                    any_move = true;
+                    depth = 0;
+                    t0 += 1;
+                } else {
+                    W = min(2u, w_cap);
+                    depth += 1;
+                    t0 += 1;
+                    break;
+                }
+            }
+            if (any_move) {                                              // new epoch, clean bitmap
+                for (int i = tid; i < ((N + 31) >> 5); i += T) s_dirty[i] = 0u;
+            }
+            __syncthreads();
+            steps_done = 0u;                                             // t0 already advanced
+            key_best = kNoKey;
+        } else if (accept_ok && !team && W == 1u) {
             // ---- accept engine: this one step, 32 candidates per round on the first 8 warps; the other warps settle
             // which candidates of the step are null (all K count, D9.1)
             const double J_cur = sh.J;
@@ -1064,7 +1266,7 @@ size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L)
 size_t mc2_team_bytes(int64_t C) { return sizeof(TeamCtl) * (size_t)C; }
 
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
-                       void* team_ctl, int team_on, int team_off, int accept_engine, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
+                       void* team_ctl, int team_on, int team_off, int accept_engine, size_t smem_budget, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
                        uint64_t step0, void* stats, void* log, int64_t log_cap, int select_best, uint64_t depth_limit,
                        uint64_t* depth, uint64_t* steps_done, cudaStream_t st, int64_t* n_launches)
 {
@@ -1108,7 +1310,11 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
     if (lattice == 0) { G.basis = (1u << 4) | (1u << 5) | (1u << 6) | (1u << 8) | (1u << 9) | (1u << 10); G.d2[0] = 2; G.d2[1] = 4; G.d2[2] = 6; }
     else { G.basis = (1u << 3) | (1u << 4) | (1u << 5); G.d2[0] = 3; G.d2[1] = 4; G.d2[2] = 8; }
     G.distinct = P.L[0] >= 3 && P.L[1] >= 3 && P.L[2] >= 3;
-    const size_t smem = mc2_shared_bytes(occ_mode, lattice, P.L);
+    size_t smem = mc2_shared_bytes(occ_mode, lattice, P.L);
+    // the pipelined accept engine needs its record, bitmap and offset buffers on top; without room it is simply off
+    const size_t pae_bytes = sizeof(PRec) * (size_t)kPaeRecs + 4u * (size_t)((P.N + 31) >> 5) + 4u * (size_t)P.A * (size_t)P.Z + 16u;
+    AA.pae = (accept_engine == 2 && threads >= 512 && smem + pae_bytes <= smem_budget) ? 1 : 0;
+    if (AA.pae) smem += pae_bytes;
     const int part = (lattice != 0 ? 1 : 0) + (select_best ? 2 : 0);
     cudaError_t e = part == 0 ? launch_mc2_part0(sym, occ_mode, P, host_tab, &AA, C, threads, smem, st)
                   : part == 1 ? launch_mc2_part1(sym, occ_mode, P, host_tab, &AA, C, threads, smem, st)

@@ -213,10 +213,12 @@ def test_mc_halo_engine_teams_reject_regime(hb, team, threads):
                                                    ("fcc", (3, 3, 3), [0.5, 0.5], 1, 33), ("bcc", (4, 4, 4), [1 / 8] * 8, 2, 128),
                                                    ("fcc", (2, 2, 2), [0.25] * 4, 3, 40), ("fcc", (5, 4, 3), [1 / 6] * 6, 3, 17)])
 @pytest.mark.parametrize("threads,team", [(512, 1), (1024, 1), (1024, 3)])
-def test_mc_halo_engine_accept_engine(hb, lattice, dims, conc, S, K, threads, team):
-    # single-step windows run 8 lanes per candidate (T >= 512); same trajectory as thread-per-candidate and the oracle
+@pytest.mark.parametrize("accept", [2, 3])
+def test_mc_halo_engine_accept_engine(hb, lattice, dims, conc, S, K, threads, team, accept):
+    # single-step windows run 8 lanes per candidate (T >= 512), accept = 3: pipelined over epochs with records computed
+    # ahead (small cells make most records stale: the recompute path); same trajectory as thread-per-candidate and the oracle
     w = small(lattice, dims, conc, S, target_seed=9, K=K, n_steps=400, rng=(-0.2, 0.2))
-    st = run_both(hb, w, 3, 400, log_cap=400, opts={"mc_engine": 2, "mc_threads": threads, "mc_team": team, "mc_accept": 2})
+    st = run_both(hb, w, 3, 400, log_cap=400, opts={"mc_engine": 2, "mc_threads": threads, "mc_team": team, "mc_accept": accept})
     assert st["n_accept"].sum() > 5
 
 
