@@ -98,9 +98,17 @@ int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host);
  *   "mc_window"       cap on the speculative step window (steps evaluated against one configuration before the
  *                     lowest improving (step, k) is applied): 0 = auto, 1 = strictly step by step, up to 2^20
  *   "mc_neighbors"    0 = auto, 1 = always the neighbour table, 2 = interior sites use site + offset (no table load)
- *   "sro_warps"       recount: warps per block, 0 = auto (16), 1..16
- *   "sro_stages"      recount: cap on the per-warp ring of 32-site table tiles in shared memory, 0 = auto, 1..8
- *   "sro_blocks_per_sm"  recount: resident blocks per SM the grid and the shared-memory split are sized for, 0 = auto, 1..4
+ *   "sro_engine"      recount: 0 = auto (the table-free stencil kernel when occ_dev is aligned to the basis size,
+ *                     else the table-driven kernel), 1 = table-driven (HBM-bound, 4 Z + 1 bytes per atom),
+ *                     2 = stencil (1 byte per atom; HEA_EINVAL when occ_dev is not aligned)
+ *   "sro_tile_xy"     stencil recount: cap on the tile extent along x and y in cells, 0 = auto (8), 1..8
+ *   "sro_tile_z"      stencil recount: row pitch of the staged tile, 0 = auto, else 12, 22 or 34 (tiles of up to
+ *                     10, 20, 32 cells along z)
+ *   "sro_flush_tiles" stencil recount: cap on the tiles a thread accumulates before its packed rows are unpacked,
+ *                     0 = auto (what the packed fields hold), 1..2^20
+ *   "sro_warps"       table recount: warps per block, 0 = auto (16), 1..16
+ *   "sro_stages"      table recount: cap on the per-warp ring of 32-site table tiles in shared memory, 0 = auto, 1..8
+ *   "sro_blocks_per_sm"  recount (both engines): resident blocks per SM the grid and the shared-memory split are sized for, 0 = auto, 1..4
  * Unknown name or value -> HEA_EINVAL.
  */
 int hea_set_option(hea_ctx* ctx, const char* name, int64_t value);

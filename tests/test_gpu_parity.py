@@ -50,10 +50,15 @@ def test_info_and_neighbor_table(hb, lattice, dims, conc, S):
         np.testing.assert_array_equal(h.neighbor_table(s), o.neighbor_table(s))
 
 
+SRO_ENGINES = [1, 2]          # 1 = table-driven (hea_sro.cu), 2 = table-free stencil (hea_sro2.cu); 0 = auto picks 2
+
+
+@pytest.mark.parametrize("engine", SRO_ENGINES)
 @pytest.mark.parametrize("lattice,dims,conc,S", LATTICES)
-def test_init_and_sro_full_bit_exact(hb, lattice, dims, conc, S):
+def test_init_and_sro_full_bit_exact(hb, lattice, dims, conc, S, engine):
     w = small(lattice, dims, conc, S, target_seed=3)
     h, o = pair(hb, w)
+    h.set_option("sro_engine", engine)
     B = 5
     occ = h.init_random(B, seed=w.seed, chain0=7)
     want_occ = o.init_random(B, seed=w.seed, chain0=7)
@@ -65,10 +70,12 @@ def test_init_and_sro_full_bit_exact(hb, lattice, dims, conc, S):
     np.testing.assert_array_equal(obj.cpu().numpy(), wj)
 
 
-def test_sro_full_ordered_structures(hb):
+@pytest.mark.parametrize("engine", SRO_ENGINES)
+def test_sro_full_ordered_structures(hb, engine):
     # B2 on bcc: closed form alpha (+1/-1), through the GPU path
     w = small("bcc", (6, 6, 6), [0.5, 0.5], 3)
     h, o = pair(hb, w)
+    h.set_option("sro_engine", engine)
     import torch
     occ = torch.tensor(np.arange(h.N, dtype=np.int64) % 2, dtype=torch.uint8, device="cuda").reshape(1, -1)
     counts, alpha, obj = h.sro_full(occ)
@@ -78,8 +85,9 @@ def test_sro_full_ordered_structures(hb):
     np.testing.assert_array_equal(counts.cpu().numpy()[0], o.pair_counts(occ.cpu().numpy()[0]))
 
 
+@pytest.mark.parametrize("engine", SRO_ENGINES)
 @pytest.mark.parametrize("L,B", [(10, 3), (16, 2), (23, 1)])
-def test_sro_full_multi_tile_and_ragged(hb, L, B):
+def test_sro_full_multi_tile_and_ragged(hb, L, B, engine):
     # several blocks / grid-stride iterations, flushes of the 16-bit accumulators, N % 4 != 0 for bcc odd L
     for lattice, conc in (("fcc", [0.2] * 5), ("bcc", None)):
         if conc is None:
@@ -87,11 +95,100 @@ def test_sro_full_multi_tile_and_ragged(hb, L, B):
             conc = [0.5, 0.25, 0.25] if n % 4 == 0 else [0.5, 0.5]
         w = small(lattice, (L, L, L), conc, 3, target_seed=9)
         h, o = pair(hb, w)
+        h.set_option("sro_engine", engine)
         occ = h.init_random(B, seed=5)
         counts, alpha, obj = h.sro_full(occ)
         wc, wa, wj = o.sro_full(occ.cpu().numpy(), n_threads=4)
         np.testing.assert_array_equal(counts.cpu().numpy(), wc)
         np.testing.assert_array_equal(obj.cpu().numpy(), wj)
+
+
+@pytest.mark.parametrize("lattice,dims,conc,S", [("fcc", (17, 9, 45), [0.2] * 5, 3), ("bcc", (9, 21, 35), [0.25] * 4, 3),
+                                                 ("fcc", (8, 8, 33), [0.5, 0.25, 0.25], 2), ("bcc", (11, 3, 70), [1 / 7] * 7, 3),
+                                                 ("fcc", (2, 13, 1), [0.5, 0.5], 3), ("fcc", (12, 10, 21), [0.125] * 8, 3)])
+@pytest.mark.parametrize("tile_xy,tile_z", [(0, 0), (1, 12), (3, 22), (8, 34), (5, 12)])
+def test_sro_stencil_tilings(hb, lattice, dims, conc, S, tile_xy, tile_z):
+    # the stencil engine over every row-pitch variant, ragged last tiles in all three directions, tiles smaller and
+    # larger than the cell, z extents above one tile; the table engine and the oracle must both agree
+    w = small(lattice, dims, conc, S, target_seed=4)
+    h, o = pair(hb, w)
+    occ = h.init_random(3, seed=11)
+    h.set_option("sro_engine", 1)
+    c_tab, _, _ = h.sro_full(occ)
+    h.set_option("sro_engine", 2)
+    h.set_option("sro_tile_xy", tile_xy)
+    h.set_option("sro_tile_z", tile_z)
+    c_st, _, j_st = h.sro_full(occ)
+    wc, _, wj = o.sro_full(occ.cpu().numpy(), n_threads=4)
+    np.testing.assert_array_equal(c_st.cpu().numpy(), wc)
+    np.testing.assert_array_equal(c_tab.cpu().numpy(), wc)
+    np.testing.assert_array_equal(j_st.cpu().numpy(), wj)
+
+
+@pytest.mark.parametrize("bps,flush", [(1, 2), (1, 0), (4, 1), (0, 3)])
+def test_sro_stencil_blocks_spanning_configurations_and_flushes(hb, bps, flush):
+    # 40 configurations x 18 tiles over 148..592 persistent blocks: blocks cross configuration boundaries in the middle
+    # of their item range and unpack their packed rows every `flush` tiles
+    w = small("fcc", (20, 20, 40), [0.2] * 5, 3, target_seed=6)
+    h, o = pair(hb, w)
+    occ = h.init_random(40, seed=13)
+    h.set_option("sro_engine", 2)
+    h.set_option("sro_blocks_per_sm", bps)
+    h.set_option("sro_flush_tiles", flush)
+    counts, _, obj = h.sro_full(occ)
+    wc, _, wj = o.sro_full(occ.cpu().numpy(), n_threads=8)
+    np.testing.assert_array_equal(counts.cpu().numpy(), wc)
+    np.testing.assert_array_equal(obj.cpu().numpy(), wj)
+
+
+@pytest.mark.parametrize("conc", [[0.01, 0.01, 0.01, 0.01, 0.96], [0.96, 0.01, 0.01, 0.01, 0.01], [0.02, 0.02, 0.02, 0.94],
+                                  [0.005] * 7 + [0.965], [1.0]])
+@pytest.mark.parametrize("tile_z", [12, 22, 34])
+def test_sro_stencil_packed_field_capacity(hb, conc, tile_z):
+    # nearly pure configurations drive single packed fields to their maximum (12 per site and shell): long item ranges
+    # per block (one block per SM) must unpack before any field of the per-thread rows overflows
+    w = small("fcc", (16, 16, 80), conc, 3, target_seed=6)
+    h, o = pair(hb, w)
+    occ = h.init_random(6, seed=17)
+    h.set_option("sro_engine", 2)
+    h.set_option("sro_blocks_per_sm", 1)
+    h.set_option("sro_tile_z", tile_z)
+    counts, _, obj = h.sro_full(occ)
+    wc, _, wj = o.sro_full(occ.cpu().numpy(), n_threads=8)
+    np.testing.assert_array_equal(counts.cpu().numpy(), wc)
+    np.testing.assert_array_equal(obj.cpu().numpy(), wj)
+
+
+def test_sro_stencil_unaligned_occupancy_falls_back_to_table_kernel(hb):
+    import torch
+    w = small("fcc", (6, 6, 6), [0.2] * 5, 3, target_seed=6)
+    h, o = pair(hb, w)
+    occ = h.init_random(2, seed=3)
+    buf = torch.zeros(occ.numel() + 8, dtype=torch.uint8, device="cuda")
+    shifted = buf[1:1 + occ.numel()].view(2, -1)
+    shifted.copy_(occ)
+    assert shifted.data_ptr() % 4 == 1
+    counts, _, _ = h.sro_full(shifted)                       # auto: table kernel (another CUDA kernel, no CPU path)
+    np.testing.assert_array_equal(counts.cpu().numpy(), o.sro_full(occ.cpu().numpy())[0])
+    h.set_option("sro_engine", 2)
+    with pytest.raises(hb.HeaError):
+        h.sro_full(shifted)
+
+
+def test_sro_stencil_full_size_sweep_point(hb):
+    # configs[4] at its largest cell in the launch configuration the sweep times (fcc 100^3, 5 species, 3 shells):
+    # stencil == table engine on every count, and == the oracle
+    w = small("fcc", (100, 100, 100), [0.2] * 5, 3, target_seed=2)
+    h, o = pair(hb, w)
+    occ = h.init_random(2, seed=5)
+    h.set_option("sro_engine", 1)
+    c_tab, _, _ = h.sro_full(occ)
+    h.set_option("sro_engine", 2)
+    c_st, _, j_st = h.sro_full(occ)
+    np.testing.assert_array_equal(c_st.cpu().numpy(), c_tab.cpu().numpy())
+    wc, _, wj = o.sro_full(occ.cpu().numpy(), n_threads=8)
+    np.testing.assert_array_equal(c_st.cpu().numpy(), wc)
+    np.testing.assert_array_equal(j_st.cpu().numpy(), wj)
 
 
 def run_both(hb, w, n_chains, n_steps, log_cap=16, chain0=0, step0=0, opts=None, threads=8):
