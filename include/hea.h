@@ -106,6 +106,7 @@ int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host);
  *                     10, 20, 32 cells along z)
  *   "sro_flush_tiles" stencil recount: cap on the tiles a thread accumulates before its packed rows are unpacked,
  *                     0 = auto (what the packed fields hold), 1..2^20
+ *   "sro_threads"     stencil recount: threads per block, 0 = auto, else a multiple of 32 in [128, 384]
  *   "sro_warps"       table recount: warps per block, 0 = auto (16), 1..16
  *   "sro_stages"      table recount: cap on the per-warp ring of 32-site table tiles in shared memory, 0 = auto, 1..8
  *   "sro_blocks_per_sm"  recount (both engines): resident blocks per SM the grid and the shared-memory split are sized for, 0 = auto, 1..4

@@ -31,7 +31,7 @@ namespace hea {
 
 namespace {
 
-constexpr int kStThreads = 256;
+constexpr int kStMaxThreads = 384;         // block size is chosen per tile shape (whole passes over the tile's words)
 constexpr int kStPY = 10;                 // frame rows per x-plane: tiles are at most 8 cells along y
 constexpr int kStMaxTx = 8;
 
@@ -133,19 +133,24 @@ __device__ __forceinline__ void stencil_site(const uint32_t* const (&bp)[4], uin
     h[0] = shell_sum<LAT, PZ, B, 0>(bp, std::make_integer_sequence<int, h0>{});
     if constexpr (S > 1) h[1] = shell_sum<LAT, PZ, B, h0>(bp, std::make_integer_sequence<int, h1>{});
     if constexpr (S > 2) h[2] = shell_sum<LAT, PZ, B, h0 + h1>(bp, std::make_integer_sequence<int, h2>{});
+    // the row select is a multiply-add by the 0/1 flag "row r is mine": IMAD runs on the FMA pipe, which is otherwise
+    // idle, instead of compare + select + add on the ALU pipe that already carries the histogram adds (ncu: ALU-bound)
+    uint32_t mine[MT];
+#pragma unroll
+    for (int r = 0; r < MT; ++r) mine[r] = (own >> PK::pos(r)) & 1u;
 #pragma unroll
     for (int s = 0; s < S; ++s)
 #pragma unroll
         for (int w = 0; w < PK::NW; ++w) {
             const uint32_t word = (h[s] >> PK::pos(w)) & PK::mask(w);
 #pragma unroll
-            for (int r = 0; r < MT; ++r) acc[s][r][w] += (own == (1u << PK::pos(r))) ? word : 0u;
+            for (int r = 0; r < MT; ++r) acc[s][r][w] += word * mine[r];
         }
 }
 
 // MT = 4 serves M <= 4, MT = 5 serves M = 5, MT = 8 serves M = 6..8 (rows and fields >= M stay zero).
 template <int MT, int LAT, int S, int PZ>
-__global__ void __launch_bounds__(kStThreads, 3)
+__global__ void __launch_bounds__(kStMaxThreads, 2)
 sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __restrict__ occ_all,
                    int32_t* __restrict__ counts_all)
 {
@@ -157,7 +162,7 @@ sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __rest
 
     extern __shared__ __align__(16) uint32_t s_w[];                   // [A][tx + 2][PY][PZ]
     __shared__ int s_bins[NB];
-    for (int i = threadIdx.x; i < NB; i += kStThreads) s_bins[i] = 0;
+    for (int i = threadIdx.x; i < NB; i += blockDim.x) s_bins[i] = 0;
 
     const int M = P.M, SMM = S * M * M;
     const int Lx = P.L[0], Ly = P.L[1], Lz = P.L[2];
@@ -188,7 +193,7 @@ sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __rest
 
         __syncthreads();                  // the previous tile has been read (first pass: the bins are zero)
         // ---- stage the tile and its halo: one padded cell (A sites) per thread and pass
-        for (int p = threadIdx.x; p < n_load; p += kStThreads) {
+        for (int p = threadIdx.x; p < n_load; p += blockDim.x) {
             const int px = (int)div_magic((uint32_t)p, Q.mg_load);
             const int r = p - px * Q.rows_load;
             const int py = r / PZ, pz = r - py * PZ;
@@ -211,7 +216,7 @@ sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __rest
         __syncthreads();
 
         // ---- lanes run over the words of the interior rows; the halo words of a row idle
-        for (int q = threadIdx.x; q < n_main; q += kStThreads) {
+        for (int q = threadIdx.x; q < n_main; q += blockDim.x) {
             const int x = (int)div_magic((uint32_t)q, Q.mg_main);
             const int r = q - x * Q.rows_main;
             const int y = r / PZ, pz = r - y * PZ;
@@ -261,10 +266,11 @@ sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __rest
                 __syncthreads();
                 // N_ij = H_ij + H_ji
                 int32_t* counts = counts_all + (size_t)cfg * SMM;
-                int v[(NB + kStThreads - 1) / kStThreads];
+                constexpr int NU = (NB + 127) / 128;                  // blocks have at least 128 threads
+                int v[NU];
 #pragma unroll
-                for (int u = 0; u < (NB + kStThreads - 1) / kStThreads; ++u) {
-                    const int k = threadIdx.x + u * kStThreads;
+                for (int u = 0; u < NU; ++u) {
+                    const int k = threadIdx.x + u * blockDim.x;
                     v[u] = 0;
                     if (k < SMM) {
                         const int s = k / (M * M), i = (k / M) % M, j = k % M;
@@ -273,45 +279,59 @@ sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __rest
                     }
                 }
                 __syncthreads();
-                for (int i = threadIdx.x; i < NB; i += kStThreads) s_bins[i] = 0;
+                for (int i = threadIdx.x; i < NB; i += blockDim.x) s_bins[i] = 0;
                 if (tile == n_tiles) { tile = 0; ++cfg; }
             }
         }
     }
 }
 
+// Grid: a contiguous range of items per block, sized for the blocks that are resident at once (occupancy query x
+// SMs, or blocks_per_sm if given), so that every block unpacks its rows as rarely as the item order allows.
 template <int MT, int LAT, int S, int PZ>
-cudaError_t launch_st_one(const KParams& P, const StencilParams& Q, const uint8_t* occ, int32_t* counts, unsigned grid,
-                          size_t smem, cudaStream_t st)
+cudaError_t launch_st_one(const KParams& P, StencilParams Q, const uint8_t* occ, int32_t* counts, int n_sms,
+                          int blocks_per_sm, int threads, size_t smem, cudaStream_t st)
 {
     auto kern = sro_stencil_kernel<MT, LAT, S, PZ>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<grid, kStThreads, smem, st>>>(P, Q, occ, counts);
+    int resident = blocks_per_sm;
+    if (resident <= 0) {
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, threads, smem);
+        if (e != cudaSuccess) return e;
+        if (resident < 1) return cudaErrorInvalidConfiguration;
+    }
+    const long long slots = (long long)n_sms * resident;
+    long long ipb = (Q.n_items + slots - 1) / slots;
+    ipb = std::max<long long>(1, std::min<long long>(ipb, 1 << 20));
+    Q.items_per_block = (int)ipb;
+    const long long grid = (Q.n_items + ipb - 1) / ipb;
+    if (grid > 0x7FFFFFFF) return cudaErrorInvalidConfiguration;
+    kern<<<(unsigned)grid, threads, smem, st>>>(P, Q, occ, counts);
     return cudaGetLastError();
 }
 
 template <int MT, int PZ>
 cudaError_t launch_st_m(const KParams& P, const StencilParams& Q, int lat, const uint8_t* occ, int32_t* counts,
-                        unsigned grid, size_t smem, cudaStream_t st)
+                        int n_sms, int blocks_per_sm, int threads, size_t smem, cudaStream_t st)
 {
     switch (lat * 3 + P.S) {
-        case 1: return launch_st_one<MT, 0, 1, PZ>(P, Q, occ, counts, grid, smem, st);
-        case 2: return launch_st_one<MT, 0, 2, PZ>(P, Q, occ, counts, grid, smem, st);
-        case 3: return launch_st_one<MT, 0, 3, PZ>(P, Q, occ, counts, grid, smem, st);
-        case 4: return launch_st_one<MT, 1, 1, PZ>(P, Q, occ, counts, grid, smem, st);
-        case 5: return launch_st_one<MT, 1, 2, PZ>(P, Q, occ, counts, grid, smem, st);
-        default: return launch_st_one<MT, 1, 3, PZ>(P, Q, occ, counts, grid, smem, st);
+        case 1: return launch_st_one<MT, 0, 1, PZ>(P, Q, occ, counts, n_sms, blocks_per_sm, threads, smem, st);
+        case 2: return launch_st_one<MT, 0, 2, PZ>(P, Q, occ, counts, n_sms, blocks_per_sm, threads, smem, st);
+        case 3: return launch_st_one<MT, 0, 3, PZ>(P, Q, occ, counts, n_sms, blocks_per_sm, threads, smem, st);
+        case 4: return launch_st_one<MT, 1, 1, PZ>(P, Q, occ, counts, n_sms, blocks_per_sm, threads, smem, st);
+        case 5: return launch_st_one<MT, 1, 2, PZ>(P, Q, occ, counts, n_sms, blocks_per_sm, threads, smem, st);
+        default: return launch_st_one<MT, 1, 3, PZ>(P, Q, occ, counts, n_sms, blocks_per_sm, threads, smem, st);
     }
 }
 
 template <int PZ>
 cudaError_t launch_st_pz(const KParams& P, const StencilParams& Q, int lat, const uint8_t* occ, int32_t* counts,
-                         unsigned grid, size_t smem, cudaStream_t st)
+                         int n_sms, int blocks_per_sm, int threads, size_t smem, cudaStream_t st)
 {
-    if (P.M <= 4) return launch_st_m<4, PZ>(P, Q, lat, occ, counts, grid, smem, st);
-    if (P.M == 5) return launch_st_m<5, PZ>(P, Q, lat, occ, counts, grid, smem, st);
-    return launch_st_m<8, PZ>(P, Q, lat, occ, counts, grid, smem, st);
+    if (P.M <= 4) return launch_st_m<4, PZ>(P, Q, lat, occ, counts, n_sms, blocks_per_sm, threads, smem, st);
+    if (P.M == 5) return launch_st_m<5, PZ>(P, Q, lat, occ, counts, n_sms, blocks_per_sm, threads, smem, st);
+    return launch_st_m<8, PZ>(P, Q, lat, occ, counts, n_sms, blocks_per_sm, threads, smem, st);
 }
 
 uint32_t magic_of(int d) { return (uint32_t)(((1ull << 31) + (uint64_t)d - 1) / (uint64_t)d); }
@@ -334,10 +354,12 @@ bool sro_stencil_usable(const Lattice& lat, const uint8_t* occ)
 }
 
 // tile_xy: cap on the tile extent along x and y, cells (0 = auto = 8, 1..8).  tile_z: row pitch variant (0 = auto: the
-// one with the best lane efficiency L / (tiles * PZ), else 12, 22 or 34).  blocks_per_sm: grid sizing (0 = auto = 3).
+// one with the best lane efficiency L / (tiles * PZ), else 12, 22 or 34).  blocks_per_sm: grid sizing (0 = auto: the occupancy query).
+// opt_threads: block size (0 = auto, else a multiple of 32 in [128, 384]).
 // flush_tiles: cap on the tiles a lane accumulates before its rows are unpacked (0 = auto: what the fields hold).
 cudaError_t launch_sro_stencil(const KParams& P, const Lattice& lat, const uint8_t* occ, int64_t B, int32_t* counts,
-                               int n_sms, int tile_xy, int tile_z, int blocks_per_sm, int flush_tiles, cudaStream_t st,
+                               int n_sms, int tile_xy, int tile_z, int blocks_per_sm, int flush_tiles, int opt_threads,
+                               cudaStream_t st,
                                int64_t* n_launches)
 {
     const int SMM = P.S * P.M * P.M;
@@ -388,24 +410,25 @@ cudaError_t launch_sro_stencil(const KParams& P, const Lattice& lat, const uint8
     Q.mg_load = magic_of(Q.rows_load);
     Q.mg_main = magic_of(Q.rows_main);
     const int n_main = Q.tx * Q.rows_main;
-    const int sites_per_lane = ((n_main + kStThreads - 1) / kStThreads) * lat.A;
+    // block size (measured on B200, profiles/r1_sweeps.md): small blocks when there are enough (configuration, tile)
+    // items to fill the chip several times over -- six 4-warp blocks per SM overlap one block's staging with the
+    // others' counting -- and larger blocks when a launch has few items, so that a tile is finished sooner.
+    const int64_t n_items_all = (int64_t)Q.ntx * Q.nty * Q.ntz * B;
+    int warps = n_items_all < n_sms ? 12 : (n_items_all < 5 * (int64_t)n_sms ? 8 : 4);
+    if (opt_threads > 0) warps = opt_threads / 32;
+    const int threads = warps * 32;
+    const int sites_per_lane = ((n_main + threads - 1) / threads) * lat.A;
     const int sites_cap = P.M <= 4 ? Pack<4>::kSitesCap : (P.M == 5 ? Pack<5>::kSitesCap : Pack<8>::kSitesCap);
     Q.cap_tiles = std::max(1, sites_cap / sites_per_lane);
     if (sites_per_lane > sites_cap) return cudaErrorInvalidConfiguration;
     if (flush_tiles > 0) Q.cap_tiles = std::min(Q.cap_tiles, flush_tiles);
     const int64_t n_tiles = (int64_t)Q.ntx * Q.nty * Q.ntz;
     Q.n_items = (long long)(n_tiles * B);
-    const int64_t slots = (int64_t)n_sms * (blocks_per_sm > 0 ? blocks_per_sm : 3);
-    int64_t ipb = (Q.n_items + slots - 1) / slots;
-    ipb = std::max<int64_t>(1, std::min<int64_t>(ipb, 1 << 20));
-    Q.items_per_block = (int)ipb;
-    const int64_t grid = (Q.n_items + ipb - 1) / ipb;
-    if (grid > 0x7FFFFFFF) return cudaErrorInvalidConfiguration;
     const size_t smem = sizeof(uint32_t) * (size_t)lat.A * Q.plane;
     switch (PZ) {
-        case 12: e = launch_st_pz<12>(P, Q, lat.type, occ, counts, (unsigned)grid, smem, st); break;
-        case 22: e = launch_st_pz<22>(P, Q, lat.type, occ, counts, (unsigned)grid, smem, st); break;
-        default: e = launch_st_pz<34>(P, Q, lat.type, occ, counts, (unsigned)grid, smem, st); break;
+        case 12: e = launch_st_pz<12>(P, Q, lat.type, occ, counts, (unsigned)n_sms, blocks_per_sm, threads, smem, st); break;
+        case 22: e = launch_st_pz<22>(P, Q, lat.type, occ, counts, (unsigned)n_sms, blocks_per_sm, threads, smem, st); break;
+        default: e = launch_st_pz<34>(P, Q, lat.type, occ, counts, (unsigned)n_sms, blocks_per_sm, threads, smem, st); break;
     }
     if (e != cudaSuccess) return e;
     ++*n_launches;
