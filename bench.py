@@ -16,8 +16,10 @@ memory, recount, MC, D2H of occupancies + counts + stats inside the timed region
 Multi-GPU: chains are independent, so rank r runs chains [16 r, 16 r + 16) with no data-path collective ("weak").
 
 `roofline` is for the dominant kernel of the step (the MC kernel; ALU-issue bound, model in DESIGN.md section 6);
-`recount_roofline` is for the recount kernel on the sweep point of configs[4] where the neighbour table exceeds L2
-(fcc 100^3 = 4,000,000 atoms, 3 shells, batch 1; HBM bound, 4*Z+1 = 169 B/atom).
+`recount_roofline` is for the table-driven recount kernel (sro_engine = 1) on the sweep point of configs[4] where the
+neighbour table exceeds L2 (fcc 100^3 = 4,000,000 atoms, 3 shells, batch 1; HBM bound, 4*Z+1 = 169 B/atom);
+`recount_stencil` is the table-free kernel `hea_sro_full` runs by default on the same point (1 B/atom of HBM traffic;
+bound by instruction issue, model in DESIGN.md section 6.1b) with its atoms/s beside the table kernel's.
 `cpu_baseline` / `--impl reference`: the CPU oracle (oracle/hea_oracle.c), as it stands, on the host cores, on a
 bounded sample (the first steps of the same trajectory).
 """
@@ -51,6 +53,7 @@ def load_peaks():
 # profiles/r1_mc_halo_c4_full.md (whole c4 trajectory, one launch) and profiles/r1_sro_count_v3.md (fcc 100^3, batch 1).
 NCU_TRAFFIC_MC_C4_FULL = 4_412_160 + 26_112
 NCU_TRAFFIC_RECOUNT_L100 = 680_663_040
+NCU_TRAFFIC_STENCIL_L100 = None                # filled from profiles/r1_sro_stencil.md
 
 
 # ALU-issue model of one swap trial: thread-instructions the method needs per candidate.
@@ -59,6 +62,19 @@ def mc_ops_per_trial(Z, S, M):
     gather = 2 * Z * 5                  # per neighbour entry: index, species load, 2 compares folded, shift, add
     objective = S * M * M * 6 + S * M + S * 2   # per cell: cvt, mul, sub, sub, mul, add; row/shell/weight combines
     return philox + gather + objective
+
+
+def stencil_ops_per_atom(Z, S, M):
+    """Thread-instructions the table-free recount needs per atom as it is formulated: Z/2 shared-memory
+    loads and Z/2 adds of the half-shell histogram, per shell and wide word one extract and M multiply-adds of the row
+    select (2 words for M <= 5, 4 above), M own-species flags."""
+    nw = 2 if M <= 5 else 4
+    return Z // 2 + Z // 2 + S * nw * (1 + M) + M
+
+
+def issue_peak(n_sms, sm_mhz):
+    """T thread-instr/s: SMs x 128 lanes/clk x clock."""
+    return n_sms * 128 * sm_mhz * 1e6 / 1e12
 
 
 class ClockSampler:
@@ -190,22 +206,29 @@ def run_sweep(args):
                 continue
             occ = hr.init_random(B, wr.seed)
             cnt = torch.empty((B, hr.S, hr.M, hr.M), dtype=torch.int32, device=dev)
-            for _ in range(2):
-                hr.sro_full(occ, counts=cnt, want_alpha=False, want_obj=False)
             reps = max(3, min(50, int(2e9 // (B * hr.N)) or 3))
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
-            e0.record()
-            for _ in range(reps):
-                hr.sro_full(occ, counts=cnt, want_alpha=False, want_obj=False)
-            e1.record()
-            torch.cuda.synchronize()
-            t = e0.elapsed_time(e1) * 1e-3 / reps
+            t_eng = {}
+            for engine in (1, 2):                      # 1 = table-driven kernel, 2 = table-free stencil kernel (default)
+                hr.set_option("sro_engine", engine)
+                for _ in range(2):
+                    hr.sro_full(occ, counts=cnt, want_alpha=False, want_obj=False)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record()
+                for _ in range(reps):
+                    hr.sro_full(occ, counts=cnt, want_alpha=False, want_obj=False)
+                e1.record()
+                torch.cuda.synchronize()
+                t_eng[engine] = e0.elapsed_time(e1) * 1e-3 / reps
+            t = t_eng[1]
             table_bytes, occ_bytes = 4 * Z * hr.N, B * hr.N
             out["recount"].append({"L": L, "atoms": hr.N, "batch": B, "us": 1e6 * t, "atoms_per_s": B * hr.N / t,
                                    "model_GBps_table_once": (table_bytes + occ_bytes) / t / 1e9,
                                    "frac_hbm_table_once": (table_bytes + occ_bytes) / t / 1e9 / hbm_peak,
-                                   "table_MB": table_bytes / 1e6})
+                                   "table_MB": table_bytes / 1e6,
+                                   "stencil_us": 1e6 * t_eng[2], "stencil_atoms_per_s": B * hr.N / t_eng[2],
+                                   "stencil_frac_issue": B * hr.N / t_eng[2] * stencil_ops_per_atom(Z, hr.S, hr.M) / 1e12
+                                   / issue_peak(148, 1965.0)})
             del occ, cnt
         hr.close()
     for C in workloads.CHAIN_SWEEP_C:
@@ -372,31 +395,48 @@ def main():
     d2h = C * N + 4 * SMM * C + 40 * C
 
     # ---- recount roofline point: table larger than L2 (inputs > L2, so no flush needed)
-    recount = None
+    recount = recount_stencil = None
     if not args.no_recount:
         wr = workloads.recount_sweep_workload(args.recount_L, 1)
         hr = binding.Hea(*wr.create_args(), device=local_rank)
         occ_r = hr.init_random(1, wr.seed)
         cnt_r = torch.empty((1, hr.S, hr.M, hr.M), dtype=torch.int32, device=dev)
-        for _ in range(3):
-            hr.sro_full(occ_r, counts=cnt_r, want_alpha=False, want_obj=False)
-        reps = 10
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        e0.record()
-        for _ in range(reps):
-            hr.sro_full(occ_r, counts=cnt_r, want_alpha=False, want_obj=False)
-        e1.record()
-        torch.cuda.synchronize()
-        t_r = e0.elapsed_time(e1) * 1e-3 / reps
+        def time_recount(engine, reps=10):
+            hr.set_option("sro_engine", engine)
+            for _ in range(3):
+                hr.sro_full(occ_r, counts=cnt_r, want_alpha=False, want_obj=False)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps):
+                hr.sro_full(occ_r, counts=cnt_r, want_alpha=False, want_obj=False)
+            e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) * 1e-3 / reps
+
+        t_r = time_recount(1)                      # table-driven kernel: the HBM-bound one
+        ref_r = cnt_r.clone()
+        t_s = time_recount(2)                      # table-free stencil kernel (what hea_sro_full runs by default)
+        assert bool((cnt_r == ref_r).all()), "recount engines disagree"
         Zr = sum(hr.z)
         bytes_r = (4 * Zr + 1) * hr.N
         recount = {"bound": "hbm", "achieved": bytes_r / t_r / 1e9, "peak": hbm_peak, "unit": "GB/s",
                    "frac": bytes_r / t_r / 1e9 / hbm_peak,
                    "traffic": NCU_TRAFFIC_RECOUNT_L100 if args.recount_L == 100 else None, "peak_source": peak_src,
-                   "kernel": "sro_count_kernel", "workload": f"fcc {args.recount_L}^3 ({hr.N} atoms), 5 species, "
+                   "kernel": "sro_count_kernel (sro_engine = 1)", "workload": f"fcc {args.recount_L}^3 ({hr.N} atoms), 5 species, "
                    f"3 shells (Z={Zr}), batch 1; table {4 * Zr * hr.N / 1e6:.0f} MB > L2",
                    "bytes_per_atom": 4 * Zr + 1, "atoms_per_s": hr.N / t_r, "ms_per_launch": t_r * 1e3}
+        ops_s = stencil_ops_per_atom(Zr, hr.S, hr.M)
+        sm_mhz_r = float(clocks.get("sm_max_mhz") or 1965.0)
+        n_sms_r = torch.cuda.get_device_properties(dev).multi_processor_count
+        recount_stencil = {"bound": "alu", "achieved": hr.N / t_s * ops_s / 1e12, "peak": issue_peak(n_sms_r, sm_mhz_r),
+                           "unit": "T thread-instr/s", "frac": hr.N / t_s * ops_s / 1e12 / issue_peak(n_sms_r, sm_mhz_r),
+                           "traffic": NCU_TRAFFIC_STENCIL_L100 if args.recount_L == 100 else None,
+                           "kernel": "sro_stencil_kernel (sro_engine = 2, the default)", "ops_per_atom": ops_s,
+                           "workload": f"fcc {args.recount_L}^3 ({hr.N} atoms), 5 species, 3 shells, batch 1; 1 byte per atom",
+                           "atoms_per_s": hr.N / t_s, "ms_per_launch": t_s * 1e3,
+                           "hbm_GBps": hr.N / t_s / 1e9, "speedup_vs_table_kernel": t_r / t_s,
+                           "peak_source": "SMs x 128 lanes/clk x max SM clock (DESIGN.md section 6)"}
         hr.close()
 
     # ---- reduce over ranks: max time
@@ -439,6 +479,7 @@ def main():
         line["config"]["workload"] = f"EXPLORATION (not the metric's workload): {w.name}, {C} chains, K={K}, N={N}"
     if recount:
         line["recount_roofline"] = recount
+        line["recount_stencil"] = recount_stencil
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(w)
