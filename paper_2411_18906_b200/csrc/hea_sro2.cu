@@ -193,25 +193,38 @@ sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __rest
 
         __syncthreads();                  // the previous tile has been read (first pass: the bins are zero)
         // ---- stage the tile and its halo: one padded cell (A sites) per thread and pass
-        for (int p = threadIdx.x; p < n_load; p += blockDim.x) {
-            const int px = (int)div_magic((uint32_t)p, Q.mg_load);
-            const int r = p - px * Q.rows_load;
-            const int py = r / PZ, pz = r - py * PZ;
-            if (pz > Q.tz + 1) continue;                              // frame words beyond the tile's rows
-            int gx = x0 + px - 1, gy = y0 + py - 1, gz = z0 + pz - 1;
-            if (gx < 0) gx += Lx;
-            while (gx >= Lx) gx -= Lx;
-            if (gy < 0) gy += Ly;
-            while (gy >= Ly) gy -= Ly;
-            if (gz < 0) gz += Lz;
-            while (gz >= Lz) gz -= Lz;
-            const int cell = (gx * Ly + gy) * Lz + gz;
-            uint32_t v;
-            if (A == 4) v = __ldg(reinterpret_cast<const uint32_t*>(occ) + cell);
-            else v = __ldg(reinterpret_cast<const uint16_t*>(occ) + cell);
-            uint32_t* dst = s_w + px * XP + r;
+        // (four cells in flight per thread: the global loads of a batch are issued before any of its stores)
+        for (int p0 = threadIdx.x; p0 < n_load; p0 += 4 * blockDim.x) {
+            uint32_t v[4];
+            int word[4];
 #pragma unroll
-            for (int b = 0; b < A; ++b) dst[b * Q.plane] = 1u << PK::pos((int)((v >> (8 * b)) & 0xFFu));
+            for (int u = 0; u < 4; ++u) {
+                const int p = p0 + u * blockDim.x;
+                word[u] = -1;
+                if (p >= n_load) continue;
+                const int px = (int)div_magic((uint32_t)p, Q.mg_load);
+                const int r = p - px * Q.rows_load;
+                const int py = r / PZ, pz = r - py * PZ;
+                if (pz > Q.tz + 1) continue;                          // frame words beyond the tile's rows
+                int gx = x0 + px - 1, gy = y0 + py - 1, gz = z0 + pz - 1;
+                if (gx < 0) gx += Lx;
+                while (gx >= Lx) gx -= Lx;
+                if (gy < 0) gy += Ly;
+                while (gy >= Ly) gy -= Ly;
+                if (gz < 0) gz += Lz;
+                while (gz >= Lz) gz -= Lz;
+                const int cell = (gx * Ly + gy) * Lz + gz;
+                if (A == 4) v[u] = __ldg(reinterpret_cast<const uint32_t*>(occ) + cell);
+                else v[u] = __ldg(reinterpret_cast<const uint16_t*>(occ) + cell);
+                word[u] = px * XP + r;
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (word[u] < 0) continue;
+                uint32_t* dst = s_w + word[u];
+#pragma unroll
+                for (int b = 0; b < A; ++b) dst[b * Q.plane] = 1u << PK::pos((int)((v[u] >> (8 * b)) & 0xFFu));
+            }
         }
         __syncthreads();
 
