@@ -205,6 +205,28 @@ def test_pair_counts_equal_python_double_loop():
     np.testing.assert_array_equal(o.pair_counts(occ), want)
 
 
+@pytest.mark.parametrize("lattice,dims,conc,S", [("fcc", (5, 4, 3), [0.2] * 5, 3), ("bcc", (4, 5, 6), [0.25] * 4, 3),
+                                                 ("fcc", (1, 1, 1), [0.5, 0.5], 3), ("bcc", (1, 2, 3), [0.5, 0.5], 3),
+                                                 ("fcc", (2, 2, 2), [0.125] * 8, 3), ("bcc", (2, 2, 2), [0.5, 0.25, 0.25], 3)])
+def test_half_shell_identity_of_the_sorted_offset_list(lattice, dims, conc, S):
+    """The fact the table-free recount kernel rests on, pinned on the oracle's table with numpy only:
+    in the D2 order entry z-1-k of a shell is the reverse of entry k (following k and then z-1-k returns to the start
+    site, on every cell size), hence the counts H over the second half of each shell give N = H + H^T, multi-edges and
+    self-neighbours of tiny cells included."""
+    o = make(lattice, dims, conc, S)
+    occ = o.init_random(2, seed=21)
+    for s in range(S):
+        tab = o.neighbor_table(s).astype(np.int64)
+        z = o.z[s]
+        for k in range(z):
+            np.testing.assert_array_equal(tab[tab[:, k], z - 1 - k], np.arange(o.N))
+        for c in range(2):
+            H = np.zeros((o.M, o.M), dtype=np.int64)
+            for k in range(z // 2, z):
+                np.add.at(H, (occ[c], occ[c][tab[:, k]]), 1)
+            np.testing.assert_array_equal(H + H.T, o.pair_counts(occ[c])[s])
+
+
 # ------------------------------------------------------------------ D8: random start
 def test_init_is_fisher_yates_with_pinned_philox():
     o = make("bcc", (3, 3, 3), [0.5, 0.5], 1)
