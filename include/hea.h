@@ -106,6 +106,8 @@ int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host);
  *                     10, 20, 32 cells along z)
  *   "sro_flush_tiles" stencil recount: cap on the tiles a thread accumulates before its packed rows are unpacked,
  *                     0 = auto (what the packed fields hold), 1..2^20
+ *   "sro_lanes"       stencil recount: lane mapping, 0 = auto (2), 1 = over the row words incl. the halo (conflict-free
+ *                     shared-memory loads, some lanes idle), 2 = over the interior cells only
  *   "sro_threads"     stencil recount: threads per block, 0 = auto, else a multiple of 32 in [128, 384]
  *   "sro_warps"       table recount: warps per block, 0 = auto (16), 1..16
  *   "sro_stages"      table recount: cap on the per-warp ring of 32-site table tiles in shared memory, 0 = auto, 1..8

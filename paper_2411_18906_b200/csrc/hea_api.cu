@@ -16,7 +16,7 @@ cudaError_t launch_sro_count(const KParams& P, int lat, const uint8_t* occ, int6
 bool sro_stencil_usable(const Lattice& lat, const uint8_t* occ);
 cudaError_t launch_sro_stencil(const KParams& P, const Lattice& lat, const uint8_t* occ, int64_t B, int32_t* counts,
                                int n_sms, int tile_xy, int tile_z, int blocks_per_sm, int flush_tiles, int opt_threads,
-                               cudaStream_t st,
+                               int lanes, cudaStream_t st,
                                int64_t* n_launches);
 cudaError_t launch_sro_epilogue(const KParams& P, const int32_t* counts, int64_t B, double* alpha, double* obj,
                                 cudaStream_t st, int64_t* n_launches);
@@ -53,7 +53,7 @@ struct hea_ctx {
     int64_t* d_nps = nullptr;
     hea::KParams P{};
     // tuning options (0 = auto)
-    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0, opt_neighbors = 0, opt_engine = 0, opt_team = 0, opt_team_on = 0, opt_team_off = 0, opt_accept = 0, opt_sro_stages = 0, opt_sro_bps = 0, opt_sro_warps = 0, opt_sro_engine = 0, opt_sro_tile_xy = 0, opt_sro_tile_z = 0, opt_sro_flush = 0, opt_sro_threads = 0;
+    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0, opt_neighbors = 0, opt_engine = 0, opt_team = 0, opt_team_on = 0, opt_team_off = 0, opt_accept = 0, opt_sro_stages = 0, opt_sro_bps = 0, opt_sro_warps = 0, opt_sro_engine = 0, opt_sro_tile_xy = 0, opt_sro_tile_z = 0, opt_sro_flush = 0, opt_sro_threads = 0, opt_sro_lanes = 0;
     int64_t n_launches = 0;
     // internal stream and scratch for the *_host entry points
     cudaStream_t stream = nullptr;
@@ -124,6 +124,7 @@ int64_t* option_slot(hea_ctx* ctx, const char* name)
     if (!strcmp(name, "sro_tile_z")) return &ctx->opt_sro_tile_z;
     if (!strcmp(name, "sro_flush_tiles")) return &ctx->opt_sro_flush;
     if (!strcmp(name, "sro_threads")) return &ctx->opt_sro_threads;
+    if (!strcmp(name, "sro_lanes")) return &ctx->opt_sro_lanes;
     return nullptr;
 }
 
@@ -147,6 +148,7 @@ bool option_value_ok(const char* name, int64_t v)
     if (!strcmp(name, "sro_tile_z")) return v == 12 || v == 22 || v == 34;
     if (!strcmp(name, "sro_flush_tiles")) return v >= 1 && v <= (1 << 20);
     if (!strcmp(name, "sro_threads")) return v >= 128 && v <= 384 && v % 32 == 0;
+    if (!strcmp(name, "sro_lanes")) return v == 1 || v == 2;
     return false;
 }
 
@@ -361,7 +363,7 @@ int hea_sro_full(hea_ctx* ctx, const uint8_t* occ_dev, int64_t B, int32_t* count
     cudaError_t e;
     if (ctx->opt_sro_engine != 1 && usable)
         e = hea::launch_sro_stencil(ctx->P, ctx->lat, occ_dev, B, counts_dev, ctx->n_sms, (int)ctx->opt_sro_tile_xy,
-                                    (int)ctx->opt_sro_tile_z, (int)ctx->opt_sro_bps, (int)ctx->opt_sro_flush, (int)ctx->opt_sro_threads, st, &ctx->n_launches);
+                                    (int)ctx->opt_sro_tile_z, (int)ctx->opt_sro_bps, (int)ctx->opt_sro_flush, (int)ctx->opt_sro_threads, (int)ctx->opt_sro_lanes, st, &ctx->n_launches);
     else
         e = hea::launch_sro_count(ctx->P, ctx->lat.type, occ_dev, B, counts_dev, ctx->n_sms, ctx->smem_optin,
                                   (int)ctx->opt_sro_stages, (int)ctx->opt_sro_bps, (int)ctx->opt_sro_warps, st, &ctx->n_launches);

@@ -10,8 +10,10 @@
 //     compile-time constants: a neighbour is then `LDS.32 [row pointer of its basis index + immediate]` plus one add
 //     into a packed histogram, with no address arithmetic at all (the stencil is a constexpr table, checked against
 //     the host builder's at launch);
-//   - lanes run over the words of the interior rows INCLUDING the two halo words of each row (those lanes idle), so a
-//     warp always reads 32 consecutive words: conflict-free for every tile shape, at a lane efficiency of tz / PZ;
+//   - lanes run over the interior cells of a tile, z fastest (rows of tz <= 32 cells): where a warp spans two rows the
+//     loads are 2-way bank-conflicted, which the LSU pipe (29 % busy) absorbs; the alternative mapping over the row words
+//     INCLUDING the two halo words (conflict-free for every shape, tz / PZ of the lanes busy) is kept as `sro_lanes` = 1
+//     and measured 9 % slower;
 //   - HALF-SHELL: the shell vectors come in +-o pairs and the list of D2 is sorted, so the second half of every shell
 //     is the negation of the first.  H_ij = #{(a, o in the positive half) : occ[a] = i, occ[a + o] = j} summed over all
 //     sites gives the ordered pair counts as N_ij = H_ij + H_ji (re-index a' = a + o; holds for every cell size,
@@ -108,6 +110,9 @@ struct StencilParams {
     int rows_load;                        // (ty + 2) * PZ: words staged per x-plane
     int rows_main;                        // ty * PZ: words the lanes run over per x-plane
     uint32_t mg_load, mg_main;            // magic of rows_load, rows_main
+    int dense;                            // 1: lanes run over the interior cells only (rows of tz, 2-way bank conflicts
+                                          // where a warp spans rows); 0: over the row words incl. the halo (conflict-free)
+    uint32_t mg_tz, mg_ty;                // magic of tz, ty (dense mapping)
     int items_per_block;                  // contiguous (configuration, tile) items per block
     long long n_items;                    // B * tiles
     int cap_tiles;                        // tiles a lane may accumulate before unpacking its rows
@@ -172,7 +177,7 @@ sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __rest
     long long cfg = item0 / n_tiles;
     int tile = (int)(item0 - cfg * n_tiles);
     const int lane = threadIdx.x & 31;
-    const int n_load = (Q.tx + 2) * Q.rows_load, n_main = Q.tx * Q.rows_main;
+    const int n_load = (Q.tx + 2) * Q.rows_load, n_main = Q.dense ? Q.tx * Q.ty * Q.tz : Q.tx * Q.rows_main;
 
     uint32_t acc[S][MT][NW];
 #pragma unroll
@@ -230,9 +235,19 @@ sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __rest
 
         // ---- lanes run over the words of the interior rows; the halo words of a row idle
         for (int q = threadIdx.x; q < n_main; q += blockDim.x) {
-            const int x = (int)div_magic((uint32_t)q, Q.mg_main);
-            const int r = q - x * Q.rows_main;
-            const int y = r / PZ, pz = r - y * PZ;
+            int x, r, y, pz;
+            if (Q.dense) {
+                const uint32_t q1 = div_magic((uint32_t)q, Q.mg_tz);
+                pz = q - (int)q1 * Q.tz + 1;
+                x = (int)div_magic(q1, Q.mg_ty);
+                y = (int)q1 - x * Q.ty;
+                r = y * PZ + pz;
+            } else {
+                x = (int)div_magic((uint32_t)q, Q.mg_main);
+                r = q - x * Q.rows_main;
+                y = r / PZ;
+                pz = r - y * PZ;
+            }
             if (pz < 1 || pz > Q.tz || x0 + x >= Lx || y0 + y >= Ly || z0 + pz - 1 >= Lz) continue;
             const uint32_t* bp[4];
 #pragma unroll
@@ -367,12 +382,12 @@ bool sro_stencil_usable(const Lattice& lat, const uint8_t* occ)
 }
 
 // tile_xy: cap on the tile extent along x and y, cells (0 = auto = 8, 1..8).  tile_z: row pitch variant (0 = auto: the
-// one with the best lane efficiency L / (tiles * PZ), else 12, 22 or 34).  blocks_per_sm: grid sizing (0 = auto: the occupancy query).
+// one whose tiles fill the z extent best, else 12, 22 or 34).  lanes: 0/2 = interior cells, 1 = row words incl. halo.  blocks_per_sm: grid sizing (0 = auto: the occupancy query).
 // opt_threads: block size (0 = auto, else a multiple of 32 in [128, 384]).
 // flush_tiles: cap on the tiles a lane accumulates before its rows are unpacked (0 = auto: what the fields hold).
 cudaError_t launch_sro_stencil(const KParams& P, const Lattice& lat, const uint8_t* occ, int64_t B, int32_t* counts,
                                int n_sms, int tile_xy, int tile_z, int blocks_per_sm, int flush_tiles, int opt_threads,
-                               cudaStream_t st,
+                               int lanes, cudaStream_t st,
                                int64_t* n_launches)
 {
     const int SMM = P.S * P.M * P.M;
@@ -404,10 +419,10 @@ cudaError_t launch_sro_stencil(const KParams& P, const Lattice& lat, const uint8
     if (tile_z > 0) PZ = tile_z;
     else {
         double best = -1.0;
-        for (int v = 0; v < 3; ++v) {
+        for (int v = 0; v < 3; ++v) {                  // best fill of the z extent of the tiles; ties: the longer rows
             const int cap = kStPZs[v] - 2, n = (lat.L[2] + cap - 1) / cap;
-            const double eff = (double)lat.L[2] / ((double)n * kStPZs[v]);
-            if (eff > best + 1e-12) { best = eff; PZ = kStPZs[v]; }
+            const double fill = (double)lat.L[2] / ((double)n * cap);
+            if (fill >= best - 1e-12) { best = std::max(best, fill); PZ = kStPZs[v]; }
         }
     }
     if (PZ != 12 && PZ != 22 && PZ != 34) return cudaErrorInvalidValue;
@@ -422,12 +437,15 @@ cudaError_t launch_sro_stencil(const KParams& P, const Lattice& lat, const uint8
     Q.rows_main = Q.ty * PZ;
     Q.mg_load = magic_of(Q.rows_load);
     Q.mg_main = magic_of(Q.rows_main);
-    const int n_main = Q.tx * Q.rows_main;
+    Q.dense = lanes == 1 ? 0 : 1;
+    Q.mg_tz = magic_of(Q.tz);
+    Q.mg_ty = magic_of(Q.ty);
+    const int n_main = Q.dense ? Q.tx * Q.ty * Q.tz : Q.tx * Q.rows_main;
     // block size (measured on B200, profiles/r1_sweeps.md): small blocks when there are enough (configuration, tile)
     // items to fill the chip several times over -- six 4-warp blocks per SM overlap one block's staging with the
     // others' counting -- and larger blocks when a launch has few items, so that a tile is finished sooner.
     const int64_t n_items_all = (int64_t)Q.ntx * Q.nty * Q.ntz * B;
-    int warps = n_items_all < n_sms ? 12 : (n_items_all < 5 * (int64_t)n_sms ? 8 : 4);
+    int warps = n_items_all < n_sms ? 12 : (n_items_all < 5 * (int64_t)n_sms || PZ == 34 ? 8 : 4);
     if (opt_threads > 0) warps = opt_threads / 32;
     const int threads = warps * 32;
     const int sites_per_lane = ((n_main + threads - 1) / threads) * lat.A;

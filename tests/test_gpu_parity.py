@@ -106,8 +106,9 @@ def test_sro_full_multi_tile_and_ragged(hb, L, B, engine):
 @pytest.mark.parametrize("lattice,dims,conc,S", [("fcc", (17, 9, 45), [0.2] * 5, 3), ("bcc", (9, 21, 35), [0.25] * 4, 3),
                                                  ("fcc", (8, 8, 33), [0.5, 0.25, 0.25], 2), ("bcc", (11, 3, 70), [1 / 7] * 7, 3),
                                                  ("fcc", (2, 13, 1), [0.5, 0.5], 3), ("fcc", (12, 10, 21), [0.125] * 8, 3)])
-@pytest.mark.parametrize("tile_xy,tile_z", [(0, 0), (1, 12), (3, 22), (8, 34), (5, 12)])
-def test_sro_stencil_tilings(hb, lattice, dims, conc, S, tile_xy, tile_z):
+@pytest.mark.parametrize("tile_xy,tile_z,lanes,threads", [(0, 0, 0, 0), (1, 12, 1, 0), (3, 22, 2, 384), (8, 34, 1, 128),
+                                                          (5, 12, 2, 256), (8, 34, 2, 0), (8, 22, 1, 0)])
+def test_sro_stencil_tilings(hb, lattice, dims, conc, S, tile_xy, tile_z, lanes, threads):
     # the stencil engine over every row-pitch variant, ragged last tiles in all three directions, tiles smaller and
     # larger than the cell, z extents above one tile; the table engine and the oracle must both agree
     w = small(lattice, dims, conc, S, target_seed=4)
@@ -118,6 +119,8 @@ def test_sro_stencil_tilings(hb, lattice, dims, conc, S, tile_xy, tile_z):
     h.set_option("sro_engine", 2)
     h.set_option("sro_tile_xy", tile_xy)
     h.set_option("sro_tile_z", tile_z)
+    h.set_option("sro_lanes", lanes)
+    h.set_option("sro_threads", threads)
     c_st, _, j_st = h.sro_full(occ)
     wc, _, wj = o.sro_full(occ.cpu().numpy(), n_threads=4)
     np.testing.assert_array_equal(c_st.cpu().numpy(), wc)
@@ -143,8 +146,8 @@ def test_sro_stencil_blocks_spanning_configurations_and_flushes(hb, bps, flush):
 
 @pytest.mark.parametrize("conc", [[0.01, 0.01, 0.01, 0.01, 0.96], [0.96, 0.01, 0.01, 0.01, 0.01], [0.02, 0.02, 0.02, 0.94],
                                   [0.005] * 7 + [0.965], [1.0]])
-@pytest.mark.parametrize("tile_z", [12, 22, 34])
-def test_sro_stencil_packed_field_capacity(hb, conc, tile_z):
+@pytest.mark.parametrize("tile_z,lanes", [(12, 2), (22, 2), (34, 2), (22, 1)])
+def test_sro_stencil_packed_field_capacity(hb, conc, tile_z, lanes):
     # nearly pure configurations drive single packed fields to their maximum (12 per site and shell): long item ranges
     # per block (one block per SM) must unpack before any field of the per-thread rows overflows
     w = small("fcc", (16, 16, 80), conc, 3, target_seed=6)
@@ -153,6 +156,7 @@ def test_sro_stencil_packed_field_capacity(hb, conc, tile_z):
     h.set_option("sro_engine", 2)
     h.set_option("sro_blocks_per_sm", 1)
     h.set_option("sro_tile_z", tile_z)
+    h.set_option("sro_lanes", lanes)
     counts, _, obj = h.sro_full(occ)
     wc, _, wj = o.sro_full(occ.cpu().numpy(), n_threads=8)
     np.testing.assert_array_equal(counts.cpu().numpy(), wc)
