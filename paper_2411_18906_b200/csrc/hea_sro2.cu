@@ -95,6 +95,11 @@ struct Pack {
     static constexpr int kMinFieldBits = MT == 5 ? 10 : 16;
     static constexpr int kSitesCap = ((1 << kMinFieldBits) - 1) / 12;   // sites a lane may add before its rows are unpacked
     __host__ __device__ static constexpr int pos(int r) { return MT == 5 ? 5 * r + (r >> 1) : FB * r; }
+    // pos() of four species bytes at once (species < 8: no carries between the bytes)
+    __device__ __forceinline__ static uint32_t pos4(uint32_t v)
+    {
+        return MT == 5 ? v * 5u + ((v >> 1) & 0x7F7F7F7Fu) : v * (uint32_t)FB;
+    }
     __host__ __device__ static constexpr uint32_t mask(int w)
     {
         uint32_t m = 0;
@@ -198,37 +203,46 @@ sro_stencil_kernel(const KParams P, const StencilParams Q, const uint8_t* __rest
 
         __syncthreads();                  // the previous tile has been read (first pass: the bins are zero)
         // ---- stage the tile and its halo: one padded cell (A sites) per thread and pass
-        // (four cells in flight per thread: the global loads of a batch are issued before any of its stores)
+        // (four cells in flight per thread: the global loads of a batch are issued before any of its stores; branch-free:
+        // one conditional add / subtract wraps a coordinate because -1 <= g <= tiles * extent <= 2 L - 1)
+        const uint32_t s_w_addr = (uint32_t)__cvta_generic_to_shared(s_w);
+        const uint32_t plane_bytes = 4u * (uint32_t)Q.plane;
         for (int p0 = threadIdx.x; p0 < n_load; p0 += 4 * blockDim.x) {
             uint32_t v[4];
             int word[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int p = p0 + u * blockDim.x;
-                word[u] = -1;
-                if (p >= n_load) continue;
+                const int pu = p0 + u * blockDim.x;
+                const bool in = pu < n_load;
+                const int p = in ? pu : 0;
                 const int px = (int)div_magic((uint32_t)p, Q.mg_load);
                 const int r = p - px * Q.rows_load;
                 const int py = r / PZ, pz = r - py * PZ;
-                if (pz > Q.tz + 1) continue;                          // frame words beyond the tile's rows
+                const bool use = in && pz <= Q.tz + 1;                // frame words beyond the tile's rows are not staged
                 int gx = x0 + px - 1, gy = y0 + py - 1, gz = z0 + pz - 1;
-                if (gx < 0) gx += Lx;
-                while (gx >= Lx) gx -= Lx;
-                if (gy < 0) gy += Ly;
-                while (gy >= Ly) gy -= Ly;
-                if (gz < 0) gz += Lz;
-                while (gz >= Lz) gz -= Lz;
+                gx += gx < 0 ? Lx : 0;
+                gx -= gx >= Lx ? Lx : 0;
+                gy += gy < 0 ? Ly : 0;
+                gy -= gy >= Ly ? Ly : 0;
+                gz += gz < 0 ? Lz : 0;
+                gz -= gz >= Lz ? Lz : 0;
                 const int cell = (gx * Ly + gy) * Lz + gz;
-                if (A == 4) v[u] = __ldg(reinterpret_cast<const uint32_t*>(occ) + cell);
-                else v[u] = __ldg(reinterpret_cast<const uint16_t*>(occ) + cell);
-                word[u] = px * XP + r;
+                v[u] = 0;
+                if (use) {
+                    if (A == 4) v[u] = __ldg(reinterpret_cast<const uint32_t*>(occ) + cell);
+                    else v[u] = __ldg(reinterpret_cast<const uint16_t*>(occ) + cell);
+                }
+                word[u] = use ? px * XP + r : -1;
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                if (word[u] < 0) continue;
-                uint32_t* dst = s_w + word[u];
+                const uint32_t p4 = PK::pos4(v[u]);                   // the bit positions of the cell's A species, bytewise
+                const uint32_t dst = s_w_addr + 4u * (uint32_t)word[u];
 #pragma unroll
-                for (int b = 0; b < A; ++b) dst[b * Q.plane] = 1u << PK::pos((int)((v[u] >> (8 * b)) & 0xFFu));
+                for (int b = 0; b < A; ++b) {
+                    const uint32_t one = 1u << ((p4 >> (8 * b)) & 0xFFu);
+                    if (word[u] >= 0) asm volatile("st.shared.u32 [%0], %1;" ::"r"(dst + (uint32_t)b * plane_bytes), "r"(one) : "memory");
+                }
             }
         }
         __syncthreads();
