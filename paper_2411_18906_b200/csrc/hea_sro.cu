@@ -270,12 +270,35 @@ init_random_kernel(const KParams P, uint8_t* __restrict__ occ_all, uint64_t seed
             s_j[i] = __umulhi(r.x, n + 1u);
         }
         __syncthreads();
-        if (threadIdx.x == 0) {
-            for (int i = 0; i <= hi - lo; ++i) {
+        // The swaps are a serial chain, but 32 consecutive ones commute when they touch disjoint sites: all j distinct and
+        // no j inside the group's own range of n (other than j = n, a no-op).  Warp 0 applies such a group with one swap
+        // per lane (32 random accesses in flight instead of one); a group with a collision is applied in order by lane 0.
+        // Collisions are likely only while n is small (~1500 / n per group).  Same result as the serial order, bit for bit.
+        if (threadIdx.x < 32) {
+            const int lane = threadIdx.x;
+            const int cnt = hi - lo + 1;
+            for (int i0 = 0; i0 < cnt; i0 += 32) {
+                const int i = i0 + lane;
+                const bool have = i < cnt;
                 const int n = hi - i;
-                const uint32_t j = s_j[i];
-                const uint8_t a = o[n], b = o[j];
-                o[n] = b; o[j] = a;
+                const uint32_t j = have ? s_j[i] : 0xFFFFFFFFu - (uint32_t)lane;     // idle lanes: distinct dummies
+                const int n_lo = hi - min(i0 + 31, cnt - 1);                             // the group covers n_lo .. hi - i0
+                const uint32_t same_j = __match_any_sync(0xFFFFFFFFu, j);              // every lane takes part
+                const bool clash = have && (same_j != (1u << lane) || (j >= (uint32_t)n_lo && j != (uint32_t)n));
+                if (!__any_sync(0xFFFFFFFFu, clash)) {
+                    if (have) {
+                        const uint8_t a = o[n], b = o[j];
+                        o[n] = b; o[j] = a;
+                    }
+                } else if (lane == 0) {
+                    for (int k = i0; k < min(i0 + 32, cnt); ++k) {
+                        const int nn = hi - k;
+                        const uint32_t jj = s_j[k];
+                        const uint8_t a = o[nn], b = o[jj];
+                        o[nn] = b; o[jj] = a;
+                    }
+                }
+                __syncwarp();
             }
         }
         __syncthreads();

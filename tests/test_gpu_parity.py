@@ -70,6 +70,17 @@ def test_init_and_sro_full_bit_exact(hb, lattice, dims, conc, S, engine):
     np.testing.assert_array_equal(obj.cpu().numpy(), wj)
 
 
+@pytest.mark.parametrize("lattice,dims,conc", [("fcc", (40, 40, 40), [0.25] * 4), ("bcc", (30, 20, 25), [0.2] * 5),
+                                               ("fcc", (37, 41, 43), [0.4, 0.4, 0.1, 0.1]), ("bcc", (3, 2, 2), [0.5, 0.5])])
+def test_init_random_large_cells_bit_exact(hb, lattice, dims, conc):
+    # D8 at sizes where the kernel applies groups of 32 commuting swaps in parallel (shared-memory and global-memory
+    # configurations): the occupancies must equal the oracle's serial Fisher-Yates byte for byte
+    w = small(lattice, dims, conc, 2)
+    h, o = pair(hb, w)
+    occ = h.init_random(3, seed=77, chain0=5)
+    np.testing.assert_array_equal(occ.cpu().numpy(), o.init_random(3, seed=77, chain0=5))
+
+
 @pytest.mark.parametrize("engine", SRO_ENGINES)
 def test_sro_full_ordered_structures(hb, engine):
     # B2 on bcc: closed form alpha (+1/-1), through the GPU path
