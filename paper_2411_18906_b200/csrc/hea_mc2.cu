@@ -222,7 +222,10 @@ __device__ __forceinline__ typename Pack<M>::W pack_F(const int (&F)[M])
 //         leader writes the state back, posts a phase record, and the followers reload and join.
 constexpr int kMaxTeam = 32;
 constexpr int kHaloThreads = 512;            // block size cap: 128 registers per thread, no spills in the hot paths
-constexpr int kTeamRounds = 32;             // candidates per thread per TEAM window (the null mask has 64 bits)
+constexpr int kTeamRounds = 128;            // candidates per thread per window: longer windows amortise the imbalance between
+                                            // warps and blocks at the window barrier (c4 reject regime, trials/s: 32 rounds 3.9e10,
+                                            // 64 4.1e10, 128 4.25e10, 256 4.15e10 -- two more mask registers cost more than they save)
+constexpr int kNullWords = kTeamRounds / 64; // 64-bit words of the per-thread null mask
 
 struct TeamSlot {                 // 64 bytes
     uint32_t seq;                 // team-window number + 1 when the record below is valid
@@ -900,7 +903,9 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             uint32_t win_key = kNoKey, win_a = 0, win_b = 0, win_pq = 0;
             PW win_d0 = 0, win_d1 = 0, win_d2 = 0;
             double win_J = 0.0;
-            uint64_t nullmask = 0;
+            uint64_t nullmask[kNullWords];                          // bit j = this thread's j-th candidate of the window is null
+#pragma unroll
+            for (int wd = 0; wd < kNullWords; ++wd) nullmask[wd] = 0;
 
             // ---- long windows run in two stages: an integer pre-filter on the first shell (a candidate can only
             // improve if w_1 e_ij(N_ij + dN_ij) < J_cur for every cell, i.e. dN_ij inside a precomputed interval),
@@ -985,7 +990,8 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 SiteC sa, sb;
                 propose(t0 + ts, k, a, b, sa, sb, hp, hq);
                 if (hp == hq) {
-                    nullmask |= 1ull << j;
+#pragma unroll
+                    for (int wd = 0; wd < kNullWords; ++wd) nullmask[wd] |= (j >> 6) == wd ? 1ull << (j & 63) : 0ull;
                 } else if (best_mode || key < hint) {               // same step, higher k than a known move: only nullness counts
                     const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
                     int c[M], F0[M];
@@ -1117,10 +1123,15 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
 
             // ---- commit: null counts of the committed steps, then the move (D9.4)
             steps_done = key_best != kNoKey ? (key_best >> 10) + 1u : Wc;
-            if (nullmask) {
+            {
                 const uint32_t lim = steps_done * (uint32_t)K;       // candidates c < lim are committed
                 const uint32_t n_comm = gtid < lim ? (lim - 1u - gtid) / GT + 1u : 0u;
-                my_null += __popcll(n_comm >= 64u ? nullmask : (nullmask & ((1ull << n_comm) - 1ull)));
+#pragma unroll
+                for (int wd = 0; wd < kNullWords; ++wd) {
+                    const uint32_t lo = 64u * (uint32_t)wd;
+                    if (n_comm > lo)
+                        my_null += __popcll(n_comm >= lo + 64u ? nullmask[wd] : (nullmask[wd] & ((1ull << (n_comm - lo)) - 1ull)));
+                }
             }
             if (key_best != kNoKey) {
                 apply_move(mv, key_best & 1023u, t0 + (key_best >> 10));
