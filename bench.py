@@ -51,7 +51,7 @@ def load_peaks():
 
 # DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed `ncu --set full` captures:
 # profiles/r1_mc_halo_c4_full.md (whole c4 trajectory, one launch) and profiles/r1_sro_count_v3.md (fcc 100^3, batch 1).
-NCU_TRAFFIC_MC_C4_FULL = 4_412_160 + 26_112
+NCU_TRAFFIC_MC_C4_FULL = 7_350_016 + 49_664
 NCU_TRAFFIC_RECOUNT_L100 = 680_663_040
 NCU_TRAFFIC_STENCIL_L100 = 4_030_464           # dram bytes read + written per launch, profiles/r1_sro_stencil.md
 

@@ -1135,7 +1135,8 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             }
             if (key_best != kNoKey) {
                 apply_move(mv, key_best & 1023u, t0 + (key_best >> 10));
-                W = min(steps_done, w_cap);                         // the observed gap
+                W = min(steps_done, w_cap);                         // the observed gap (a quarter of the gap between moves
+                                                                    // was tried: no gain on c4, 3-6 % slower on the chain sweep)
                 depth = 0;
             } else {
                 W = min(W * 2u, w_cap);
