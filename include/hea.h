@@ -130,6 +130,9 @@ int hea_init_random(hea_ctx* ctx, uint8_t* occ_dev, int64_t C, uint64_t seed, ui
  *   alpha[s][i][j]  = 1 - counts * g,  g = N / (z_s N_i N_j)                       (optional, may be NULL)
  *   obj[b]          = J = sum_s w_s sum_i sum_j (alpha - alpha_target)^2           (optional, may be NULL)
  * evaluated in fp64 in the fixed order of D6 (no FMA contraction).  counts_dev is overwritten.
+ * Two device engines give the same integers ("sro_engine"): the table-free stencil kernel (default; 1 byte of HBM traffic
+ * per atom; needs occ_dev aligned to the basis size, 4 for fcc, 2 for bcc) and the table-driven kernel (4 Z + 1 bytes per
+ * atom, HBM-bound; taken automatically for unaligned occ_dev).  Asynchronous on cuda_stream.
  */
 int hea_sro_full(hea_ctx* ctx, const uint8_t* occ_dev, int64_t B,
                  int32_t* counts_dev, double* alpha_dev, double* obj_dev, void* cuda_stream);
