@@ -335,13 +335,31 @@ cudaError_t launch_st_one(const KParams& P, StencilParams Q, const uint8_t* occ,
                           int blocks_per_sm, int threads, size_t smem, cudaStream_t st)
 {
     auto kern = sro_stencil_kernel<MT, LAT, S, PZ>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    // the shared-memory opt-in and the occupancy query are remembered per device for this instantiation (small launches
+    // are latency-bound and would pay the two driver calls every time).  The opt-in only ever grows, so concurrent callers
+    // can at worst repeat a call.
+    constexpr int kDevs = 16;
+    static size_t s_optin[kDevs] = {0};
+    static int s_threads[kDevs] = {0}, s_resident[kDevs] = {0};
+    static size_t s_smem[kDevs] = {0};
+    cudaError_t e = cudaSuccess;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const bool cached = dev >= 0 && dev < kDevs;
+    if (!cached || smem > s_optin[dev]) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        if (cached) s_optin[dev] = smem;
+    }
     int resident = blocks_per_sm;
     if (resident <= 0) {
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, threads, smem);
-        if (e != cudaSuccess) return e;
-        if (resident < 1) return cudaErrorInvalidConfiguration;
+        if (cached && s_threads[dev] == threads && s_smem[dev] == smem) resident = s_resident[dev];
+        else {
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, threads, smem);
+            if (e != cudaSuccess) return e;
+            if (resident < 1) return cudaErrorInvalidConfiguration;
+            if (cached) { s_resident[dev] = resident; s_smem[dev] = smem; s_threads[dev] = threads; }
+        }
     }
     const long long slots = (long long)n_sms * resident;
     long long ipb = (Q.n_items + slots - 1) / slots;
