@@ -9,7 +9,10 @@
  *                     P:256-262) and J = F^2 = sum_k w_k sum_ij (alpha - alpha_target)^2 (Eq. 3)  (D4-D6)
  *   hea_mc_run        chain-parallel Monte Carlo local search (Alg. 3): per step K candidate swaps, each
  *                     evaluated by the incremental pair-count update (Eq. 4; Eq. 5), the
- *                     lowest-index improving candidate applied (D9; Eq. 6 P:313 is the "best-of-K" variant, not built)
+ *                     lowest-index improving candidate applied (D9)
+ *   hea_mc_run_ex     the same with the paper's own selection and termination: best-of-K (Eq. 6) and the
+ *                     search-depth counter (Alg. 3)  (A23)
+ *   hea_pool_select   selection step of the global search (Alg. 1)  (A24)
  *
  * Conventions for every call
  *   - All functions return HEA_OK (0) or an error code; hea_last_error() gives a thread-local message.
@@ -25,6 +28,14 @@
  *     offsets in lexicographic order, periodic; tiny cells keep exactly z_s table entries (multi-edge semantics).
  *   - Empty batches (B == 0 / C == 0) return HEA_OK without touching the buffers (their pointers may be NULL).
  *   - There is no CPU fallback: without a CUDA device every compute call returns HEA_ECUDA.
+ *   - One context serves ONE stream and ONE host thread at a time: the context owns scratch buffers (team control
+ *     blocks of hea_mc_run, the pool buffers of hea_pool_select, the staging buffers of the *_host calls) that are
+ *     reused by every call.  Calls on the same stream are ordered and safe; before using a context from another stream
+ *     or thread, or before a *_host call that follows asynchronous calls, synchronise the previous stream.  Use one
+ *     context per stream for concurrent work (contexts share nothing).
+ *   - Limits checked by hea_create: n_species in [1, 8], n_shells in [1, 3], every L >= 1, N < 2^31 and
+ *     max_s(z_s) * N < 2^31 (the ordered pair counts are int32), finite shell weights and targets.  Negative shell
+ *     weights are accepted (J may then be negative; lower-bound pruning and the reduced-precision filter switch off).
  */
 #ifndef HEA_H
 #define HEA_H

@@ -1,6 +1,8 @@
 // hea_api.cu -- the C ABI of libhea_b200 (include/hea.h): context, validation, launches.  No torch types.
 #include "../../include/hea.h"
 
+#include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -21,7 +23,7 @@ cudaError_t launch_sro_stencil(const KParams& P, const Lattice& lat, const uint8
 cudaError_t launch_sro_epilogue(const KParams& P, const int32_t* counts, int64_t B, double* alpha, double* obj,
                                 cudaStream_t st, int64_t* n_launches);
 cudaError_t launch_init_random(const KParams& P, uint8_t* occ, int64_t C, uint64_t seed, uint64_t chain0,
-                               const int64_t* n_per_species_dev, cudaStream_t st, int64_t* n_launches);
+                               const int64_t* n_per_species_dev, size_t smem_budget, cudaStream_t st, int64_t* n_launches);
 cudaError_t launch_stats_reset(void* stats, int64_t C, cudaStream_t st, int64_t* n_launches);
 size_t mc_shared_bytes(int occ_mode, int N, int AZ, bool fast_nbr);
 cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode, int threads, int cluster, int w_max,
@@ -181,6 +183,19 @@ int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz, int n_species
     if (!ctx) return fail(HEA_ENOMEM, "out of host memory");
     std::string err = hea::lattice_init(ctx->lat, lattice, Lx, Ly, Lz, n_shells);
     if (!err.empty()) { delete ctx; return fail(HEA_EINVAL, err); }
+    {
+        // the ordered pair counts (and the packed accumulators of the recount kernels) are int32: N_ij^s <= z_s * N
+        int z_max = 0;
+        for (int s = 0; s < n_shells; ++s) z_max = std::max(z_max, ctx->lat.z[s]);
+        if ((int64_t)z_max * ctx->lat.N >= (1ll << 31)) {
+            delete ctx;
+            return fail(HEA_EUNSUPPORTED, "max_s(z_s) * N must be < 2^31 (pair counts are int32)");
+        }
+    }
+    for (int s = 0; s < n_shells; ++s)
+        if (!std::isfinite(shell_w[s])) { delete ctx; return fail(HEA_EINVAL, "shell weights must be finite"); }
+    for (int i = 0; i < n_shells * n_species * n_species; ++i)
+        if (!std::isfinite(alpha_target[i])) { delete ctx; return fail(HEA_EINVAL, "alpha_target must be finite"); }
     ctx->M = n_species;
     ctx->S = n_shells;
     err = hea::species_counts(ctx->lat.N, n_species, conc, ctx->n_per_species);
@@ -343,7 +358,7 @@ int hea_init_random(hea_ctx* ctx, uint8_t* occ_dev, int64_t C, uint64_t seed, ui
     if (C == 0) return HEA_OK;
     if (!occ_dev) return fail(HEA_EINVAL, "occ_dev is NULL");
     DeviceGuard guard(ctx->device);
-    cudaError_t e = hea::launch_init_random(ctx->P, occ_dev, C, seed, chain0, ctx->d_nps, (cudaStream_t)cuda_stream,
+    cudaError_t e = hea::launch_init_random(ctx->P, occ_dev, C, seed, chain0, ctx->d_nps, ctx->smem_optin, (cudaStream_t)cuda_stream,
                                             &ctx->n_launches);
     return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_init_random launch");
 }

@@ -2,6 +2,7 @@
 // Product code (sm_100a); shares nothing with oracle/.
 #pragma once
 #include <cstdint>
+#include <cstring>
 #include <cuda_runtime.h>
 
 namespace hea {
@@ -54,6 +55,19 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 __device__ __forceinline__ double i2d_exact(int n)
 {
     return __dsub_rn(__hiloint2double(0x43300000, (int)((unsigned)n ^ 0x80000000u)), 4503601774854144.0);
+}
+
+// Order-preserving map of a double onto unsigned 64-bit integers (x < y  <=>  key(x) < key(y), also for negative values:
+// J can be negative when a shell weight is).  -0.0 sorts below +0.0; J is a sum started from +0.0 and never is -0.0.
+__host__ __device__ __forceinline__ unsigned long long ordered_bits(double x)
+{
+#ifdef __CUDA_ARCH__
+    const unsigned long long b = (unsigned long long)__double_as_longlong(x);
+#else
+    unsigned long long b;
+    memcpy(&b, &x, sizeof b);
+#endif
+    return b ^ ((b >> 63) ? ~0ull : (1ull << 63));
 }
 
 // D6: one squared deviation, every operation individually rounded (no FMA contraction).

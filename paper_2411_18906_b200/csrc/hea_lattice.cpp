@@ -137,27 +137,31 @@ void build_shell_table(const Lattice& lat, int shell, int32_t* out)
 
 std::string species_counts(int64_t N, int M, const double* conc, int64_t* out)
 {
-    double sum = 0.0;
+    // D3, written as a ranking: every species first gets the integer part of c_i N (or c_i N itself when that is an
+    // integer to 1e-9); the atoms still missing go, one each, to the species ranked by remainder, largest first,
+    // equal remainders in index order (a stable sort keeps the index order).
+    struct Share { int species; double remainder; };
+    std::vector<Share> rank;
+    double conc_sum = 0.0;
+    int64_t placed = 0;
     for (int i = 0; i < M; ++i) {
         if (!(conc[i] > 0.0)) return "concentrations must be > 0";
-        sum += conc[i];
+        conc_sum += conc[i];
+        const double want = conc[i] * (double)N;
+        const double whole = std::nearbyint(want);
+        if (std::fabs(want - whole) <= 1e-9) {
+            out[i] = (int64_t)whole;
+        } else {
+            out[i] = (int64_t)std::floor(want);
+            rank.push_back({i, want - std::floor(want)});
+        }
+        placed += out[i];
     }
-    if (std::fabs(sum - 1.0) > 1e-9) return "concentrations must sum to 1 (within 1e-9)";
-    std::vector<double> frac(M);
-    int64_t total = 0;
-    for (int i = 0; i < M; ++i) {
-        const double x = conc[i] * (double)N;
-        const double nearest = std::floor(x + 0.5);
-        if (std::fabs(x - nearest) <= 1e-9) { out[i] = (int64_t)nearest; frac[i] = 0.0; }
-        else { out[i] = (int64_t)std::floor(x); frac[i] = x - std::floor(x); }
-        total += out[i];
-    }
-    while (total < N) {   // hand out the missing atoms by largest remainder, lower index first on ties
-        int pick = 0;
-        for (int i = 1; i < M; ++i) if (frac[i] > frac[pick]) pick = i;
-        ++out[pick]; frac[pick] = -1.0; ++total;
-    }
-    if (total != N) return "species counts do not add up to N";
+    if (std::fabs(conc_sum - 1.0) > 1e-9) return "concentrations must sum to 1 (within 1e-9)";
+    const int64_t missing = N - placed;
+    if (missing < 0 || missing > (int64_t)rank.size()) return "species counts do not add up to N";
+    std::stable_sort(rank.begin(), rank.end(), [](const Share& a, const Share& b) { return a.remainder > b.remainder; });
+    for (int64_t r = 0; r < missing; ++r) ++out[rank[(size_t)r].species];
     for (int i = 0; i < M; ++i) if (out[i] <= 0) return "a species would get zero atoms";
     return "";
 }

@@ -85,7 +85,7 @@ struct Sh2 {
     float fwg[64];                //                          w_1 g_ij^2
     uint32_t q_n[3];              // queue fill, triple-buffered like best[]
     uint32_t bestk;               // best-of-K: lowest key among the minimum-J candidates of the deciding step
-    unsigned long long bestJ;     // best-of-K: minimum J (as ordered bits) among the candidates of the deciding step
+    unsigned long long bestJ;     // best-of-K: minimum J (ordered_bits key) among the candidates of the deciding step
     uint32_t queue[kQueueCap];    // keys of the candidates that passed the pre-filter
 };
 
@@ -1059,9 +1059,9 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 // best-of-K: among this block's improving candidates of the deciding step, the minimum J, then the
                 // lowest k (bestJ / bestk are reset by apply_move, which always follows)
                 const bool mine = win_key != kNoKey && (win_key >> 10) == (key_best >> 10);
-                if (mine) atomicMin(&sh.bestJ, (unsigned long long)__double_as_longlong(win_J));
+                if (mine) atomicMin(&sh.bestJ, ordered_bits(win_J));
                 __syncthreads();
-                if (mine && (unsigned long long)__double_as_longlong(win_J) == sh.bestJ) atomicMin(&sh.bestk, win_key);
+                if (mine && ordered_bits(win_J) == sh.bestJ) atomicMin(&sh.bestk, win_key);
                 __syncthreads();
                 key_best = sh.bestk;
             }
@@ -1085,7 +1085,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     if (lane < R) {
                         while (ld_acquire_u32(&slots[lane].seq) != tw + 1u) { }
                         kk = __ldcg(&slots[lane].key);
-                        if (best_mode) jb = (unsigned long long)__double_as_longlong(__ldcg(&slots[lane].J));
+                        if (best_mode) jb = ordered_bits(__ldcg(&slots[lane].J));
                     }
                     // minimum over the team: by key, or in best-of-K mode by (step, J, k)
                     const uint32_t ka = best_mode ? (kk == kNoKey ? kNoKey : kk >> 10) : kk;

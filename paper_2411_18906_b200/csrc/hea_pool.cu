@@ -3,20 +3,23 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+#include "hea_device.cuh"
+
 namespace hea {
 
 namespace {
 
-// order[r] = index of the chain of rank r (J ascending, ties -> lower index), for r < n_keep.  J >= 0, so its bit
-// pattern orders like the value.  One thread per chain, O(C^2) compares over an L2-resident array: C <= 65,536.
+// order[r] = index of the chain of rank r (J ascending, ties -> lower index), for r < n_keep.  J is compared through the
+// order-preserving integer key of hea_device.cuh (negative J, possible with a negative shell weight, included).
+// One thread per chain, O(C^2) compares over an L2-resident array: C <= 65,536.
 __global__ void pool_rank_kernel(const double* __restrict__ J, int64_t C, int64_t n_keep, int32_t* __restrict__ order)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= C) return;
-    const unsigned long long mine = (unsigned long long)__double_as_longlong(J[c]);
+    const unsigned long long mine = ordered_bits(J[c]);
     int64_t rank = 0;
     for (int64_t o = 0; o < C; ++o) {
-        const unsigned long long other = (unsigned long long)__double_as_longlong(__ldg(J + o));
+        const unsigned long long other = ordered_bits(__ldg(J + o));
         rank += (other < mine) || (other == mine && o < c);
     }
     if (rank < n_keep) order[rank] = (int32_t)c;

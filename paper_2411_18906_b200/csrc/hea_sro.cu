@@ -234,7 +234,8 @@ __global__ void sro_epilogue_kernel(const KParams P, const int32_t* __restrict__
 
 // ---------------------------------------------------------------- D8: seeded Fisher-Yates
 // One block per chain.  The Philox draws are independent and are produced by all threads in chunks; the swaps are a
-// serial dependency chain and are applied by one thread (shared memory when the configuration fits, else global).
+// serial dependency chain, applied by warp 0 in groups of 32 that touch disjoint sites (one swap per lane; a group with
+// a collision is applied in order by lane 0) -- in shared memory when the configuration fits, else in global memory.
 constexpr int kInitThreads = 256;
 constexpr int kInitChunk = 2048;
 
@@ -405,21 +406,25 @@ cudaError_t launch_sro_epilogue(const KParams& P, const int32_t* counts, int64_t
 }
 
 cudaError_t launch_init_random(const KParams& P, uint8_t* occ, int64_t C, uint64_t seed, uint64_t chain0,
-                               const int64_t* n_per_species_dev, cudaStream_t st, int64_t* n_launches)
+                               const int64_t* n_per_species_dev, size_t smem_budget, cudaStream_t st, int64_t* n_launches)
 {
     const size_t base = kInitChunk * sizeof(uint32_t);
-    const bool in_smem = (size_t)P.N + base <= 200 * 1024;
-    cudaError_t e;
+    const bool in_smem = (size_t)P.N + base <= smem_budget;      // the device's opt-in shared memory per block
+    cudaError_t e = cudaSuccess;
     if (in_smem) {
-        const size_t smem = base + (size_t)P.N;
-        e = cudaFuncSetAttribute(init_random_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(init_random_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(base + (size_t)P.N));
         if (e != cudaSuccess) return e;
-        init_random_kernel<true><<<(unsigned)C, kInitThreads, smem, st>>>(P, occ, seed, chain0, n_per_species_dev);
-    } else {
-        init_random_kernel<false><<<(unsigned)C, kInitThreads, base, st>>>(P, occ, seed, chain0, n_per_species_dev);
     }
-    ++*n_launches;
-    return cudaGetLastError();
+    const int64_t kMaxGrid = 0x7FFFFFFF;                          // gridDim.x limit: more chains go in several launches
+    for (int64_t c0 = 0; c0 < C; c0 += kMaxGrid) {
+        const unsigned grid = (unsigned)std::min<int64_t>(kMaxGrid, C - c0);
+        uint8_t* o = occ + (size_t)c0 * (size_t)P.N;
+        if (in_smem) init_random_kernel<true><<<grid, kInitThreads, base + (size_t)P.N, st>>>(P, o, seed, chain0 + (uint64_t)c0, n_per_species_dev);
+        else init_random_kernel<false><<<grid, kInitThreads, base, st>>>(P, o, seed, chain0 + (uint64_t)c0, n_per_species_dev);
+        ++*n_launches;
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
+    return e;
 }
 
 cudaError_t launch_stats_reset(void* stats, int64_t C, cudaStream_t st, int64_t* n_launches)

@@ -24,6 +24,7 @@
 //     atomicAdd per bin with the transpose folded in.
 // Integer adds commute: bit-exact with the table kernel and the oracle whatever the tiling.
 #include <algorithm>
+#include <atomic>
 #include <utility>
 
 #include "hea_device.cuh"
@@ -336,29 +337,31 @@ cudaError_t launch_st_one(const KParams& P, StencilParams Q, const uint8_t* occ,
 {
     auto kern = sro_stencil_kernel<MT, LAT, S, PZ>;
     // the shared-memory opt-in and the occupancy query are remembered per device for this instantiation (small launches
-    // are latency-bound and would pay the two driver calls every time).  The opt-in only ever grows, so concurrent callers
-    // can at worst repeat a call.
+    // are latency-bound and would pay the two driver calls every time).  Each cache entry is ONE atomic word, so
+    // concurrent callers read a consistent (threads, smem, resident) triple or repeat the driver call; a launch that
+    // fails because the opt-in was lost (device reset, new primary context) opts in again and retries once, below.
     constexpr int kDevs = 16;
-    static size_t s_optin[kDevs] = {0};
-    static int s_threads[kDevs] = {0}, s_resident[kDevs] = {0};
-    static size_t s_smem[kDevs] = {0};
+    static std::atomic<unsigned long long> s_optin[kDevs];
+    static std::atomic<unsigned long long> s_occ[kDevs];      // threads (12 bits) | resident (12 bits) | smem (40 bits)
     cudaError_t e = cudaSuccess;
     int dev = 0;
     cudaGetDevice(&dev);
     const bool cached = dev >= 0 && dev < kDevs;
-    if (!cached || smem > s_optin[dev]) {
+    if (!cached || smem > s_optin[dev].load(std::memory_order_acquire)) {
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        if (cached) s_optin[dev] = smem;
+        if (cached) s_optin[dev].store(smem, std::memory_order_release);
     }
     int resident = blocks_per_sm;
     if (resident <= 0) {
-        if (cached && s_threads[dev] == threads && s_smem[dev] == smem) resident = s_resident[dev];
+        const unsigned long long key = ((unsigned long long)threads & 0xFFFull) | ((unsigned long long)smem << 24);
+        const unsigned long long got = cached ? s_occ[dev].load(std::memory_order_acquire) : 0ull;
+        if (cached && (got & ~0xFFF000ull) == key && ((got >> 12) & 0xFFFull) != 0ull) resident = (int)((got >> 12) & 0xFFFull);
         else {
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, threads, smem);
             if (e != cudaSuccess) return e;
             if (resident < 1) return cudaErrorInvalidConfiguration;
-            if (cached) { s_resident[dev] = resident; s_smem[dev] = smem; s_threads[dev] = threads; }
+            if (cached) s_occ[dev].store(key | ((unsigned long long)(resident & 0xFFF) << 12), std::memory_order_release);
         }
     }
     const long long slots = (long long)n_sms * resident;
@@ -368,7 +371,15 @@ cudaError_t launch_st_one(const KParams& P, StencilParams Q, const uint8_t* occ,
     const long long grid = (Q.n_items + ipb - 1) / ipb;
     if (grid > 0x7FFFFFFF) return cudaErrorInvalidConfiguration;
     kern<<<(unsigned)grid, threads, smem, st>>>(P, Q, occ, counts);
-    return cudaGetLastError();
+    e = cudaGetLastError();
+    if (e == cudaErrorInvalidValue && smem > 48u * 1024u) {
+        // the cached opt-in no longer holds in this context: opt in again, retry once
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        kern<<<(unsigned)grid, threads, smem, st>>>(P, Q, occ, counts);
+        e = cudaGetLastError();
+    }
+    return e;
 }
 
 template <int MT, int PZ>

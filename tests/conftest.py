@@ -27,3 +27,12 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(scope="session")
+def hb():
+    """The ctypes binding over the C ABI (GPU tests only: asserts a CUDA device)."""
+    import torch
+    from paper_2411_18906_b200 import binding
+    assert torch.cuda.is_available()
+    return binding

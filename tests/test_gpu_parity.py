@@ -10,14 +10,6 @@ from paper_2411_18906_b200 import workloads as wl
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module")
-def hb():
-    import torch
-    from paper_2411_18906_b200 import binding
-    assert torch.cuda.is_available()
-    return binding
-
-
 def pair(hb, w):
     return hb.Hea(*w.create_args()), ho.Oracle(*w.create_args())
 

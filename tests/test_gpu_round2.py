@@ -1,0 +1,324 @@
+"""GPU parity, second set: full-length trajectories of c3 / c4 against the committed oracle goldens, the chain-count
+extremes of c5, the kernel paths that a symmetric target with positive weights never reaches (asymmetric target,
+zero and negative shell weights), candidates aimed at the accept threshold (the reduced-precision reject filter),
+and the product's own chain sharding.  Same bar as test_gpu_parity.py: integers and J bit-equal to the oracle."""
+import hashlib
+import os
+
+import numpy as np
+import pytest
+
+from oracle import hea_oracle as ho
+from paper_2411_18906_b200 import sharding
+from paper_2411_18906_b200 import workloads as wl
+
+from test_gpu_parity import assert_stats_equal, pair, run_both, run_both_ex, small
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "full_length.txt")
+
+
+def load_golden():
+    """{(config, chain): {steps_done: record}} from tests/golden/full_length.txt (written by make_full_length.py, which
+    calls only oracle/)."""
+    out = {}
+    for line in open(GOLDEN):
+        if line.startswith("#") or not line.strip():
+            continue
+        f = line.split()
+        rec = dict(n_accept=int(f[3]), n_null=int(f[4]), hash=int(f[5], 16), last_accept_step=int(f[6]),
+                   J_bits=int(f[7], 16), sha=f[8], counts=np.array([int(v) for v in f[9:]], dtype=np.int32))
+        out.setdefault((f[0], int(f[1])), {})[int(f[2])] = rec
+    return out
+
+
+def compare_with_golden(hb, gold, name, steps_done, occ, counts, stats):
+    got = hb.stats_to_numpy(stats)
+    occ_np, cnt_np = occ.cpu().numpy(), counts.cpu().numpy()
+    n = 0
+    for (cfg, chain), recs in gold.items():
+        if cfg != name or steps_done not in recs or chain >= occ_np.shape[0]:
+            continue
+        r, g = recs[steps_done], got[chain]
+        where = f"{name} chain {chain} after {steps_done} steps"
+        assert int(g["n_accept"]) == r["n_accept"], where
+        assert int(g["n_null"]) == r["n_null"], where
+        assert int(g["hash"]) == r["hash"], where
+        assert int(g["last_accept_step"]) == r["last_accept_step"], where
+        assert int(np.array([g["J"]]).view(np.uint64)[0]) == r["J_bits"], where
+        assert hashlib.sha256(occ_np[chain].tobytes()).hexdigest() == r["sha"], where
+        np.testing.assert_array_equal(cnt_np[chain].ravel(), r["counts"], err_msg=where)
+        n += 1
+    return n
+
+
+@pytest.mark.parametrize("cfg,n_golden", [(3, 16), (4, 16)])
+def test_full_length_against_oracle_goldens(hb, cfg, n_golden):
+    # BASELINE.json configs c3 (256 chains x 1e6 steps, K=64) and c4 (16 chains x 1e7 steps, K=128) at FULL length in
+    # the launch configuration bench.py times (all chains, one hea_mc_run call), compared field by field with the
+    # oracle's trajectories of the golden chains (c4: all 16; c3: chains 0, 17, ..., 255) -- Alg. 3, Eq. 4
+    gold = load_golden()
+    w = wl.config(cfg)
+    h, _ = pair(hb, w)
+    occ = h.init_random(w.n_chains, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    stats, _ = h.mc_run(occ, counts, w.n_steps, w.K, w.seed)
+    assert compare_with_golden(hb, gold, w.name, w.n_steps, occ, counts, stats) == n_golden
+    recount, _, obj = h.sro_full(occ)
+    np.testing.assert_array_equal(recount.cpu().numpy(), counts.cpu().numpy())
+    np.testing.assert_array_equal(obj.cpu().numpy(), hb.stats_to_numpy(stats)["J"])
+    # the same trajectory cut at the golden checkpoints (other window / team schedules): every prefix must match too
+    occ = h.init_random(w.n_chains, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    stats = h.new_stats(w.n_chains)
+    done = 0
+    for upto in sorted({s for recs in gold.values() for s in recs if s <= w.n_steps}):
+        if (w.name, 0) not in gold or upto not in gold[(w.name, 0)]:
+            continue
+        if upto > done:
+            h.mc_run(occ, counts, upto - done, w.K, w.seed, step0=done, stats=stats)
+            done = upto
+        assert compare_with_golden(hb, gold, w.name, upto, occ, counts, stats) == n_golden
+
+
+@pytest.mark.parametrize("n_chains,n_steps", [(4096, 400), (65536, 150)])
+def test_chain_count_extremes(hb, n_chains, n_steps):
+    # BASELINE.json configs[4], MC leg: the 2,000-atom bcc cell with thousands of chains (blocks of 32-128 threads in
+    # waves); every chain checked by properties, sampled chains element by element through the oracle
+    w = wl.chain_sweep_workload(n_chains, n_steps)
+    h, o = pair(hb, w)
+    occ = h.init_random(n_chains, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    occ0 = occ.cpu().numpy().copy()
+    stats, _ = h.mc_run(occ, counts, n_steps, w.K, w.seed)
+    got = hb.stats_to_numpy(stats)
+    occ_f, cnt_f = occ.cpu().numpy(), counts.cpu().numpy()
+    recount, _, obj = h.sro_full(occ)
+    np.testing.assert_array_equal(recount.cpu().numpy(), cnt_f)
+    np.testing.assert_array_equal(obj.cpu().numpy(), got["J"])
+    assert (np.sort(occ_f, axis=1) == np.sort(occ0, axis=1)).all()                  # composition conserved
+    sample = sorted({0, 1, 127, 128, n_chains // 2 + 3, n_chains - 149, n_chains - 2, n_chains - 1})
+    for c in sample:
+        o_occ = o.init_random(1, w.seed, chain0=c)
+        np.testing.assert_array_equal(o_occ[0], occ0[c])
+        o_cnt = np.stack([o.pair_counts(o_occ[0])])
+        o_st, _ = o.mc_run(o_occ, o_cnt, n_steps, w.K, w.seed, chain0=c, eval_all=False)
+        np.testing.assert_array_equal(occ_f[c], o_occ[0])
+        np.testing.assert_array_equal(cnt_f[c], o_cnt[0])
+        assert_stats_equal(got[c:c + 1], o_st)
+
+
+def test_single_chain_automatic_team_of_32(hb):
+    # C = 1 on a c3-size cell: hea_mc_run gives the chain a team of 32 blocks on its own
+    st = run_both(hb, wl.config(3), 1, 4000, log_cap=64)
+    assert int(st["n_accept"][0]) > 1000
+    st = run_both(hb, wl.chain_sweep_workload(1), 1, 20000, log_cap=64)
+    assert int(st["n_accept"][0]) > 50
+
+
+# ---- kernel instantiations a symmetric target with positive weights never reaches
+def odd_workload(kind, lattice="fcc", dims=(4, 4, 4), conc=(0.2, 0.2, 0.2, 0.4), S=3, K=24, n_steps=500):
+    conc = list(conc)
+    M = len(conc)
+    w = small(lattice, dims, conc, S, target_seed=5, K=K, n_steps=n_steps, rng=(-0.15, 0.15))
+    t = w.target.copy()
+    shell_w = list(w.shell_w)
+    if "asym" in kind:
+        t[0, 0, 1] += 0.03125                               # t_01 != t_10: the SYM = false instantiations
+        if S > 1:
+            t[1, M - 1, 0] -= 0.0625
+    if "zero" in kind:
+        shell_w[0] = 0.0                                    # w_1 = 0: the first-shell bound is useless, filter off
+    if "neg" in kind:
+        shell_w[S - 1] = -0.375                             # a negative weight: no lower-bound pruning, J may be < 0
+    if "allneg" in kind:
+        shell_w = [-1.0, -0.5, -0.25][:S]
+    return wl.Workload(name="odd-" + kind, lattice=lattice, dims=dims, conc=conc, n_shells=S, shell_w=shell_w,
+                       n_chains=4, n_steps=n_steps, K=K, seed=w.seed, target=t)
+
+
+ODD_KINDS = ["asym", "zero", "neg", "asym+neg", "asym+zero", "allneg"]
+
+
+@pytest.mark.parametrize("kind", ODD_KINDS)
+@pytest.mark.parametrize("opts", [{"mc_engine": 1}, {"mc_engine": 1, "mc_cluster": 4, "mc_occ_mode": 3},
+                                  {"mc_engine": 2, "mc_threads": 32}, {"mc_engine": 2, "mc_threads": 512},
+                                  {"mc_engine": 2, "mc_team": 5, "mc_threads": 64, "mc_team_on": 64, "mc_team_off": 32},
+                                  {"mc_engine": 2, "mc_occ_mode": 2, "mc_threads": 512, "mc_accept": 2}, {}])
+def test_mc_asymmetric_target_zero_and_negative_weights(hb, kind, opts):
+    w = odd_workload(kind)
+    st = run_both(hb, w, 5, w.n_steps, log_cap=128, opts=opts)
+    assert st["n_accept"].sum() > 20
+    if "neg" in kind:
+        assert (st["J"] < 0).any() or kind != "allneg"
+
+
+@pytest.mark.parametrize("kind", ODD_KINDS)
+@pytest.mark.parametrize("lattice,dims,conc,S", [("bcc", (5, 5, 5), (0.2,) * 5, 3), ("fcc", (2, 2, 2), (0.5, 0.5), 2),
+                                                 ("bcc", (4, 4, 4), (0.125,) * 8, 1)])
+def test_mc_odd_targets_other_species_counts(hb, kind, lattice, dims, conc, S):
+    w = odd_workload(kind, lattice, dims, conc, S, K=32, n_steps=300)
+    run_both(hb, w, 3, w.n_steps, log_cap=64)
+
+
+@pytest.mark.parametrize("kind", ["asym", "neg", "allneg", "asym+neg"])
+@pytest.mark.parametrize("team,threads", [(1, 64), (1, 512), (4, 128)])
+@pytest.mark.parametrize("depth_limit", [0, 40])
+def test_mc_run_ex_best_of_K_with_negative_J(hb, kind, team, threads, depth_limit):
+    # best-of-K orders the candidates of a step by J: with a negative weight J < 0, which an unsigned compare of the bit
+    # patterns would order backwards
+    w = odd_workload(kind, n_steps=600)
+    st, _ = run_both_ex(hb, w, 5, w.n_steps, True, depth_limit,
+                        opts={"mc_team": team, "mc_threads": threads, "mc_team_on": 128, "mc_team_off": 64})
+    assert st["n_accept"].sum() > 20
+
+
+@pytest.mark.parametrize("kind", ["allneg", "neg", "asym+neg"])
+def test_pool_select_ranks_negative_J(hb, kind):
+    w = odd_workload(kind, "bcc", (4, 4, 4), (0.5, 0.25, 0.25), 2, K=16)
+    h, o = pair(hb, w)
+    C, n_keep = 40, 13
+    occ = h.init_random(C, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    o_occ, o_cnt = occ.cpu().numpy().copy(), counts.cpu().numpy().copy()
+    stats, o_stats = h.new_stats(C), ho.fresh_stats(C)
+    for it in range(2):
+        h.mc_run(occ, counts, 60, w.K, w.seed, step0=60 * it, stats=stats)
+        o.mc_run(o_occ, o_cnt, 60, w.K, w.seed, step0=60 * it, stats=o_stats, eval_all=False, n_threads=8)
+        order = h.pool_select(occ, counts, stats, n_keep, seed=99 + it, new_chain0=1000 * (it + 1))
+        o_order = o.pool_select(o_occ, o_cnt, o_stats, n_keep, seed=99 + it, new_chain0=1000 * (it + 1))
+        np.testing.assert_array_equal(order.cpu().numpy(), o_order)
+        np.testing.assert_array_equal(occ.cpu().numpy(), o_occ)
+        np.testing.assert_array_equal(counts.cpu().numpy(), o_cnt)
+        assert_stats_equal(hb.stats_to_numpy(stats), o_stats)
+    J = np.array([o.objective(c) for c in o_cnt])
+    assert (J < 0).any()
+
+
+# ---- candidates aimed at the accept threshold: the reduced-precision reject filter must not change a decision
+def threshold_target(lattice, dims, conc, seed, beta_shift, gamma, S, rng_seed=0):
+    """A target for which the FIRST non-null candidate of step 0 of chain 0 lands a hair below / above J_cur.
+
+    With d = alpha(N) - t and delta = alpha(N') - alpha(N) (N' = counts after that swap, first shell), J' - J =
+    w (2 d.delta + |delta|^2) for one shell, which vanishes at d = -delta/2 + gamma v, v orthogonal to delta.  The target
+    is t = alpha(N) - d with d = -(beta0 + eta) delta + gamma v (beta0 = 1/2 for one shell; with more shells, which sit
+    exactly at their target before the move, beta0 also absorbs what they add after it); `beta_shift` selects eta: a float = relative distance
+    of J' below (+) or above (-) J, or "ulp+" / "ulp-" = the two neighbouring doubles of eta at which the oracle's fp64
+    decision flips (bisection on the oracle's own J values).  Returns (Workload, (a, b), J, J')."""
+    M = len(conc)
+    base = small(lattice, dims, list(conc), S, K=64, n_steps=40, seed=seed)
+    o = ho.Oracle(*base.create_args())
+    occ0 = o.init_random(1, seed)[0]
+    counts0 = o.pair_counts(occ0)
+    k = 0
+    while True:                                             # D9.1: first non-null candidate of step 0
+        ok, a, b = o.propose(occ0, seed, 0, 0, k)
+        if ok:
+            break
+        k += 1
+    counts1 = o.delta_counts(occ0, a, b, counts0)
+    a0, a1 = o.alpha(counts0), o.alpha(counts1)
+    delta = a1[0] - a0[0]
+    rs = np.random.RandomState(rng_seed)
+    v = rs.standard_normal((M, M))
+    v = v + v.T
+    v -= delta * (v * delta).sum() / (delta * delta).sum()
+    v /= np.sqrt((v * v).sum())
+
+    shell_w = [1.0, 0.5, 0.25][:S]
+    d1 = float((delta * delta).sum())
+    rest = sum(shell_w[s] * float(((a1[s] - a0[s]) ** 2).sum()) for s in range(1, S))   # what the other shells add after the move
+    beta0 = 0.5 + rest / (2.0 * shell_w[0] * d1)            # J' == J here (in exact arithmetic)
+
+    def build(eta):
+        t = np.zeros((S, M, M))
+        t[0] = a0[0] - (-(beta0 + eta) * delta + gamma * v)
+        t[0] = 0.5 * (t[0] + t[0].T)                        # bit-symmetric (alpha of a recount is; keep it exact)
+        for s in range(1, S):
+            t[s] = a0[s]                                    # the other shells sit at their target before the move
+        wk = wl.Workload(name="thr", lattice=lattice, dims=dims, conc=list(conc), n_shells=S,
+                         shell_w=shell_w, n_chains=1, n_steps=40, K=64, seed=seed, target=t)
+        oo = ho.Oracle(*wk.create_args())
+        return wk, oo.objective(counts0), oo.objective(counts1)
+
+    def eta_of(rel):                                        # J - J' = 2 eta w_1 |delta|^2 = rel * J
+        return rel * (beta0 * beta0 * d1 + gamma * gamma) / (2.0 * d1)
+
+    if isinstance(beta_shift, str):
+        lo, hi = eta_of(-1e-3), eta_of(1e-3)                # J' > J at lo, J' < J at hi
+        assert build(lo)[2] > build(lo)[1] and build(hi)[2] < build(hi)[1]
+        for _ in range(200):
+            mid = 0.5 * (lo + hi)
+            if mid == lo or mid == hi:
+                break
+            _, J, J1 = build(mid)
+            if J1 < J:
+                hi = mid
+            else:
+                lo = mid
+        eta = hi if beta_shift == "ulp+" else lo
+    else:
+        eta = eta_of(beta_shift)
+    wk, J, J1 = build(eta)
+    return wk, (a, b), J, J1
+
+
+@pytest.mark.parametrize("shift", [1e-3, -1e-3, 1e-5, -1e-5, 1e-7, -1e-7, 1e-9, -1e-9, 1e-12, -1e-12, "ulp+", "ulp-"])
+@pytest.mark.parametrize("gamma", [0.05, 1e-5])
+@pytest.mark.parametrize("lattice,dims,conc,S", [("fcc", (6, 6, 6), (0.25,) * 4, 1), ("bcc", (7, 7, 7), (0.2,) * 5, 2),
+                                                 ("fcc", (5, 5, 5), (0.4, 0.4, 0.1, 0.1), 2)])
+@pytest.mark.parametrize("opts", [{"mc_engine": 2, "mc_threads": 32, "mc_team": 1},
+                                  {"mc_engine": 2, "mc_threads": 64, "mc_team": 4, "mc_team_on": 1, "mc_team_off": 1},
+                                  {"mc_engine": 2, "mc_threads": 32, "mc_team": 1, "mc_occ_mode": 2}])
+def test_reject_filter_at_the_accept_threshold(hb, shift, gamma, lattice, dims, conc, S, opts):
+    # SURVEY 8f-4 / north_star "any reduced-precision variant must leave accept decisions unchanged" (the paper's own
+    # reduced precision: P:297).  The designed candidate is (step 0, lowest non-null k): accepted iff J' < J in fp64.
+    # 32-thread blocks with K = 64 put every window through the filtered two-stage path from the first step on.
+    if opts.get("mc_occ_mode") == 2 and len(conc) > 4:
+        pytest.skip("nibble layout holds at most 4 species")
+    wk, (a, b), J, J1 = threshold_target(lattice, dims, conc, 17, shift, gamma, S)
+    if isinstance(shift, float):
+        assert (J1 < J) == (shift > 0)
+        assert abs((J - J1) / J) < 4 * abs(shift) + 1e-13
+    h, o = pair(hb, wk)
+    for k, v in opts.items():
+        h.set_option(k, v)
+    occ = h.init_random(1, seed=wk.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    o_occ, o_cnt = occ.cpu().numpy().copy(), counts.cpu().numpy().copy()
+    stats, log = h.mc_run(occ, counts, wk.n_steps, wk.K, wk.seed, log_cap=64)
+    o_stats, o_log = o.mc_run(o_occ, o_cnt, wk.n_steps, wk.K, wk.seed, log_cap=64, eval_all=False)
+    if S == 1:
+        first = o_log[0][0]
+        assert (int(o_stats["n_accept"][0]) > 0 and int(first["step"]) == 0 and (int(first["a"]), int(first["b"])) == (a, b)) == (J1 < J)
+    np.testing.assert_array_equal(occ.cpu().numpy(), o_occ)
+    np.testing.assert_array_equal(counts.cpu().numpy(), o_cnt)
+    assert_stats_equal(hb.stats_to_numpy(stats), o_stats)
+    got = hb.log_to_numpy(log)
+    n = int(o_stats["n_accept"][0])
+    for f in ("step", "k", "a", "b"):
+        np.testing.assert_array_equal(got[0][:n][f], o_log[0][:n][f])
+
+
+# ---- the product's own chain sharding: two (chain0, count) shards on one device == one call
+@pytest.mark.parametrize("world", [2, 3])
+def test_product_sharding_union_equals_single_call(hb, world):
+    w = wl.config(1)
+    n_chains, n_steps = 11, 300
+    h, _ = pair(hb, w)
+    occ = h.init_random(n_chains, seed=w.seed)
+    counts, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    stats, _ = h.mc_run(occ, counts, n_steps, w.K, w.seed)
+    whole = hb.stats_to_numpy(stats)
+    for rank in range(world):
+        c0, cnt = sharding.strong_chain_range(rank, world, n_chains)
+        hr, _ = pair(hb, w)                                  # a context per "rank", as bench.py has per process
+        o_r = hr.init_random(cnt, seed=w.seed, chain0=c0)
+        c_r, _, _ = hr.sro_full(o_r, want_alpha=False, want_obj=False)
+        s_r, _ = hr.mc_run(o_r, c_r, n_steps, w.K, w.seed, chain0=c0)
+        np.testing.assert_array_equal(o_r.cpu().numpy(), occ.cpu().numpy()[c0:c0 + cnt])
+        np.testing.assert_array_equal(c_r.cpu().numpy(), counts.cpu().numpy()[c0:c0 + cnt])
+        part = hb.stats_to_numpy(s_r)
+        for f in ("n_accept", "n_null", "hash", "last_accept_step", "J"):
+            np.testing.assert_array_equal(part[f], whole[f][c0:c0 + cnt])
