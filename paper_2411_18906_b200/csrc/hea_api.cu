@@ -30,7 +30,7 @@ cudaError_t launch_mc(const KParams& P, const DevTables& host_tab, int occ_mode,
                       bool fast_nbr, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
                       uint64_t step0, void* stats, void* log, int64_t log_cap, cudaStream_t st, int64_t* n_launches,
                       int* query_max_clusters);
-size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L);
+size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L, int M);
 cudaError_t launch_pool_rank(const double* J, int64_t C, int64_t n_keep, int32_t* order, cudaStream_t st, int64_t* n_launches);
 cudaError_t launch_pool_gather(const void* src, void* dst, const int32_t* order, int64_t n_keep, size_t item,
                                cudaStream_t st, int64_t* n_launches);
@@ -242,6 +242,22 @@ int hea_create(hea_ctx** out, int lattice, int Lx, int Ly, int Lz, int n_species
             dst[0] = st.nb; dst[1] = st.sx; dst[2] = st.sy; dst[3] = st.sz;
         }
 
+    for (int b = 0; b < lat.A; ++b)
+        for (int sh = 0; sh < S; ++sh) {
+            int pos = lat.zoff[sh];
+            for (int nb = 0; nb < lat.A; ++nb)
+                for (int k = lat.zoff[sh]; k < lat.zoff[sh + 1]; ++k)
+                    if (lat.stencil[b][k].nb == nb) tab[0].by_basis[b * Z + pos++] = (uint8_t)k;
+            // the MC kernel shifts four gathered nibbles at once: every aligned group of four must have one parity of nb
+            for (int i = lat.zoff[sh]; i < lat.zoff[sh + 1]; ++i) {
+                const int first = lat.zoff[sh] + ((i - lat.zoff[sh]) & ~3);
+                if ((lat.stencil[b][tab[0].by_basis[b * Z + i]].nb & 1) != (lat.stencil[b][tab[0].by_basis[b * Z + first]].nb & 1)) {
+                    delete ctx;
+                    return fail(HEA_EUNSUPPORTED, "internal: shell entries do not group by basis parity");
+                }
+            }
+        }
+
     auto bail = [&](int code, const std::string& msg) {
         hea_destroy(ctx);
         return fail(code, msg);
@@ -431,10 +447,10 @@ int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C
     // option specific to the window engine (clusters, table neighbours, global occupancy) is set; else 1 (hea_mc.cu)
     int engine = (int)ctx->opt_engine;
     if (engine == 0) {
-        const bool fits = hea::mc2_shared_bytes(1, ctx->lat.type, ctx->P.L) <= budget ||
-                          (ctx->M <= 4 && hea::mc2_shared_bytes(2, ctx->lat.type, ctx->P.L) <= budget);
-        const bool fits_req = occ_mode == 0 || (occ_mode == 1 && hea::mc2_shared_bytes(1, ctx->lat.type, ctx->P.L) <= budget) ||
-                              (occ_mode == 2 && ctx->M <= 4 && hea::mc2_shared_bytes(2, ctx->lat.type, ctx->P.L) <= budget);
+        const bool fits = hea::mc2_shared_bytes(1, ctx->lat.type, ctx->P.L, ctx->M) <= budget ||
+                          (ctx->M <= 4 && hea::mc2_shared_bytes(2, ctx->lat.type, ctx->P.L, ctx->M) <= budget);
+        const bool fits_req = occ_mode == 0 || (occ_mode == 1 && hea::mc2_shared_bytes(1, ctx->lat.type, ctx->P.L, ctx->M) <= budget) ||
+                              (occ_mode == 2 && ctx->M <= 4 && hea::mc2_shared_bytes(2, ctx->lat.type, ctx->P.L, ctx->M) <= budget);
         engine = (fits && fits_req && ctx->opt_cluster == 0 && ctx->opt_neighbors == 0) ? 2 : 1;
     }
     if (ex_mode && engine != 2)
@@ -442,8 +458,8 @@ int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C
     if (engine == 2) {
         // halo engine (hea_mc2.cu): one block per chain, padded one-hot configuration in shared memory
         int om = occ_mode;
-        if (om == 0) om = hea::mc2_shared_bytes(1, ctx->lat.type, ctx->P.L) <= budget ? 1 : 2;
-        if (om == 3 || (om == 2 && ctx->M > 4) || hea::mc2_shared_bytes(om, ctx->lat.type, ctx->P.L) > budget)
+        if (om == 0) om = hea::mc2_shared_bytes(1, ctx->lat.type, ctx->P.L, ctx->M) <= budget ? 1 : 2;
+        if (om == 3 || (om == 2 && ctx->M > 4) || hea::mc2_shared_bytes(om, ctx->lat.type, ctx->P.L, ctx->M) > budget)
             return fail(HEA_EINVAL, "mc_engine 2: the padded configuration does not fit in shared memory");
         // blocks per chain: a team of R blocks (synchronised through global memory, cooperative launch) when the
         // chains alone would leave at least half of the SMs idle; one block per SM then

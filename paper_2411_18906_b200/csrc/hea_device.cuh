@@ -15,6 +15,8 @@ struct DevTables {
     double t[kSMM];                       // alpha target, same index
     double w[4];                          // shell weights
     int8_t stencil[4 * 42 * 4];           // [b][e] -> (nb, sx, sy, sz), e over the concatenated shells, stride Z
+    uint8_t by_basis[4 * 42];             // [b][i], stride Z: the entry that comes i-th when every shell's entries are
+                                          // ordered by the neighbour's basis index nb (stable); stays within the shell
 };
 
 // Scalars passed by value to every kernel.
@@ -46,6 +48,23 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
         c3 = a_lo;
         k0 += BUMP_A;
         k1 += BUMP_B;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// The same generator with the ten round keys precomputed (rk[2r], rk[2r+1] = key + r * bump): when rk lives in
+// kernel-parameter space the keys are constant-bank operands of the xors and cost no instruction.
+__device__ __forceinline__ uint4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint32_t (&rk)[20])
+{
+    constexpr uint32_t MUL_A = 0xD2511F53u, MUL_B = 0xCD9E8D57u;
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        const uint32_t a_hi = __umulhi(MUL_A, c0), a_lo = MUL_A * c0;
+        const uint32_t b_hi = __umulhi(MUL_B, c2), b_lo = MUL_B * c2;
+        c0 = b_hi ^ c1 ^ rk[2 * round];
+        c1 = b_lo;
+        c2 = a_hi ^ c3 ^ rk[2 * round + 1];
+        c3 = a_lo;
     }
     return make_uint4(c0, c1, c2, c3);
 }

@@ -42,8 +42,10 @@ template <int LAT> __host__ __device__ constexpr int zpad() { return pad4(LatC<L
 // Lattice geometry of the padded layout (kernel parameter).
 struct Geo {
     int L[3];
-    uint32_t magy, magz;          // floor(2^32 / Ly), floor(2^32 / Lz) (0xFFFFFFFF for a divisor of 1): quotient off by <= 1
-    uint32_t pmagy, pmagz;        // the same for the padded counts Ly + 2, Lz + 2
+    uint32_t mq, sq;              // site / (A Lz)    = umulhi(site, mq) >> sq, exact for every site < 2^31 (see div_magic)
+    uint32_t mx, sx;              // site / (A Ly Lz) = umulhi(site, mx) >> sx
+    uint32_t cx, cc;              // padded index = site + 2 A q + cx x + cc,  q = site / (A Lz) = x Ly + y,  x = site / (A Ly Lz)
+    uint32_t pmagy, pmagz;        // floor(2^32 / (Ly + 2)), floor(2^32 / (Lz + 2)): quotient off by <= 1 (load_state only)
     int PLy, PLz;                 // padded cell counts L + 2
     int NP;                       // padded sites
     uint32_t basis;               // bit 3b + d = doubled coordinate d of basis site b
@@ -81,8 +83,8 @@ struct Sh2 {
     int4 wdesc[24];               // accumulator word w -> (int4 index in the offset row, slot mask, shell, side)
     double g[kSMM], t[kSMM];      // objective constants with a per-lane index
     // two-stage evaluation of long windows: integer pre-filter on shell 1, survivors queued for the full evaluation
-    float fb2[64];                // first-shell cell (i, j): 2 (N_ij - n*_ij), n* = the count at which alpha = target
-    float fwg[64];                //                          w_1 g_ij^2
+    double nstar[64];             // first-shell cell (i, j): n*_ij = (1 - t_ij) / g_ij, the (real) count at which alpha = target
+    double W1[64];                //                          w_1 g_ij^2
     uint32_t q_n[3];              // queue fill, triple-buffered like best[]
     uint32_t bestk;               // best-of-K: lowest key among the minimum-J candidates of the deciding step
     unsigned long long bestJ;     // best-of-K: minimum J (ordered_bits key) among the candidates of the deciding step
@@ -94,20 +96,21 @@ struct SiteC {
     int x, y, z, b;               // cell coordinates and basis index
 };
 
+// Site index -> cell coordinates, basis index and padded index.  Two exact multiply-high divisions by constants (a
+// site index is divided by A Lz and by A Ly Lz directly, so no divisor is 1); the padded index needs no coordinates:
+// ((x+1) PLy + (y+1)) PLz + (z+1) = cell + 2 q + 2 PLz x + (PLy PLz + PLz + 1) with q = x Ly + y.  y and z are dead code
+// wherever only the padded index is used.
 template <int LAT>
 __device__ __forceinline__ SiteC decode_site(const Geo& G, uint32_t a)
 {
     SiteC s;
-    const uint32_t cell = a >> LatC<LAT>::lgA;
+    const uint32_t q = __umulhi(a, G.mq) >> G.sq;
+    const uint32_t x = __umulhi(a, G.mx) >> G.sx;
     s.b = (int)(a & (uint32_t)(LatC<LAT>::A - 1));
-    uint32_t q1 = __umulhi(cell, G.magz);
-    uint32_t z = cell - q1 * (uint32_t)G.L[2];
-    if (z >= (uint32_t)G.L[2]) { z -= (uint32_t)G.L[2]; ++q1; }
-    uint32_t q2 = __umulhi(q1, G.magy);
-    uint32_t y = q1 - q2 * (uint32_t)G.L[1];
-    if (y >= (uint32_t)G.L[1]) { y -= (uint32_t)G.L[1]; ++q2; }
-    s.x = (int)q2; s.y = (int)y; s.z = (int)z;
-    s.pidx = ((((q2 + 1u) * (uint32_t)G.PLy + (y + 1u)) * (uint32_t)G.PLz + (z + 1u)) << LatC<LAT>::lgA) | (uint32_t)s.b;
+    s.x = (int)x;
+    s.y = (int)(q - x * (uint32_t)G.L[1]);
+    s.z = (int)((a >> LatC<LAT>::lgA) - q * (uint32_t)G.L[2]);
+    s.pidx = a + (uint32_t)(2 * LatC<LAT>::A) * q + G.cx * x + G.cc;
     return s;
 }
 
@@ -130,29 +133,28 @@ __device__ __forceinline__ void occ_set(uint8_t* s_occ, uint32_t pidx, uint32_t 
 }
 
 // One-hot codes of the ZS neighbours of a site in one shell, four byte slots per accumulator word.
-// Table entries: OCC2_U8 -> padded index offset; OCC2_NIB -> 8 * byte offset + nibble shift (relative to the byte
-// pair of the site, see the table build).
+// Table entries: OCC2_U8 -> padded index offset; OCC2_NIB -> 8 * byte offset + nibble shift, relative to the byte of the
+// site.  The entries of a shell are ordered by the basis index of the neighbour (see the table build), so the four
+// entries of a group share their nibble shift: four byte loads are merged into a word, then shifted and masked once.
 template <int OCC, int ZS>
 __device__ __forceinline__ void gather_shell(const uint8_t* __restrict__ s_occ, const int4* __restrict__ trow, uint32_t pidx,
                                              uint32_t (&acc)[(ZS + 3) / 4])
 {
-    const uint32_t base = OCC == OCC2_NIB ? (pidx & ~1u) << 2 : pidx;
+    const uint8_t* base = s_occ + (OCC == OCC2_NIB ? pidx >> 1 : pidx);
 #pragma unroll
     for (int g = 0; g < (ZS + 3) / 4; ++g) {
         const int4 o = trow[g];
-        uint32_t w = 0;
+        uint32_t x[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             if (g * 4 + j < ZS) {
                 const int oj = j == 0 ? o.x : j == 1 ? o.y : j == 2 ? o.z : o.w;
-                const uint32_t t = base + (uint32_t)oj;
-                uint32_t x;
-                if (OCC == OCC2_NIB) x = (uint32_t)s_occ[t >> 3] >> (t & 4u);
-                else x = s_occ[t];
-                w += x << (8 * j);
+                x[j] = base[OCC == OCC2_NIB ? (oj >> 3) : oj];
             }
         }
-        if (OCC == OCC2_NIB) w &= 0x0F0F0F0Fu;
+        // bytes 1..3 of a loaded value are zero: selector 0x1140 = (x.b0, y.b0, 0, 0)
+        uint32_t w = __byte_perm(__byte_perm(x[0], x[1], 0x1140), __byte_perm(x[2], x[3], 0x1140), 0x5410);
+        if (OCC == OCC2_NIB) w = (w >> (o.x & 4)) & 0x0F0F0F0Fu;
         acc[g] = w;
     }
 }
@@ -225,7 +227,9 @@ constexpr int kHaloThreads = 512;            // block size cap: 128 registers pe
 constexpr int kTeamRounds = 128;            // candidates per thread per window: longer windows amortise the imbalance between
                                             // warps and blocks at the window barrier (c4 reject regime, trials/s: 32 rounds 3.9e10,
                                             // 64 4.1e10, 128 4.25e10, 256 4.15e10 -- two more mask registers cost more than they save)
-constexpr int kNullWords = kTeamRounds / 64; // 64-bit words of the per-thread null mask
+constexpr int kNullWords = kTeamRounds / 32; // 32-bit words of the per-thread null mask
+// Row of the reject-filter table (one per ordered species pair (p, q)): threshold, X, 2 pad, L[M], Q[M], c'[M] floats.
+__host__ __device__ constexpr int filt_row(int M) { return (4 + 3 * M + 3) & ~3; }
 
 struct TeamSlot {                 // 64 bytes
     uint32_t seq;                 // team-window number + 1 when the record below is valid
@@ -263,6 +267,7 @@ struct Mc2Args {
     int team_on, team_off;        // enter TEAM when W*K >= team_on; leave it after a move with steps_done*K < team_off
     int accept_engine;            // 1: single-step windows run on the 8-lanes-per-candidate engine
     int pae;                      // 1: ... pipelined over epochs of steps (record, dirty-bitmap and offset buffers present)
+    uint32_t rk[20];              // Philox round keys of the seed (D7): key + r * (0x9E3779B9, 0xBB67AE85), r = 0..9
     // hea_mc_run_ex
     int select_best;              // 1: the minimum J_k of a step is taken (ties -> lowest k) instead of the lowest improving k
     unsigned long long depth_limit;        // > 0: a chain stops after this many consecutive steps without a move
@@ -288,7 +293,9 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     Sh2& sh = *reinterpret_cast<Sh2*>(s_raw + occ_bytes);
     int* s_tab = reinterpret_cast<int*>(s_raw + occ_bytes + ((sizeof(Sh2) + 15) & ~(size_t)15));
     // pipelined accept engine buffers (only when AA.pae): records | dirty bitmap over logical sites | logical offsets [A][Z]
-    PRec* s_prec = reinterpret_cast<PRec*>(s_tab + LC::A * ZP);
+    constexpr int RS = filt_row(M);
+    float* s_ftab = reinterpret_cast<float*>(s_tab + LC::A * ZP);       // [M*M][RS] reject-filter rows (16-byte aligned)
+    PRec* s_prec = reinterpret_cast<PRec*>(s_ftab + MM * RS);
     uint32_t* s_dirty = reinterpret_cast<uint32_t*>(s_prec + kPaeRecs);
     int* s_loff = reinterpret_cast<int*>(s_dirty + ((P.N + 31) >> 5));
 
@@ -302,7 +309,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     unsigned long long* g_stats = A.stats_all + chain_local * 5;
     TeamCtl* ctl = R > 1 ? AA.team + chain_local : nullptr;
     const uint32_t chain = (uint32_t)(A.chain0 + chain_local);
-    const uint32_t key0 = (uint32_t)A.seed, key1 = (uint32_t)(A.seed >> 32);
     const int Lx = G.L[0], Ly = G.L[1], Lz = G.L[2];
 
     // counts and the padded one-hot configuration from global memory (L2 loads: a leader may just have written them)
@@ -350,7 +356,8 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         const int zs = s == 0 ? LC::z0 : s == 1 ? LC::z1 : LC::z2;
         int entry = 0;
         if (s < S && e < zs) {
-            const int8_t* st = P.tab->stencil + (b * P.Z + P.zoff[s] + e) * 4;     // (nb, sx, sy, sz)
+            // slot e holds the entry that comes e-th when the shell is ordered by the neighbour's basis index
+            const int8_t* st = P.tab->stencil + (b * P.Z + (int)P.tab->by_basis[b * P.Z + P.zoff[s] + e]) * 4;     // (nb, sx, sy, sz)
             const int off = ((((int)st[1] * G.PLy + (int)st[2]) * G.PLz + (int)st[3]) << LC::lgA) + ((int)st[0] - b);
             if (OCC == OCC2_NIB) {
                 const int tt = (b & 1) + off;                 // padded index parity of the site == b & 1 (A is even)
@@ -362,6 +369,11 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         s_tab[i] = entry;
     }
     for (int i = tid; i < SMM; i += T) { sh.g[i] = Kc.g[i]; sh.t[i] = Kc.t[i]; }
+    for (int i = tid; i < MM; i += T) {
+        const double gi = Kc.g[i];
+        sh.nstar[i] = (1.0 - Kc.t[i]) / gi;
+        sh.W1[i] = Kc.w[0] * gi * gi;
+    }
     if (AA.pae) {
         for (int i = tid; i < ((P.N + 31) >> 5); i += T) s_dirty[i] = 0u;
         for (int i = tid; i < LC::A * P.Z; i += T) {      // neighbour e of a site of basis b without periodic wrap
@@ -496,7 +508,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     // D9.1: the proposal of candidate (step, k): sites, their decoded positions and one-hot species (equal codes = null)
     auto propose2 = [&](unsigned long long step, uint32_t k, uint32_t& a, uint32_t& b, SiteC& sa, SiteC& sb, uint32_t& hp,
                         uint32_t& hq, uint32_t& a1, uint32_t& b1) {
-        const uint4 r = philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), k, chain, key0, key1);
+        const uint4 r = philox4x32_10_rk((uint32_t)step, (uint32_t)(step >> 32), k, chain, AA.rk);
         a = __umulhi(r.x, (uint32_t)N); b = __umulhi(r.y, (uint32_t)N - 1u);
         b += (b >= a);
         a1 = a; b1 = b;
@@ -518,12 +530,11 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     auto adjacency = [&](uint32_t a, uint32_t b, const SiteC& sa, const SiteC& sb, int& mm0, int& mm1, int& mm2) {
         mm0 = 0; mm1 = 0; mm2 = 0;
         if (G.distinct) {
-            // neighbours of any shell sit in cells at most one apart (periodically): almost every pair fails this test
-            const int cx = sb.x - sa.x, cy = sb.y - sa.y, cz = sb.z - sa.z;
-            const bool nx = (uint32_t)(cx + 1) <= 2u || cx == Lx - 1 || cx == 1 - Lx;
-            const bool ny = (uint32_t)(cy + 1) <= 2u || cy == Ly - 1 || cy == 1 - Ly;
-            const bool nz = (uint32_t)(cz + 1) <= 2u || cz == Lz - 1 || cz == 1 - Lz;
-            if (nx && ny && nz) {
+            // neighbours of any shell sit in cells at most one apart (periodically): almost every pair fails on x or y
+            const int cx = sb.x - sa.x, cy = sb.y - sa.y;
+            const int ax = abs(cx), ay = abs(cy);
+            if ((ax <= 1 || ax == Lx - 1) && (ay <= 1 || ay == Ly - 1)) {
+                const int cz = sb.z - sa.z;
                 const int dx = 2 * cx + (int)((G.basis >> (3 * sb.b)) & 1u) - (int)((G.basis >> (3 * sa.b)) & 1u);
                 const int dy = 2 * cy + (int)((G.basis >> (3 * sb.b + 1)) & 1u) - (int)((G.basis >> (3 * sa.b + 1)) & 1u);
                 const int dz = 2 * cz + (int)((G.basis >> (3 * sb.b + 2)) & 1u) - (int)((G.basis >> (3 * sa.b + 2)) & 1u);
@@ -567,18 +578,14 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 const uint32_t pidx = dsc.w ? sb.pidx : sa.pidx;
                 const int bb = dsc.w ? sb.b : sa.b;
                 const int4 o = reinterpret_cast<const int4*>(s_tab + bb * ZP)[dsc.x];
-                const uint32_t base = OCC == OCC2_NIB ? (pidx & ~1u) << 2 : pidx;
+                const uint8_t* base = s_occ + (OCC == OCC2_NIB ? pidx >> 1 : pidx);
                 uint32_t acc = 0;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const int oj = j == 0 ? o.x : j == 1 ? o.y : j == 2 ? o.z : o.w;
-                    const uint32_t t = base + (uint32_t)oj;
-                    uint32_t x;
-                    if (OCC == OCC2_NIB) x = (uint32_t)s_occ[t >> 3] >> (t & 4u);
-                    else x = s_occ[t];
-                    acc += x << (8 * j);
+                    acc += (uint32_t)base[OCC == OCC2_NIB ? (oj >> 3) : oj] << (8 * j);
                 }
-                if (OCC == OCC2_NIB) acc &= 0x0F0F0F0Fu;
+                if (OCC == OCC2_NIB) acc = (acc >> (o.x & 4)) & 0x0F0F0F0Fu;   // a group shares its nibble shift (table order)
                 acc &= (uint32_t)dsc.y;
                 PD pk = 0;
 #pragma unroll
@@ -862,7 +869,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             const double J_cur = sh.J;
             if (tid >= 256) {
                 for (uint32_t k = (uint32_t)tid - 256u; k < (uint32_t)K; k += (uint32_t)T - 256u) {
-                    const uint4 r = philox4x32_10((uint32_t)t0, (uint32_t)(t0 >> 32), k, chain, key0, key1);
+                    const uint4 r = philox4x32_10_rk((uint32_t)t0, (uint32_t)(t0 >> 32), k, chain, AA.rk);
                     uint32_t a = __umulhi(r.x, (uint32_t)N), b = __umulhi(r.y, (uint32_t)N - 1u);
                     b += (b >= a);
                     uint32_t hp = occ_get<OCC>(s_occ, decode_site<LAT>(G, a).pidx), hq = occ_get<OCC>(s_occ, decode_site<LAT>(G, b).pidx);
@@ -903,36 +910,78 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             uint32_t win_key = kNoKey, win_a = 0, win_b = 0, win_pq = 0;
             PW win_d0 = 0, win_d1 = 0, win_d2 = 0;
             double win_J = 0.0;
-            uint64_t nullmask[kNullWords];                          // bit j = this thread's j-th candidate of the window is null
+            uint32_t nullw[kNullWords];                             // bit j = this thread's j-th candidate of the window is null
 #pragma unroll
-            for (int wd = 0; wd < kNullWords; ++wd) nullmask[wd] = 0;
+            for (int wd = 0; wd < kNullWords; ++wd) nullw[wd] = 0u;
 
-            // ---- long windows run in two stages: an integer pre-filter on the first shell (a candidate can only
-            // improve if w_1 e_ij(N_ij + dN_ij) < J_cur for every cell, i.e. dN_ij inside a precomputed interval),
-            // survivors queued and evaluated in full afterwards -- so that a few survivors do not hold whole warps
+            // ---- long windows run in two stages.  Stage 1: a reduced-precision REJECT FILTER on the first shell.  With
+            // w_s >= 0 the first-shell term w_1 sh_1 of a candidate is a lower bound of its J_k (partial sums of D6 are
+            // monotone), and in exact arithmetic it is a quadratic form of the first-shell count differences F:
+            //   w_1 sh_1' = C + sum_r (L_r + Q_r F_r) F_r + X (F_q - F_p)^2,   coefficients per ordered species pair (p, q)
+            // (DESIGN.md 6.2).  The form is evaluated in fp32 from a per-pair table row rebuilt after every move; the row's
+            // threshold = max(1.001 J_cur, 1e-18 w_1) - C + E rounded up, where E bounds (rigorously: coefficient
+            // rounding, the fp32 evaluation, the fp64 table arithmetic) the distance between the fp32 value and the exact
+            // one for every admissible F, and the 0.1 % margin and the floor cover the rounding of the D6 evaluation itself.
+            // A candidate above its threshold cannot improve and is dropped; the survivors are queued and evaluated exactly
+            // (stage 2), so every accept decision is the fp64 one.  Needs a bit-symmetric target and w >= 0, w_1 > 0.
             const bool use_filter = SYM && prune && Kc.w[0] > 0.0 && (unsigned long long)Wc * (unsigned)K >= 2ull * GT;
-            float filt_T0 = 0.0f, filt_thr = 0.0f;
-            if (use_filter) {
-                if (!(slack_J == J_cur)) {
-                    for (int idx = tid; idx < MM; idx += T) {
-                        const double gi = sh.g[idx];
-                        sh.fb2[idx] = (float)(2.0 * ((double)sh.cnt[idx] - (1.0 - sh.t[idx]) / gi));
-                        sh.fwg[idx] = (float)(Kc.w[0] * gi * gi);
+            if (use_filter && !(slack_J == J_cur)) {
+                for (int idx = tid; idx < MM; idx += T) {
+                    const int p = idx / M, q = idx - p * M;
+                    float* row = s_ftab + idx * RS;
+                    double Cq = 0.0, EC = 0.0;                          // C and the bound of its own error
+                    for (int c2 = 0; c2 < MM; ++c2) {
+                        const double be = (double)sh.cnt[c2] - sh.nstar[c2];
+                        const double eb = 4.44e-16 * (fabs(sh.nstar[c2]) + fabs(be));       // 2^-51: |be - beta| <= eb
+                        Cq += sh.W1[c2] * be * be;
+                        EC += sh.W1[c2] * (2.0 * fabs(be) + eb) * eb;
                     }
-                    slack_J = J_cur;
-                    __syncthreads();
+                    auto Wc2 = [&](int i, int j2) { return sh.W1[i * M + j2]; };
+                    auto b2 = [&](int i, int j2) { return 2.0 * ((double)sh.cnt[i * M + j2] - sh.nstar[i * M + j2]); };
+                    auto e2 = [&](int i, int j2) {                     // bound of the error of b2
+                        return 2.0 * 4.44e-16 * (fabs(sh.nstar[i * M + j2]) + fabs((double)sh.cnt[i * M + j2] - sh.nstar[i * M + j2]));
+                    };
+                    const double Fm = 2.0 * (double)LC::z0;            // |F_r| <= z_1 + multiplicity corrections <= 2 z_1
+                    double A = 0.0, B = 0.0;                           // sum of |term| bounds; propagated input error
+                    bool finite = p != q;
+                    for (int r = 0; r < M; ++r) {
+                        double t1, t2, Qr, cr = 0.0, et;
+                        if (r == p)      { t1 =  2.0 * Wc2(p, p) * b2(p, p); t2 = -2.0 * Wc2(p, q) * b2(p, q); Qr = 4.0 * Wc2(p, p); cr = -1.0;
+                                           et = 2.0 * Wc2(p, p) * e2(p, p) + 2.0 * Wc2(p, q) * e2(p, q); }
+                        else if (r == q) { t1 = -2.0 * Wc2(q, q) * b2(q, q); t2 =  2.0 * Wc2(p, q) * b2(p, q); Qr = 4.0 * Wc2(q, q); cr = 1.0;
+                                           et = 2.0 * Wc2(q, q) * e2(q, q) + 2.0 * Wc2(p, q) * e2(p, q); }
+                        else             { t1 =  2.0 * Wc2(p, r) * b2(p, r); t2 = -2.0 * Wc2(q, r) * b2(q, r); Qr = 2.0 * (Wc2(p, r) + Wc2(q, r));
+                                           et = 2.0 * Wc2(p, r) * e2(p, r) + 2.0 * Wc2(q, r) * e2(q, r); }
+                        const float Lf = (float)(t1 + t2), Qf = (float)Qr;
+                        row[4 + r] = Lf; row[4 + M + r] = Qf; row[4 + 2 * M + r] = (float)cr;
+                        A += (fabs(t1) + fabs(t2)) * Fm + Qr * Fm * Fm;
+                        B += et * Fm;
+                        // a coefficient lost to fp32 underflow or overflow would break the relative-error model
+                        finite = finite && isfinite(Lf) && isfinite(Qf) && (Qf >= 1.0e-30f) && (Lf == 0.0f || fabsf(Lf) >= 1.0e-30f);
+                    }
+                    const double X = 2.0 * Wc2(p, q);
+                    const float Xf = (float)X;
+                    A += X * 4.0 * Fm * Fm;
+                    finite = finite && isfinite(Xf) && Xf >= 1.0e-30f;
+                    // E: 2^-19 A covers the fp32 coefficient roundings and the <= 16 roundings of the fp32 evaluation
+                    // (gamma_16 < 2^-20) and the fp64 roundings of the table arithmetic; B and EC the cancellation in cnt - n*
+                    const double E = 1.9073486328125e-6 * A + 1.000001 * (B + EC) + 1.0e-12 * fabs(Cq);
+                    const double thr = fmax(1.001 * J_cur, 1.0e-18 * Kc.w[0]) - Cq + E;
+                    const float thr_f = __double2float_ru(thr);
+                    row[0] = (finite && isfinite(thr_f)) ? thr_f : __int_as_float(0x7f800000);   // +inf: nothing is dropped
+                    row[1] = Xf; row[2] = 0.0f; row[3] = 0.0f;
                 }
-                for (int idx = 0; idx < MM; ++idx) { const float hb = 0.5f * sh.fb2[idx]; filt_T0 = fmaf(sh.fwg[idx] * hb, hb, filt_T0); }
-                filt_thr = fmaxf((float)J_cur * 1.002f, 1.0e-30f);
+                slack_J = J_cur;
+                __syncthreads();
             }
             // the part of an evaluation after the first shell's F: D6 objective shell by shell with the exact pruning
             auto eval_rest = [&](uint32_t key, uint32_t a, uint32_t b, const SiteC& sa, const SiteC& sb, int p, int q,
-                                 const int (&c)[M], int mm1, int mm2, const int (&F0)[M]) {
+                                 int mm1, int mm2, const int (&F0)[M]) {
                 const int4* ta = reinterpret_cast<const int4*>(s_tab + sa.b * ZP);
                 const int4* tb = reinterpret_cast<const int4*>(s_tab + sb.b * ZP);
-                int F1[M], F2[M];
+                int c[M], F1[M], F2[M];
 #pragma unroll
-                for (int r2 = 0; r2 < M; ++r2) { F1[r2] = 0; F2[r2] = 0; }
+                for (int r2 = 0; r2 < M; ++r2) { c[r2] = (r2 == p) - (r2 == q); F1[r2] = 0; F2[r2] = 0; }
                 double Jk = __dmul_rn(Kc.w[0], shell_sum_F<M, SYM>(sh.cnt, Kc.g, Kc.t, F0, c));
                 Jk = __dadd_rn(0.0, Jk);
                 if (S > 1 && (!prune || __any_sync(__activemask(), Jk < J_cur))) {
@@ -972,64 +1021,63 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 }
             };
             // first-shell species-count differences of a non-null candidate
-            auto first_shell = [&](const SiteC& sa, const SiteC& sb, int mm0, const int (&c)[M], int (&F0)[M]) {
+            auto first_shell = [&](const SiteC& sa, const SiteC& sb, int mm0, int p, int q, int (&F0)[M]) {
                 uint32_t xa[NA0], xb[NA0];
                 gather_shell<OCC, LC::z0>(s_occ, reinterpret_cast<const int4*>(s_tab + sa.b * ZP), sa.pidx, xa);
                 gather_shell<OCC, LC::z0>(s_occ, reinterpret_cast<const int4*>(s_tab + sb.b * ZP), sb.pidx, xb);
                 hist_diff<M, NA0>(xa, xb, F0);
+                if (mm0 != 0) {                                     // a and b are first-shell neighbours (rare): D9.2 exclusion
 #pragma unroll
-                for (int r2 = 0; r2 < M; ++r2) F0[r2] -= mm0 * c[r2];
+                    for (int r2 = 0; r2 < M; ++r2) F0[r2] -= mm0 * ((r2 == p) - (r2 == q));
+                }
             };
 
             uint32_t ts = ts_first, k = k_first;
-            for (int j = 0; ts < Wc; ++j) {
+            uint32_t ncur = 0u;                                     // null bits of the current group of 32 candidates
+            int j = 0;
+            for (; ts < Wc; ++j) {
                 const uint32_t hint = *best_slot;
                 if ((hint >> 10) < ts) break;                       // a move at an earlier step exists: this step is void
                 const uint32_t key = (ts << 10) | k;
                 uint32_t a, b, hp, hq;
                 SiteC sa, sb;
                 propose(t0 + ts, k, a, b, sa, sb, hp, hq);
-                if (hp == hq) {
+                ncur = __funnelshift_r(ncur, hp == hq ? 1u : 0u, 1);        // candidate j ends up at bit j & 31
+                if ((j & 31) == 31) {                               // j is the same in every thread of the block
 #pragma unroll
-                    for (int wd = 0; wd < kNullWords; ++wd) nullmask[wd] |= (j >> 6) == wd ? 1ull << (j & 63) : 0ull;
-                } else if (best_mode || key < hint) {               // same step, higher k than a known move: only nullness counts
+                    for (int wd = 0; wd < kNullWords; ++wd) nullw[wd] = (j >> 5) == wd ? ncur : nullw[wd];
+                }
+                if (hp != hq && (best_mode || key < hint)) {        // same step, higher k than a known move: only nullness counts
                     const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
-                    int c[M], F0[M];
-#pragma unroll
-                    for (int r2 = 0; r2 < M; ++r2) c[r2] = (r2 == p) - (r2 == q);
+                    int F0[M];
                     int mm0, mm1, mm2;
                     adjacency(a, b, sa, sb, mm0, mm1, mm2);
-                    first_shell(sa, sb, mm0, c, F0);
+                    first_shell(sa, sb, mm0, p, q, F0);
                     bool full = true;
                     if (use_filter) {
-                        // fp32 model of w_1 sh_1 after the move: T0 + sum over the changed cells of w g^2 dN (2 b + dN),
-                        // rows p and q (dN_pj = F_j + c_j F_p, dN_qj = -F_j + c_j F_q), the mirrored cells (j, p), (j, q)
-                        // through the weight 2 - |c_j|.  Relative error ~1e-6; the threshold carries a 2e-3 margin.
-                        int Fp = 0, Fq = 0;
-#pragma unroll
-                        for (int r2 = 0; r2 < M; ++r2) { Fp = c[r2] > 0 ? F0[r2] : Fp; Fq = c[r2] < 0 ? F0[r2] : Fq; }
-                        const float* b2p = sh.fb2 + p * M; const float* wgp = sh.fwg + p * M;
-                        const float* b2q = sh.fb2 + q * M; const float* wgq = sh.fwg + q * M;
-                        float lb = filt_T0;
+                        const float* row = s_ftab + (p * M + q) * RS;
+                        float acc = 0.0f, D = 0.0f;
 #pragma unroll
                         for (int r2 = 0; r2 < M; ++r2) {
-                            const float cw = c[r2] != 0 ? 1.0f : 2.0f;
-                            const float dp = __int_as_float(0x4B400000 + (F0[r2] + c[r2] * Fp)) - 12582912.0f;
-                            const float dq = __int_as_float(0x4B400000 + (c[r2] * Fq - F0[r2])) - 12582912.0f;
-                            lb = fmaf(dp * (b2p[r2] + dp) * wgp[r2], cw, lb);
-                            lb = fmaf(dq * (b2q[r2] + dq) * wgq[r2], cw, lb);
+                            const float f = (float)F0[r2];
+                            acc = fmaf(fmaf(row[4 + M + r2], f, row[4 + r2]), f, acc);
+                            D = fmaf(row[4 + 2 * M + r2], f, D);
                         }
-                        const bool out = lb > filt_thr;
-                        full = !out;
+                        acc = fmaf(row[1] * D, D, acc);
+                        full = !(acc > row[0]);
                         if (full) {
                             const uint32_t slot = atomicAdd(&sh.q_n[buf], 1u);
                             if (slot < (uint32_t)kQueueCap) { sh.queue[slot] = key; full = false; }
                         }
                     }
-                    if (full) eval_rest(key, a, b, sa, sb, p, q, c, mm1, mm2, F0);
+                    if (full) eval_rest(key, a, b, sa, sb, p, q, mm1, mm2, F0);
                 }
                 k += k_inc; ts += ts_inc;
                 if (k >= (uint32_t)K) { k -= (uint32_t)K; ++ts; }
+            }
+            if (j & 31) {                                           // the last, partial group
+#pragma unroll
+                for (int wd = 0; wd < kNullWords; ++wd) nullw[wd] = (j >> 5) == wd ? ncur >> (32 - (j & 31)) : nullw[wd];
             }
             if (use_filter) {
                 // ---- second stage: the queued survivors, one per thread
@@ -1043,13 +1091,11 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     SiteC sa, sb;
                     propose(t0 + (key >> 10), key & 1023u, a, b, sa, sb, hp, hq);
                     const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
-                    int c[M], F0[M];
-#pragma unroll
-                    for (int r2 = 0; r2 < M; ++r2) c[r2] = (r2 == p) - (r2 == q);
+                    int F0[M];
                     int mm0, mm1, mm2;
                     adjacency(a, b, sa, sb, mm0, mm1, mm2);
-                    first_shell(sa, sb, mm0, c, F0);
-                    eval_rest(key, a, b, sa, sb, p, q, c, mm1, mm2, F0);
+                    first_shell(sa, sb, mm0, p, q, F0);
+                    eval_rest(key, a, b, sa, sb, p, q, mm1, mm2, F0);
                 }
             }
             __syncthreads();                                        // B1: window evaluated, local minimum posted
@@ -1128,9 +1174,9 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 const uint32_t n_comm = gtid < lim ? (lim - 1u - gtid) / GT + 1u : 0u;
 #pragma unroll
                 for (int wd = 0; wd < kNullWords; ++wd) {
-                    const uint32_t lo = 64u * (uint32_t)wd;
+                    const uint32_t lo = 32u * (uint32_t)wd;
                     if (n_comm > lo)
-                        my_null += __popcll(n_comm >= lo + 64u ? nullmask[wd] : (nullmask[wd] & ((1ull << (n_comm - lo)) - 1ull)));
+                        my_null += __popc(n_comm >= lo + 32u ? nullw[wd] : (nullw[wd] & ((1u << (n_comm - lo)) - 1u)));
                 }
             }
             if (key_best != kNoKey) {
@@ -1266,13 +1312,14 @@ cudaError_t launch_mc2_part2(bool, int, const KParams&, const DevTables&, const 
 cudaError_t launch_mc2_part3(bool, int, const KParams&, const DevTables&, const void*, int64_t, int, size_t, cudaStream_t);
 
 // Shared-memory bytes of the halo engine (occ_mode 1 = one-hot bytes, 2 = one-hot nibbles).
-size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L)
+size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L, int M)
 {
     const int A = lattice == 0 ? 4 : 2;
     const size_t NP = (size_t)(L[0] + 2) * (L[1] + 2) * (L[2] + 2) * A;
     size_t s = ((occ_mode == OCC2_NIB ? (NP + 1) / 2 : NP) + 15) & ~(size_t)15;
     s += (sizeof(Sh2) + 15) & ~(size_t)15;
     s += sizeof(int) * (size_t)A * (lattice == 0 ? zpad<0>() : zpad<1>());
+    s += sizeof(float) * (size_t)M * M * filt_row(M);       // reject-filter rows
     return (s + 15) & ~(size_t)15;
 }
 
@@ -1316,14 +1363,29 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
     Geo& G = AA.G;
     for (int d = 0; d < 3; ++d) G.L[d] = P.L[d];
     auto magic = [](int d) { return d == 1 ? 0xFFFFFFFFu : (uint32_t)((1ull << 32) / (uint64_t)d); };
-    G.magy = magic(P.L[1]); G.magz = magic(P.L[2]);
+    // exact division of n < 2^31 by d >= 2: with l = ceil(log2 d), s = l - 1 and m = ceil(2^(32+s) / d) < 2^32 the error
+    // e = m d - 2^(32+s) is < d <= 2^l, so n e < 2^(32+s) and floor(n m / 2^(32+s)) = floor(n / d)
+    auto div_magic = [](uint64_t d, uint32_t& m, uint32_t& sft) {
+        int l = 0;
+        while ((1ull << l) < d) ++l;
+        sft = (uint32_t)(l - 1);
+        m = (uint32_t)(((1ull << (32 + sft)) + d - 1) / d);
+    };
+    div_magic((uint64_t)P.A * (uint64_t)P.L[2], G.mq, G.sq);
+    div_magic((uint64_t)P.A * (uint64_t)P.L[1] * (uint64_t)P.L[2], G.mx, G.sx);
     G.PLy = P.L[1] + 2; G.PLz = P.L[2] + 2;
+    G.cx = (uint32_t)(2 * P.A * G.PLz);
+    G.cc = (uint32_t)(P.A * (G.PLy * G.PLz + G.PLz + 1));
     G.pmagy = magic(G.PLy); G.pmagz = magic(G.PLz);
     G.NP = (P.L[0] + 2) * G.PLy * G.PLz * P.A;
+    for (int r = 0; r < 10; ++r) {
+        AA.rk[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
+        AA.rk[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    }
     if (lattice == 0) { G.basis = (1u << 4) | (1u << 5) | (1u << 6) | (1u << 8) | (1u << 9) | (1u << 10); G.d2[0] = 2; G.d2[1] = 4; G.d2[2] = 6; }
     else { G.basis = (1u << 3) | (1u << 4) | (1u << 5); G.d2[0] = 3; G.d2[1] = 4; G.d2[2] = 8; }
     G.distinct = P.L[0] >= 3 && P.L[1] >= 3 && P.L[2] >= 3;
-    size_t smem = mc2_shared_bytes(occ_mode, lattice, P.L);
+    size_t smem = mc2_shared_bytes(occ_mode, lattice, P.L, P.M);
     // the pipelined accept engine needs its record, bitmap and offset buffers on top; without room it is simply off
     const size_t pae_bytes = sizeof(PRec) * (size_t)kPaeRecs + 4u * (size_t)((P.N + 31) >> 5) + 4u * (size_t)P.A * (size_t)P.Z + 16u;
     AA.pae = (accept_engine == 2 && threads >= 512 && smem + pae_bytes <= smem_budget) ? 1 : 0;
