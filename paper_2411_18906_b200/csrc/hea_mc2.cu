@@ -228,8 +228,9 @@ constexpr int kTeamRounds = 128;            // candidates per thread per window:
                                             // warps and blocks at the window barrier (c4 reject regime, trials/s: 32 rounds 3.9e10,
                                             // 64 4.1e10, 128 4.25e10, 256 4.15e10 -- two more mask registers cost more than they save)
 constexpr int kNullWords = kTeamRounds / 32; // 32-bit words of the per-thread null mask
-// Row of the reject-filter table (one per ordered species pair (p, q)): threshold, X, 2 pad, L[M], Q[M], c'[M] floats.
-__host__ __device__ constexpr int filt_row(int M) { return (4 + 3 * M + 3) & ~3; }
+// Reject-filter table: per ordered species pair (p, q) the elements threshold, X, L[M], Q[M], c'[M] (floats), stored
+// element-major (element e of pair i at [e * M*M + i]) so that lanes with different pairs read different banks.
+__host__ __device__ constexpr int filt_row(int M) { return 2 + 3 * M; }
 
 struct TeamSlot {                 // 64 bytes
     uint32_t seq;                 // team-window number + 1 when the record below is valid
@@ -294,8 +295,8 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     int* s_tab = reinterpret_cast<int*>(s_raw + occ_bytes + ((sizeof(Sh2) + 15) & ~(size_t)15));
     // pipelined accept engine buffers (only when AA.pae): records | dirty bitmap over logical sites | logical offsets [A][Z]
     constexpr int RS = filt_row(M);
-    float* s_ftab = reinterpret_cast<float*>(s_tab + LC::A * ZP);       // [M*M][RS] reject-filter rows (16-byte aligned)
-    PRec* s_prec = reinterpret_cast<PRec*>(s_ftab + MM * RS);
+    float* s_ftab = reinterpret_cast<float*>(s_tab + LC::A * ZP);       // [RS][M*M] reject-filter table, element-major
+    PRec* s_prec = reinterpret_cast<PRec*>(s_ftab + ((MM * RS + 3) & ~3));
     uint32_t* s_dirty = reinterpret_cast<uint32_t*>(s_prec + kPaeRecs);
     int* s_loff = reinterpret_cast<int*>(s_dirty + ((P.N + 31) >> 5));
 
@@ -928,7 +929,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             if (use_filter && !(slack_J == J_cur)) {
                 for (int idx = tid; idx < MM; idx += T) {
                     const int p = idx / M, q = idx - p * M;
-                    float* row = s_ftab + idx * RS;
+                    float* row = s_ftab + idx;                           // element e at row[e * MM]
                     double Cq = 0.0, EC = 0.0;                          // C and the bound of its own error
                     for (int c2 = 0; c2 < MM; ++c2) {
                         const double be = (double)sh.cnt[c2] - sh.nstar[c2];
@@ -953,7 +954,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                         else             { t1 =  2.0 * Wc2(p, r) * b2(p, r); t2 = -2.0 * Wc2(q, r) * b2(q, r); Qr = 2.0 * (Wc2(p, r) + Wc2(q, r));
                                            et = 2.0 * Wc2(p, r) * e2(p, r) + 2.0 * Wc2(q, r) * e2(q, r); }
                         const float Lf = (float)(t1 + t2), Qf = (float)Qr;
-                        row[4 + r] = Lf; row[4 + M + r] = Qf; row[4 + 2 * M + r] = (float)cr;
+                        row[(2 + r) * MM] = Lf; row[(2 + M + r) * MM] = Qf; row[(2 + 2 * M + r) * MM] = (float)cr;
                         A += (fabs(t1) + fabs(t2)) * Fm + Qr * Fm * Fm;
                         B += et * Fm;
                         // a coefficient lost to fp32 underflow or overflow would break the relative-error model
@@ -969,7 +970,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     const double thr = fmax(1.001 * J_cur, 1.0e-18 * Kc.w[0]) - Cq + E;
                     const float thr_f = __double2float_ru(thr);
                     row[0] = (finite && isfinite(thr_f)) ? thr_f : __int_as_float(0x7f800000);   // +inf: nothing is dropped
-                    row[1] = Xf; row[2] = 0.0f; row[3] = 0.0f;
+                    row[MM] = Xf;
                 }
                 slack_J = J_cur;
                 __syncthreads();
@@ -1055,15 +1056,15 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     first_shell(sa, sb, mm0, p, q, F0);
                     bool full = true;
                     if (use_filter) {
-                        const float* row = s_ftab + (p * M + q) * RS;
+                        const float* row = s_ftab + (p * M + q);
                         float acc = 0.0f, D = 0.0f;
 #pragma unroll
                         for (int r2 = 0; r2 < M; ++r2) {
                             const float f = (float)F0[r2];
-                            acc = fmaf(fmaf(row[4 + M + r2], f, row[4 + r2]), f, acc);
-                            D = fmaf(row[4 + 2 * M + r2], f, D);
+                            acc = fmaf(fmaf(row[(2 + M + r2) * MM], f, row[(2 + r2) * MM]), f, acc);
+                            D = fmaf(row[(2 + 2 * M + r2) * MM], f, D);
                         }
-                        acc = fmaf(row[1] * D, D, acc);
+                        acc = fmaf(row[MM] * D, D, acc);
                         full = !(acc > row[0]);
                         if (full) {
                             const uint32_t slot = atomicAdd(&sh.q_n[buf], 1u);
@@ -1319,7 +1320,7 @@ size_t mc2_shared_bytes(int occ_mode, int lattice, const int* L, int M)
     size_t s = ((occ_mode == OCC2_NIB ? (NP + 1) / 2 : NP) + 15) & ~(size_t)15;
     s += (sizeof(Sh2) + 15) & ~(size_t)15;
     s += sizeof(int) * (size_t)A * (lattice == 0 ? zpad<0>() : zpad<1>());
-    s += sizeof(float) * (size_t)M * M * filt_row(M);       // reject-filter rows
+    s += (sizeof(float) * (size_t)M * M * filt_row(M) + 15) & ~(size_t)15;       // reject-filter table
     return (s + 15) & ~(size_t)15;
 }
 
