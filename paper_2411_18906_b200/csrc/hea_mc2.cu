@@ -81,6 +81,8 @@ struct Sh2 {
     // accept engine (8 lanes per candidate)
     MoveRec cand[32];             // improving records of the 32 groups of a round
     int4 wdesc[24];               // accumulator word w -> (int4 index in the offset row, slot mask, shell, side)
+    int4 fs_rd[4];                // first shell without the offset table: per basis index, per group of four, the part of a
+                                  // neighbour's padded-index offset that depends on the site's basis (see Mc2Args::fs_c)
     double g[kSMM], t[kSMM];      // objective constants with a per-lane index
     // two-stage evaluation of long windows: integer pre-filter on shell 1, survivors queued for the full evaluation
     double nstar[64];             // first-shell cell (i, j): n*_ij = (1 - t_ij) / g_ij, the (real) count at which alpha = target
@@ -155,6 +157,23 @@ __device__ __forceinline__ void gather_shell(const uint8_t* __restrict__ s_occ, 
         // bytes 1..3 of a loaded value are zero: selector 0x1140 = (x.b0, y.b0, 0, 0)
         uint32_t w = __byte_perm(__byte_perm(x[0], x[1], 0x1140), __byte_perm(x[2], x[3], 0x1140), 0x5410);
         if (OCC == OCC2_NIB) w = (w >> (o.x & 4)) & 0x0F0F0F0Fu;
+        acc[g] = w;
+    }
+}
+
+// First shell through Mc2Args::fs_c / fs_rd (no offset-table loads): same accumulator words as gather_shell, the groups
+// being the odd-component classes of the lattice vectors.
+template <int OCC, int NA>
+__device__ __forceinline__ void gather_first_direct(const uint8_t* __restrict__ s_occ, const int4 rd, uint32_t pidx,
+                                                    const int (&fc)[12], uint32_t (&acc)[NA])
+{
+#pragma unroll
+    for (int g = 0; g < NA; ++g) {
+        const uint32_t n = pidx + (uint32_t)(g == 0 ? rd.x : g == 1 ? rd.y : rd.z);
+        const uint8_t* base = s_occ + (OCC == OCC2_NIB ? n >> 1 : n);
+        const uint32_t x0 = base[fc[4 * g]], x1 = base[fc[4 * g + 1]], x2 = base[fc[4 * g + 2]], x3 = base[fc[4 * g + 3]];
+        uint32_t w = __byte_perm(__byte_perm(x0, x1, 0x1140), __byte_perm(x2, x3, 0x1140), 0x5410);
+        if (OCC == OCC2_NIB) w = (w >> ((n & 1u) * 4u)) & 0x0F0F0F0Fu;
         acc[g] = w;
     }
 }
@@ -269,6 +288,13 @@ struct Mc2Args {
     int accept_engine;            // 1: single-step windows run on the 8-lanes-per-candidate engine
     int pae;                      // 1: ... pipelined over epochs of steps (record, dirty-bitmap and offset buffers present)
     uint32_t rk[20];              // Philox round keys of the seed (D7): key + r * (0x9E3779B9, 0xBB67AE85), r = 0..9
+    // First shell without the offset table.  A first-shell lattice vector v reaches, from basis offset beta (components
+    // 0/1), the cell shifted by floor(v_d / 2) + beta_d [v_d odd]: the padded-index offset splits into a part that depends
+    // only on v (fs_c: A * cell part, same for every site; stored halved for the nibble layout) and a part that depends
+    // only on the site's basis index and on WHICH components of v are odd (fs_rd[b][group]; the vectors are grouped by
+    // that pattern, four per group).  neighbour = pidx + fs_rd[b][g] + fs_c[g][j]: one add with a constant-bank operand.
+    int fs_c[12];
+    int fs_rd[4][4];
     // hea_mc_run_ex
     int select_best;              // 1: the minimum J_k of a step is taken (ties -> lowest k) instead of the lowest improving k
     unsigned long long depth_limit;        // > 0: a chain stops after this many consecutive steps without a move
@@ -370,6 +396,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         s_tab[i] = entry;
     }
     for (int i = tid; i < SMM; i += T) { sh.g[i] = Kc.g[i]; sh.t[i] = Kc.t[i]; }
+    if (tid < 4) sh.fs_rd[tid] = make_int4(AA.fs_rd[tid][0], AA.fs_rd[tid][1], AA.fs_rd[tid][2], AA.fs_rd[tid][3]);
     for (int i = tid; i < MM; i += T) {
         const double gi = Kc.g[i];
         sh.nstar[i] = (1.0 - Kc.t[i]) / gi;
@@ -1024,8 +1051,8 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             // first-shell species-count differences of a non-null candidate
             auto first_shell = [&](const SiteC& sa, const SiteC& sb, int mm0, int p, int q, int (&F0)[M]) {
                 uint32_t xa[NA0], xb[NA0];
-                gather_shell<OCC, LC::z0>(s_occ, reinterpret_cast<const int4*>(s_tab + sa.b * ZP), sa.pidx, xa);
-                gather_shell<OCC, LC::z0>(s_occ, reinterpret_cast<const int4*>(s_tab + sb.b * ZP), sb.pidx, xb);
+                gather_first_direct<OCC, NA0>(s_occ, sh.fs_rd[sa.b], sa.pidx, AA.fs_c, xa);
+                gather_first_direct<OCC, NA0>(s_occ, sh.fs_rd[sb.b], sb.pidx, AA.fs_c, xb);
                 hist_diff<M, NA0>(xa, xb, F0);
                 if (mm0 != 0) {                                     // a and b are first-shell neighbours (rare): D9.2 exclusion
 #pragma unroll
@@ -1379,6 +1406,32 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
     G.cc = (uint32_t)(P.A * (G.PLy * G.PLz + G.PLz + 1));
     G.pmagy = magic(G.PLy); G.pmagz = magic(G.PLz);
     G.NP = (P.L[0] + 2) * G.PLy * G.PLz * P.A;
+    {
+        // first-shell decomposition (see Mc2Args): groups = vectors with the same neighbour basis seen from basis 0
+        const int A = P.A, Z = P.Z, z0 = P.z[0];
+        auto off = [&](int b, int k) {
+            const int8_t* stn = host_tab.stencil + (b * Z + k) * 4;
+            return (((int)stn[1] * G.PLy + (int)stn[2]) * G.PLz + (int)stn[3]) * A + ((int)stn[0] - b);
+        };
+        int order[24], n_ord = 0;
+        for (int nb = 0; nb < A; ++nb)
+            for (int k = 0; k < z0; ++k)
+                if (host_tab.stencil[(0 * Z + k) * 4] == nb) order[n_ord++] = k;
+        if (n_ord != z0 || z0 > 12 || (z0 & 3)) return cudaErrorInvalidValue;
+        for (int i = 0; i < 12; ++i) AA.fs_c[i] = 0;
+        for (int b = 0; b < 4; ++b) for (int g = 0; g < 4; ++g) AA.fs_rd[b][g] = 0;
+        for (int i = 0; i < z0; ++i) {
+            const int k = order[i], nb0 = host_tab.stencil[(0 * Z + k) * 4];
+            const int c = off(0, k) - nb0;                   // A * (cell part): even
+            if (c & 1) return cudaErrorInvalidValue;
+            AA.fs_c[i] = occ_mode == OCC2_NIB ? c / 2 : c;
+            for (int b = 0; b < A; ++b) {
+                const int rd = off(b, k) - c;
+                if ((i & 3) == 0) AA.fs_rd[b][i >> 2] = rd;
+                else if (AA.fs_rd[b][i >> 2] != rd) return cudaErrorInvalidValue;      // not of the assumed form
+            }
+        }
+    }
     for (int r = 0; r < 10; ++r) {
         AA.rk[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
         AA.rk[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
