@@ -14,6 +14,7 @@
 //  * Whether b is a neighbour of a (the exclusion of D9.2) comes from the lattice coordinates of the two sites
 //    (minimum-image displacement, squared length == shell distance), not from a compare per table entry.
 //  * Shell sizes and the basis count are template constants (fcc 12/6/24, bcc 8/6/12), so every gather is unrolled.
+#include <cstdio>
 #include <cstring>
 #include <type_traits>
 
@@ -81,6 +82,12 @@ struct Sh2 {
     // accept engine (8 lanes per candidate)
     MoveRec cand[32];             // improving records of the 32 groups of a round
     int4 wdesc[24];               // accumulator word w -> (int4 index in the offset row, slot mask, shell, side)
+    uint4 mlog[kPaeRecs / kPaeK]; // serial accept engine: the move of each step of the epoch (a, b, p | q << 8 | 1 << 16, -)
+    uint32_t swe_stop;            //   steps of the epoch consumed so far | (a step needs the candidates beyond kPaeK) << 31
+    uint32_t sbest[3], sstale[3]; //   lowest improving record / mask of stale records of a step, triple-buffered
+    uint32_t sbest2[3];           //   lowest improving REBUILT record of the step
+    uint32_t pad2[2];
+    MoveRec cand2[2][kPaeK];      //   improving records of a step, by step parity (the role warps read one step behind)
     int4 fs_rd[4];                // first shell without the offset table: per basis index, per group of four, the part of a
                                   // neighbour's padded-index offset that depends on the site's basis (see Mc2Args::fs_c)
     double g[kSMM], t[kSMM];      // objective constants with a per-lane index
@@ -287,6 +294,7 @@ struct Mc2Args {
     int team_on, team_off;        // enter TEAM when W*K >= team_on; leave it after a move with steps_done*K < team_off
     int accept_engine;            // 1: single-step windows run on the 8-lanes-per-candidate engine
     int pae;                      // 1: ... pipelined over epochs of steps (record, dirty-bitmap and offset buffers present)
+    uint32_t k_mq, k_sq;          // candidate index / K = umulhi(index, k_mq) >> k_sq (K >= 2)
     uint32_t rk[20];              // Philox round keys of the seed (D7): key + r * (0x9E3779B9, 0xBB67AE85), r = 0..9
     // First shell without the offset table.  A first-shell lattice vector v reaches, from basis offset beta (components
     // 0/1), the cell shifted by floor(v_d / 2) + beta_d [v_d odd]: the padded-index offset splits into a part that depends
@@ -462,6 +470,38 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     unsigned long long depth = (depth_limit && AA.depth_all) ? AA.depth_all[chain_local] : 0ull;
     const bool accept_ok = T >= 512 && AA.accept_engine != 0 && !best_mode;   // 8 evaluating warps + null-settling warps
 
+    // one-hot code of a site and of its ghost images (only cells on the boundary have any)
+    auto write_site = [&](uint32_t u, uint32_t code) {
+        const SiteC sc = decode_site<LAT>(G, u);
+        if (sc.x >= 1 && sc.x <= Lx - 2 && sc.y >= 1 && sc.y <= Ly - 2 && sc.z >= 1 && sc.z <= Lz - 2) {
+            occ_set<OCC>(s_occ, sc.pidx, code);               // interior cell: no ghost image
+        } else {
+            const int px[3] = {sc.x + 1, sc.x == Lx - 1 ? 0 : -1, sc.x == 0 ? Lx + 1 : -1};
+            const int py[3] = {sc.y + 1, sc.y == Ly - 1 ? 0 : -1, sc.y == 0 ? Ly + 1 : -1};
+            const int pz[3] = {sc.z + 1, sc.z == Lz - 1 ? 0 : -1, sc.z == 0 ? Lz + 1 : -1};
+            for (int ix = 0; ix < 3; ++ix)
+                for (int iy = 0; iy < 3; ++iy)
+                    for (int iz = 0; iz < 3; ++iz) {
+                        if (px[ix] < 0 || py[iy] < 0 || pz[iz] < 0) continue;
+                        const uint32_t pi = (uint32_t)((((px[ix] * G.PLy + py[iy]) * G.PLz + pz[iz]) << LC::lgA) | sc.b);
+                        occ_set<OCC>(s_occ, pi, code);
+                    }
+        }
+    };
+    // the two sites of a move and all their neighbours are now "touched" (pipelined accept engine); lanes 0..31 of one warp
+    auto mark_one = [&](uint32_t u, int lane) {
+        const SiteC sc = decode_site<LAT>(G, u);
+        const bool interior = sc.x >= 1 && sc.x <= Lx - 2 && sc.y >= 1 && sc.y <= Ly - 2 && sc.z >= 1 && sc.z <= Lz - 2;
+        for (int e = lane; e < P.Z; e += 32) {
+            const uint32_t v = interior ? u + (uint32_t)s_loff[sc.b * P.Z + e] : (uint32_t)__ldg(P.nbr_site + (size_t)u * P.Z + e);
+            atomicOr(&s_dirty[v >> 5], 1u << (v & 31u));
+        }
+        if (lane == 0) atomicOr(&s_dirty[u >> 5], 1u << (u & 31u));
+    };
+    auto mark_touched = [&](uint32_t ma, uint32_t mb, int lane) {
+        mark_one(ma, lane);
+        mark_one(mb, lane);
+    };
     // D9.4: apply an accepted move in every thread of the block (counts by the first S*M*M threads, the swap with its
     // ghost images by thread T-1, bookkeeping by thread T-2); ends with a barrier.
     auto apply_move = [&](const MoveRec* mv, uint32_t kk, unsigned long long step) {
@@ -473,41 +513,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             sh.cnt[idx] += ci * Pack<M>::field(d, jj) + cj * Pack<M>::field(d, i);
         }
         if (tid == T - 1) {
-#pragma unroll 1
-            for (int which = 0; which < 2; ++which) {
-                const SiteC sc = decode_site<LAT>(G, which ? mv->b : mv->a);
-                const uint32_t code = 1u << (which ? p : q);
-                if (sc.x >= 1 && sc.x <= Lx - 2 && sc.y >= 1 && sc.y <= Ly - 2 && sc.z >= 1 && sc.z <= Lz - 2) {
-                    occ_set<OCC>(s_occ, sc.pidx, code);       // interior cell: no ghost image
-                } else {
-                    const int px[3] = {sc.x + 1, sc.x == Lx - 1 ? 0 : -1, sc.x == 0 ? Lx + 1 : -1};
-                    const int py[3] = {sc.y + 1, sc.y == Ly - 1 ? 0 : -1, sc.y == 0 ? Ly + 1 : -1};
-                    const int pz[3] = {sc.z + 1, sc.z == Lz - 1 ? 0 : -1, sc.z == 0 ? Lz + 1 : -1};
-                    for (int ix = 0; ix < 3; ++ix)
-                        for (int iy = 0; iy < 3; ++iy)
-                            for (int iz = 0; iz < 3; ++iz) {
-                                if (px[ix] < 0 || py[iy] < 0 || pz[iz] < 0) continue;
-                                const uint32_t pi = (uint32_t)((((px[ix] * G.PLy + py[iy]) * G.PLz + pz[iz]) << LC::lgA) | sc.b);
-                                occ_set<OCC>(s_occ, pi, code);
-                            }
-                }
-            }
+            write_site(mv->a, 1u << q);
+            write_site(mv->b, 1u << p);
         }
-        if (AA.pae && tid >= 32 && tid < 64) {
-            // pipelined accept engine: the two sites and all their neighbours are now "touched"
-            const int lane = tid - 32;
-#pragma unroll 1
-            for (int which = 0; which < 2; ++which) {
-                const uint32_t u = which ? mv->b : mv->a;
-                const SiteC sc = decode_site<LAT>(G, u);
-                const bool interior = sc.x >= 1 && sc.x <= Lx - 2 && sc.y >= 1 && sc.y <= Ly - 2 && sc.z >= 1 && sc.z <= Lz - 2;
-                for (int e = lane; e < P.Z; e += 32) {
-                    const uint32_t v = interior ? u + (uint32_t)s_loff[sc.b * P.Z + e] : (uint32_t)__ldg(nbr + (size_t)u * P.Z + e);
-                    atomicOr(&s_dirty[v >> 5], 1u << (v & 31u));
-                }
-                if (lane == 0) atomicOr(&s_dirty[u >> 5], 1u << (u & 31u));
-            }
-        }
+        if (AA.pae && tid >= 32 && tid < 64) mark_touched(mv->a, mv->b, tid - 32);
         if (tid == T - 2) {
             const uint32_t a = mv->a, b = mv->b;
             sh.J = mv->J;
@@ -696,6 +705,46 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         }
         return Jk;
     };
+    // the same with the counts of this lane's rows in registers (serial accept engine)
+    auto g8_Jr = [&](const int (&cntr)[NRR][M], const int (&c)[M], int p, int q, const int (&F0)[M], const int (&F1)[M],
+                     const int (&F2)[M]) -> double {
+        const int l8 = tid & 7;
+        double rowv[NRR];
+#pragma unroll
+        for (int rr = 0; rr < NRR; ++rr) {
+            const int rho = l8 + 8 * rr;
+            double row = 0.0;
+            if (rho < S * M) {
+                const int s = rho / M, i = rho - s * M;
+                const int ci = (i == p) - (i == q);
+                int Fi = 0;
+#pragma unroll
+                for (int j = 0; j < M; ++j) { const int Fj = s == 0 ? F0[j] : s == 1 ? F1[j] : F2[j]; Fi = j == i ? Fj : Fi; }
+#pragma unroll
+                for (int j = 0; j < M; ++j) {
+                    const int Fj = s == 0 ? F0[j] : s == 1 ? F1[j] : F2[j];
+                    const int n = cntr[rr][j] + ci * Fj + c[j] * Fi;
+                    row = __dadd_rn(row, sq_dev(n, sh.g[rho * M + j], sh.t[rho * M + j]));
+                }
+            }
+            rowv[rr] = row;
+        }
+        double Jk = 0.0;
+#pragma unroll
+        for (int s = 0; s < 3; ++s) {
+            if (s < S) {
+                double shs = 0.0;
+#pragma unroll
+                for (int i = 0; i < M; ++i) {
+                    const int rho = s * M + i;
+                    const double v = __shfl_sync(0xFFFFFFFFu, rowv[rho >> 3], (tid & 24) | (rho & 7));
+                    shs = __dadd_rn(shs, v);
+                }
+                Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[s], shs));
+            }
+        }
+        return Jk;
+    };
     auto g8_post = [&](bool live, double Jk, double J_cur, uint32_t k, uint32_t a, uint32_t b, int p, int q,
                        const int (&F0)[M], const int (&F1)[M], const int (&F2)[M], int grp, int buf) {
         const int l8 = tid & 7;
@@ -720,6 +769,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         g8_post(live, Jk, J_cur, k, a, b, p, q, F0, F1, F2, grp, buf);
     };
 
+#ifdef HEA_DBG
+    __shared__ long long dbg_t[16];
+    if (tid < 16) dbg_t[tid] = 0;
+#endif
     unsigned long long t0 = A.step0;
     const unsigned long long t_end = A.step0 + A.n_steps;
     uint32_t W = 1;
@@ -752,119 +805,249 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         }
         uint32_t key_best = kNoKey, steps_done = 1u;
         if (accept_ok && !team && W == 1u && AA.pae) {
-            // ---- pipelined accept engine.  In the accept regime nearly every step applies a move found among its first
-            // few candidates, and a step is one candidate evaluation long.  What depends only on the configuration
-            // (proposal, adjacency, the 2Z gathers) is therefore computed AHEAD for an epoch of T / 16 steps x 16
-            // candidates, one record per thread; the serial part of a step is the objective of those records against
-            // the current counts (8 lanes per record), the selection, and the move.  A record is stale once a move has
-            // touched one of its drawn sites or one of their neighbours: every move marks its two sites and their
-            // neighbours in a bitmap, and a warp that meets a stale record recomputes its records from the current
-            // configuration.  Steps whose first 16 candidates do not improve fall back to rounds of 32 candidates.
+            // ---- serial accept engine.  In the accept regime nearly every step applies a move found among its first few
+            // candidates, so a chain advances one dependent move at a time and what counts is the latency of a step.
+            // (P) What depends only on the configuration (proposal, adjacency, the 2Z gathers) is computed AHEAD for an
+            //     epoch of T / 16 steps x 16 candidates by the whole block, one record per thread.
+            // (S) FOUR warps (16 records x 8 lanes) then run the steps of the epoch, synchronised among themselves by a
+            //     named barrier while the other warps wait: the objective of the records against the current counts, the
+            //     lowest improving candidate, then counts, configuration, bitmap and bookkeeping dealt over the four
+            //     warps.  A record is stale once a move has touched one of its drawn sites or one of their neighbours (a
+            //     bitmap marked by every move); stale records below the first improving one are rebuilt from the
+            //     current configuration.  A step whose first 16 candidates do not improve goes to the whole block
+            //     (rounds of 32 candidates, 8 lanes each).
+            // (N) The null candidates of the consumed steps (all K count, D9.1) are settled afterwards by the whole
+            //     block against the final configuration, sites touched by moves of the epoch being traced back
+            //     through the epoch's move log.
             const uint32_t n_ep = (uint32_t)min((unsigned long long)(T / kPaeK), t_end - t0);
-            {
-                const uint32_t es = (uint32_t)tid / (uint32_t)kPaeK, k = (uint32_t)tid % (uint32_t)kPaeK;
-                if ((uint32_t)tid < n_ep * (uint32_t)kPaeK) {
-                    PRec rec;
-                    rec.pad = 0; rec.d0 = rec.d1 = rec.d2 = 0ull; rec.a = rec.b = rec.a1 = rec.b1 = 0u;
-                    rec.pqn = 1u << 17;                                   // absent (k >= K)
-                    if (k < (uint32_t)K) {
-                        uint32_t a, b, hp, hq, a1, b1;
-                        SiteC sa, sb;
-                        propose2(t0 + es, k, a, b, sa, sb, hp, hq, a1, b1);
-                        rec.a = a; rec.b = b; rec.a1 = a1; rec.b1 = b1;
-                        if (hp == hq) {
-                            rec.pqn = 1u << 16;                           // null
-                        } else {
-                            const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
-                            int c[M], F0[M], F1[M], F2[M];
+            const unsigned long long t_ep = t0;
+#ifdef HEA_DBG
+            long long dbg_c0 = clock64();
+#endif
+            auto build_record = [&](unsigned long long step, uint32_t k) -> PRec {
+                PRec rec;
+                rec.pad = 0; rec.d0 = rec.d1 = rec.d2 = 0ull; rec.a = rec.b = rec.a1 = rec.b1 = 0u;
+                rec.pqn = 1u << 17;                                   // absent (k >= K)
+                if (k < (uint32_t)K) {
+                    uint32_t a, b, hp, hq, a1, b1;
+                    SiteC sa, sb;
+                    propose2(step, k, a, b, sa, sb, hp, hq, a1, b1);
+                    rec.a = a; rec.b = b; rec.a1 = a1; rec.b1 = b1;
+                    if (hp == hq) {
+                        rec.pqn = 1u << 16;                           // null
+                    } else {
+                        const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+                        int c[M], F0[M], F1[M], F2[M];
 #pragma unroll
-                            for (int r2 = 0; r2 < M; ++r2) { c[r2] = (r2 == p) - (r2 == q); F1[r2] = 0; F2[r2] = 0; }
-                            int mm0, mm1, mm2;
-                            adjacency(a, b, sa, sb, mm0, mm1, mm2);
-                            const int4* ta = reinterpret_cast<const int4*>(s_tab + sa.b * ZP);
-                            const int4* tb = reinterpret_cast<const int4*>(s_tab + sb.b * ZP);
-                            {
-                                uint32_t xa[NA0], xb[NA0];
-                                gather_shell<OCC, LC::z0>(s_occ, ta, sa.pidx, xa);
-                                gather_shell<OCC, LC::z0>(s_occ, tb, sb.pidx, xb);
-                                hist_diff<M, NA0>(xa, xb, F0);
-                            }
-                            if (S > 1) {
-                                uint32_t xa[NA1], xb[NA1];
-                                gather_shell<OCC, LC::z1>(s_occ, ta + NA0, sa.pidx, xa);
-                                gather_shell<OCC, LC::z1>(s_occ, tb + NA0, sb.pidx, xb);
-                                hist_diff<M, NA1>(xa, xb, F1);
-                            }
-                            if (S > 2) {
-                                uint32_t xa[NA2], xb[NA2];
-                                gather_shell<OCC, LC::z2>(s_occ, ta + NA0 + NA1, sa.pidx, xa);
-                                gather_shell<OCC, LC::z2>(s_occ, tb + NA0 + NA1, sb.pidx, xb);
-                                hist_diff<M, NA2>(xa, xb, F2);
-                            }
-#pragma unroll
-                            for (int r2 = 0; r2 < M; ++r2) { F0[r2] -= mm0 * c[r2]; F1[r2] -= mm1 * c[r2]; F2[r2] -= mm2 * c[r2]; }
-                            rec.pqn = (uint32_t)p | ((uint32_t)q << 8);
-                            rec.d0 = (unsigned long long)pack_F<M>(F0); rec.d1 = (unsigned long long)pack_F<M>(F1);
-                            rec.d2 = (unsigned long long)pack_F<M>(F2);
-                        }
-                    }
-                    s_prec[tid] = rec;
-                }
-            }
-            __syncthreads();
-            bool any_move = false;
-            for (uint32_t es = 0; es < n_ep; ++es) {
-                const double J_cur = sh.J;
-                if (tid >= 256) {                                        // which of the K candidates of this step are null
-                    for (uint32_t k = (uint32_t)tid - 256u; k < (uint32_t)K; k += (uint32_t)T - 256u) {
-                        uint32_t a, b, hp, hq;
-                        SiteC sa, sb;
-                        propose(t0, k, a, b, sa, sb, hp, hq);
-                        my_null += hp == hq;
-                    }
-                }
-                int buf = (int)(it % 3u);
-                if (tid < kPaeK * 8) {
-                    const int grp = tid >> 3;
-                    const PRec rec = s_prec[es * kPaeK + grp];
-                    auto dirty = [&](uint32_t v) { return (s_dirty[v >> 5] >> (v & 31u)) & 1u; };
-                    const bool absent = (rec.pqn >> 17) & 1u;
-                    const bool stale = !absent && (dirty(rec.a) | dirty(rec.b) | dirty(rec.a1) | dirty(rec.b1));
-                    uint32_t a = rec.a, b = rec.b;
-                    bool live = !absent && !((rec.pqn >> 16) & 1u);
-                    int p = (int)(rec.pqn & 0xFFu), q = (int)((rec.pqn >> 8) & 0xFFu);
-                    int c[M], F0[M], F1[M], F2[M];
-                    if (__any_sync(0xFFFFFFFFu, stale)) {                // recompute this warp's four records
-                        uint32_t hp, hq;
-                        SiteC sa, sb;
-                        propose(t0, (uint32_t)grp, a, b, sa, sb, hp, hq);
-                        live = !absent && hp != hq;
-                        p = 31 - __clz((int)hp); q = 31 - __clz((int)hq);
+                        for (int r2 = 0; r2 < M; ++r2) { c[r2] = (r2 == p) - (r2 == q); F1[r2] = 0; F2[r2] = 0; }
                         int mm0, mm1, mm2;
                         adjacency(a, b, sa, sb, mm0, mm1, mm2);
-                        g8_F(sa, sb, mm0, mm1, mm2, p, q, c, F0, F1, F2);
-                    } else {
+                        const int4* ta = reinterpret_cast<const int4*>(s_tab + sa.b * ZP);
+                        const int4* tb = reinterpret_cast<const int4*>(s_tab + sb.b * ZP);
+                        {
+                            uint32_t xa[NA0], xb[NA0];
+                            gather_shell<OCC, LC::z0>(s_occ, ta, sa.pidx, xa);
+                            gather_shell<OCC, LC::z0>(s_occ, tb, sb.pidx, xb);
+                            hist_diff<M, NA0>(xa, xb, F0);
+                        }
+                        if (S > 1) {
+                            uint32_t xa[NA1], xb[NA1];
+                            gather_shell<OCC, LC::z1>(s_occ, ta + NA0, sa.pidx, xa);
+                            gather_shell<OCC, LC::z1>(s_occ, tb + NA0, sb.pidx, xb);
+                            hist_diff<M, NA1>(xa, xb, F1);
+                        }
+                        if (S > 2) {
+                            uint32_t xa[NA2], xb[NA2];
+                            gather_shell<OCC, LC::z2>(s_occ, ta + NA0 + NA1, sa.pidx, xa);
+                            gather_shell<OCC, LC::z2>(s_occ, tb + NA0 + NA1, sb.pidx, xb);
+                            hist_diff<M, NA2>(xa, xb, F2);
+                        }
 #pragma unroll
-                        for (int r2 = 0; r2 < M; ++r2) {
-                            c[r2] = live ? (r2 == p) - (r2 == q) : 0;
-                            F0[r2] = Pack<M>::field((PW)rec.d0, r2); F1[r2] = Pack<M>::field((PW)rec.d1, r2);
-                            F2[r2] = Pack<M>::field((PW)rec.d2, r2);
+                        for (int r2 = 0; r2 < M; ++r2) { F0[r2] -= mm0 * c[r2]; F1[r2] -= mm1 * c[r2]; F2[r2] -= mm2 * c[r2]; }
+                        rec.pqn = (uint32_t)p | ((uint32_t)q << 8);
+                        rec.d0 = (unsigned long long)pack_F<M>(F0); rec.d1 = (unsigned long long)pack_F<M>(F1);
+                        rec.d2 = (unsigned long long)pack_F<M>(F2);
+                    }
+                }
+                return rec;
+            };
+            if ((uint32_t)tid < n_ep * (uint32_t)kPaeK)
+                s_prec[tid] = build_record(t0 + (uint32_t)tid / (uint32_t)kPaeK, (uint32_t)tid % (uint32_t)kPaeK);
+            if (tid < kPaeRecs / kPaeK) sh.mlog[tid] = make_uint4(0u, 0u, 0u, 0u);
+            __syncthreads();
+#ifdef HEA_DBG
+            long long dbg_c1 = clock64();
+            if (tid == 0) dbg_t[0] += dbg_c1 - dbg_c0;
+#endif
+            uint32_t e_done = 0;                                         // steps of the epoch consumed
+            bool leave = false;
+            while (e_done < n_ep && !leave) {
+                // warps 0-3 (EVAL): 16 records x 8 lanes, the pair counts of a lane's objective rows in registers.
+                // warps 4-7 (ROLES): what a move changes besides the counts -- touched-site bitmap (warps 4, 5), the swap
+                // with its ghost images (warp 6), shared counts, J, hash, logs (warp 7) -- one step behind the evaluation.
+                // Named barriers: 2 = "bitmap and configuration of the previous move are in place" (roles arrive, eval
+                // waits), 3 = "selection of this step posted" (all eight warps), 4 = the same after rebuilt records.
+                if (tid < 256) {
+                    const bool is_eval = tid < 128;
+                    const int grp = (tid >> 3) & 15, l8 = tid & 7;
+                    auto dirty = [&](uint32_t v) { return (s_dirty[v >> 5] >> (v & 31u)) & 1u; };
+                    int cntr[NRR][M];                                    // EVAL: counts of rows l8 + 8 rr
+#pragma unroll
+                    for (int rr = 0; rr < NRR; ++rr) {
+                        const int rho = l8 + 8 * rr;
+#pragma unroll
+                        for (int j = 0; j < M; ++j) cntr[rr][j] = (is_eval && rho < S * M) ? sh.cnt[rho * M + j] : 0;
+                    }
+                    double J_cur = sh.J;
+                    if (tid < 3) { sh.sbest[tid] = kNoKey; sh.sbest2[tid] = kNoKey; sh.sstale[tid] = 0u; }
+                    asm volatile("bar.sync 4, 256;" ::: "memory");
+                    if (!is_eval && tid < 224) asm volatile("bar.arrive 2, 224;" ::: "memory");
+                    uint32_t es = e_done, pend = 0u, sit = 0u;
+                    bool moved = false;
+                    for (; es < n_ep; ++es, ++sit) {
+                        const int sb = (int)(sit % 3u), par = (int)(sit & 1u);
+                        const unsigned long long step = t_ep + es;
+                        PRec rec;
+                        uint32_t a = 0, b = 0;
+                        bool absent = true, live = false;
+                        int p = 0, q = 0;
+                        int c[M], F0[M], F1[M], F2[M];
+                        double Jk = 0.0;
+                        if (is_eval) {
+                            rec = s_prec[es * kPaeK + grp];
+                            absent = (rec.pqn >> 17) & 1u;
+                            a = rec.a; b = rec.b;
+                            live = !absent && !((rec.pqn >> 16) & 1u);
+                            p = (int)(rec.pqn & 0xFFu); q = (int)((rec.pqn >> 8) & 0xFFu);
+#pragma unroll
+                            for (int r2 = 0; r2 < M; ++r2) {
+                                c[r2] = live ? (r2 == p) - (r2 == q) : 0;
+                                F0[r2] = Pack<M>::field((PW)rec.d0, r2); F1[r2] = Pack<M>::field((PW)rec.d1, r2);
+                                F2[r2] = Pack<M>::field((PW)rec.d2, r2);
+                            }
+                            Jk = g8_Jr(cntr, c, p, q, F0, F1, F2);
+                            asm volatile("bar.sync 2, 224;" ::: "memory");       // the previous move is in the bitmap
+                            const bool stale = !absent && (dirty(rec.a) | dirty(rec.b) | dirty(rec.a1) | dirty(rec.b1));
+                            if (l8 == 0) {
+                                if (stale) {
+                                    atomicOr(&sh.sstale[sb], 1u << grp);
+                                } else if (live && Jk < J_cur) {
+                                    MoveRec& m = sh.cand2[par][grp];
+                                    m.key = (uint32_t)grp; m.a = a; m.b = b; m.pq = (uint32_t)p | ((uint32_t)q << 8); m.J = Jk;
+                                    m.d[0] = rec.d0; m.d[1] = rec.d1; m.d[2] = rec.d2;
+                                    atomicMin(&sh.sbest[sb], (uint32_t)grp);
+                                }
+                            }
+                        }
+                        asm volatile("bar.sync 3, 256;" ::: "memory");           // selection posted
+                        uint32_t kb = sh.sbest[sb];
+                        const uint32_t sm = sh.sstale[sb];
+                        // stale records below the first improving fresh one decide the step: their warps rebuild their
+                        // four records from the current configuration (8 lanes per record) and evaluate again
+                        const uint32_t need = sm & (kb == kNoKey ? 0xFFFFFFFFu : ((1u << kb) - 1u));
+                        if (need) {
+                            if (is_eval && ((need >> (grp & ~3)) & 0xFu)) {
+                                uint32_t hp, hq;
+                                SiteC sa, sb2;
+                                propose(step, (uint32_t)grp, a, b, sa, sb2, hp, hq);
+                                live = !absent && hp != hq;
+                                p = 31 - __clz((int)hp); q = 31 - __clz((int)hq);
+                                int mm0, mm1, mm2;
+                                adjacency(a, b, sa, sb2, mm0, mm1, mm2);
+                                g8_F(sa, sb2, mm0, mm1, mm2, p, q, c, F0, F1, F2);
+                                if (!live) {
+#pragma unroll
+                                    for (int r2 = 0; r2 < M; ++r2) c[r2] = 0;
+                                }
+                                Jk = g8_Jr(cntr, c, p, q, F0, F1, F2);
+                                if (l8 == 0 && live && Jk < J_cur) {
+                                    MoveRec& m = sh.cand2[par][grp];
+                                    m.key = (uint32_t)grp; m.a = a; m.b = b; m.pq = (uint32_t)p | ((uint32_t)q << 8); m.J = Jk;
+                                    m.d[0] = pack_F<M>(F0); m.d[1] = pack_F<M>(F1); m.d[2] = pack_F<M>(F2);
+                                    atomicMin(&sh.sbest2[sb], (uint32_t)grp);     // (a slot of its own: barrier 3 readers still compare sbest)
+                                }
+                            }
+                            asm volatile("bar.sync 4, 256;" ::: "memory");
+                            kb = min(kb, sh.sbest2[sb]);
+                        }
+                        if (tid == 255) { sh.sbest[(sb + 2) % 3] = kNoKey; sh.sbest2[(sb + 2) % 3] = kNoKey; sh.sstale[(sb + 2) % 3] = 0u; }
+                        if (kb == kNoKey) { pend = 1u; break; }
+                        moved = true;
+                        const MoveRec* mv = &sh.cand2[par][kb];
+                        const int wp = (int)(mv->pq & 0xFFu), wq = (int)(mv->pq >> 8);
+                        if (is_eval) {
+                            // D9.4 on the register copy of this lane's rows
+                            J_cur = mv->J;
+#pragma unroll
+                            for (int rr = 0; rr < NRR; ++rr) {
+                                const int rho = l8 + 8 * rr;
+                                if (rho < S * M) {
+                                    const int s2 = rho / M, i = rho - s2 * M;
+                                    const PW d = (PW)mv->d[s2];
+                                    const int ci = (i == wp) - (i == wq);
+                                    const int Fi = Pack<M>::field(d, i);
+#pragma unroll
+                                    for (int j = 0; j < M; ++j)
+                                        cntr[rr][j] += ci * Pack<M>::field(d, j) + ((j == wp) - (j == wq)) * Fi;
+                                }
+                            }
+                        } else if (tid < 192) {                          // warps 4, 5: neighbourhoods of a and of b
+                            mark_one(tid < 160 ? mv->a : mv->b, tid & 31);
+                            asm volatile("bar.arrive 2, 224;" ::: "memory");
+                        } else if (tid < 224) {                          // warp 6: the swap (one lane: a and b may share a byte)
+                            if (tid == 192) { write_site(mv->a, 1u << wq); write_site(mv->b, 1u << wp); }
+                            asm volatile("bar.arrive 2, 224;" ::: "memory");
+                        } else {                                         // warp 7: shared counts and bookkeeping
+                            for (int idx = tid - 224; idx < SMM; idx += 32) {
+                                const int s2 = idx / MM, rem = idx - s2 * MM, i = rem / M, jj = rem - i * M;
+                                const PW d = (PW)mv->d[s2];
+                                const int ci = (i == wp) - (i == wq), cj = (jj == wp) - (jj == wq);
+                                sh.cnt[idx] += ci * Pack<M>::field(d, jj) + cj * Pack<M>::field(d, i);
+                            }
+                            if (tid == 224) {
+                                const uint32_t wa = mv->a, wb = mv->b;
+                                sh.J = mv->J;
+                                sh.n_accept += 1;
+                                sh.last_accept = step;
+                                unsigned long long hsh = sh.hash;
+                                hsh = (hsh ^ (uint32_t)step) * 0x100000001b3ULL;
+                                hsh = (hsh ^ (uint32_t)(step >> 32)) * 0x100000001b3ULL;
+                                hsh = (hsh ^ kb) * 0x100000001b3ULL;
+                                hsh = (hsh ^ wa) * 0x100000001b3ULL;
+                                hsh = (hsh ^ wb) * 0x100000001b3ULL;
+                                sh.hash = hsh;
+                                sh.mlog[es] = make_uint4(wa, wb, mv->pq | (1u << 16), 0u);
+                                const unsigned long long nl = sh.n_logged;
+                                if (rank == 0 && A.log_all != nullptr && (long long)nl < A.log_cap) {
+                                    unsigned long long* lr = A.log_all + (chain_local * (size_t)A.log_cap + nl) * 3;
+                                    lr[0] = step;
+                                    lr[1] = (unsigned long long)kb | ((unsigned long long)wa << 32);
+                                    lr[2] = (unsigned long long)wb;
+                                }
+                                sh.n_logged = nl + 1;
+                            }
                         }
                     }
-                    const double Jk = g8_J(c, p, q, F0, F1, F2);
-                    g8_post(live, Jk, J_cur, (uint32_t)grp, a, b, p, q, F0, F1, F2, grp, buf);
+                    // barrier 2 is left balanced: one arrival is outstanding unless the loop stopped at a step without a move
+                    if (is_eval && !pend) asm volatile("bar.sync 2, 224;" ::: "memory");
+                    if (tid == 0) sh.swe_stop = es | (pend << 31);
+                    (void)moved;
                 }
                 __syncthreads();
-                key_best = sh.best[buf];
-                if (tid == 0) { sh.best[(buf + 2) % 3] = kNoKey; sh.q_n[(buf + 2) % 3] = 0u; }
-                ++it;
-                uint32_t rd0 = 0;
-                if (key_best == kNoKey) {                                // none of the first 16: the other candidates
-                    for (rd0 = (uint32_t)kPaeK; rd0 < (uint32_t)K; rd0 += 32u) {
-                        buf = (int)(it % 3u);
+                const uint32_t st = sh.swe_stop;
+                if ((st & 0x7FFFFFFFu) > e_done) depth = 0;              // every step the serial engine consumed applied a move
+                e_done = st & 0x7FFFFFFFu;
+                if (st >> 31) {
+                    // step t_ep + e_done: none of the first kPaeK candidates improves -> the others, rounds of 32 on 8 warps
+                    const unsigned long long tstep = t_ep + e_done;
+                    const double J_cur = sh.J;
+                    uint32_t rd0 = (uint32_t)kPaeK;
+                    key_best = kNoKey;
+                    for (; rd0 < (uint32_t)K; rd0 += 32u) {
+                        const int buf = (int)(it % 3u);
                         if (tid < 256) {
                             const uint32_t k = rd0 + ((uint32_t)tid >> 3);
-                            eval_g8(t0, k, k < (uint32_t)K, tid >> 3, buf, J_cur);
+                            eval_g8(tstep, k, k < (uint32_t)K, tid >> 3, buf, J_cur);
                         }
                         __syncthreads();
                         key_best = sh.best[buf];
@@ -872,23 +1055,79 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                         ++it;
                         if (key_best != kNoKey) break;
                     }
-                }
-                if (key_best != kNoKey) {
-                    apply_move(&sh.cand[key_best - rd0], key_best, t0);
-                    any_move = true;
-                    depth = 0;
-                    t0 += 1;
-                } else {
-                    W = min(2u, w_cap);
-                    depth += 1;
-                    t0 += 1;
-                    break;
+                    if (key_best != kNoKey) {
+                        const MoveRec* mv = &sh.cand[key_best - rd0];
+                        if (tid == 0) sh.mlog[e_done] = make_uint4(mv->a, mv->b, mv->pq | (1u << 16), 0u);
+                        apply_move(mv, key_best, tstep);                 // ends with a barrier
+                        depth = 0;
+                    } else {
+                        W = min(2u, w_cap);
+                        depth += 1;
+                        leave = true;
+                    }
+                    e_done += 1;
                 }
             }
-            if (any_move) {                                              // new epoch, clean bitmap
+#ifdef HEA_DBG
+            long long dbg_c2 = clock64();
+            if (tid == 0) { dbg_t[1] += dbg_c2 - dbg_c1; dbg_t[10] += e_done; }
+#endif
+            // ---- (N) null candidates of the e_done consumed steps, all K of each.  The species of a drawn site at its
+            // step is the final one unless a move of the epoch touched the site (the bitmap says so, conservatively):
+            // then the moves from the end of the epoch back to that step are undone for this site.
+            {
+                static_assert(kPaeRecs / kPaeK == 32, "the epoch's move log is scanned one entry per lane");
+                const uint32_t n_cand = e_done * (uint32_t)K;
+                const int lane = tid & 31;
+                const uint4 my_log = sh.mlog[lane];
+                const bool my_log_valid = ((my_log.z >> 16) & 1u) && (uint32_t)lane < e_done;
+                // species code of `site` as step e_at saw it; every lane of the warp takes part
+                auto species_at = [&](uint32_t site, uint32_t e_at) -> uint32_t {
+                    uint32_t code = occ_get<OCC>(s_occ, decode_site<LAT>(G, site).pidx);
+                    uint32_t todo = __ballot_sync(0xFFFFFFFFu, ((s_dirty[site >> 5] >> (site & 31u)) & 1u) != 0u);
+                    while (todo) {                                   // flagged lanes, one at a time: 32 lanes x 32 log entries
+                        const int src = __ffs((int)todo) - 1;
+                        todo &= todo - 1u;
+                        const uint32_t s_site = __shfl_sync(0xFFFFFFFFu, site, src), s_e = __shfl_sync(0xFFFFFFFFu, e_at, src);
+                        const bool in_range = my_log_valid && (uint32_t)lane >= s_e;
+                        const uint32_t hit_a = __ballot_sync(0xFFFFFFFFu, in_range && my_log.x == s_site);
+                        const uint32_t hit_b = __ballot_sync(0xFFFFFFFFu, in_range && my_log.y == s_site);
+                        if (hit_a | hit_b) {
+                            // the earliest move at or after e_at that touches the site: before it, a held p and b held q
+                            const int e2 = __ffs((int)(hit_a | hit_b)) - 1;
+                            const uint32_t pq2 = __shfl_sync(0xFFFFFFFFu, my_log.z, e2);
+                            const uint32_t c2 = ((hit_a >> e2) & 1u) ? 1u << (pq2 & 0xFFu) : 1u << ((pq2 >> 8) & 0xFFu);
+                            if (lane == src) code = c2;
+                        }
+                    }
+                    return code;
+                };
+                const uint32_t n_iter = (n_cand + (uint32_t)T - 1u) / (uint32_t)T;
+                for (uint32_t i2 = 0; i2 < n_iter; ++i2) {
+                    const uint32_t cnd0 = i2 * (uint32_t)T + (uint32_t)tid;
+                    const bool valid = cnd0 < n_cand;
+                    const uint32_t cnd = valid ? cnd0 : 0u;
+                    const uint32_t e_at = K == 1 ? cnd : __umulhi(cnd, AA.k_mq) >> AA.k_sq, k = cnd - e_at * (uint32_t)K;
+                    const unsigned long long step = t_ep + e_at;
+                    const uint4 r = philox4x32_10_rk((uint32_t)step, (uint32_t)(step >> 32), k, chain, AA.rk);
+                    uint32_t a1 = __umulhi(r.x, (uint32_t)N), b1 = __umulhi(r.y, (uint32_t)N - 1u);
+                    b1 += (b1 >= a1);
+                    uint32_t a2 = __umulhi(r.z, (uint32_t)N), b2 = __umulhi(r.w, (uint32_t)N - 1u);
+                    b2 += (b2 >= a2);
+                    const uint32_t h1 = species_at(a1, e_at), h2 = species_at(b1, e_at);
+                    const uint32_t h3 = species_at(a2, e_at), h4 = species_at(b2, e_at);
+                    my_null += (valid && h1 == h2 && h3 == h4) ? 1u : 0u;
+                }
+            }
+            __syncthreads();
+            if (e_done > 0u) {                                           // new epoch, clean bitmap
                 for (int i = tid; i < ((N + 31) >> 5); i += T) s_dirty[i] = 0u;
             }
             __syncthreads();
+#ifdef HEA_DBG
+            if (tid == 0) { dbg_t[2] += clock64() - dbg_c2; dbg_t[3] += 1; }
+#endif
+            t0 = t_ep + e_done;
             steps_done = 0u;                                             // t0 already advanced
             key_best = kNoKey;
         } else if (accept_ok && !team && W == 1u) {
@@ -1244,6 +1483,11 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         }
     }
 
+#ifdef HEA_DBG
+    if (tid == 0 && blockIdx.x == 0 && dbg_t[3] > 0)
+        printf("DBG epochs %lld steps %lld | P %lld S %lld N %lld cyc/epoch | per step: eval %lld stale %lld (n %lld) apply %lld mark %lld\n", dbg_t[3], dbg_t[10],
+               dbg_t[0] / dbg_t[3], dbg_t[1] / dbg_t[3], dbg_t[2] / dbg_t[3], dbg_t[4] / (dbg_t[8] + 1), dbg_t[5] / (dbg_t[8] + 1), dbg_t[9], dbg_t[6] / (dbg_t[8] + 1), dbg_t[7] / (dbg_t[8] + 1));
+#endif
     // ---- epilogue: release waiting followers, write back (rank 0 owns the global copy; nulls are summed over blocks)
     if (R > 1 && rank == 0 && !team) {
         __syncthreads();
@@ -1399,6 +1643,8 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
         sft = (uint32_t)(l - 1);
         m = (uint32_t)(((1ull << (32 + sft)) + d - 1) / d);
     };
+    AA.k_mq = 0u; AA.k_sq = 0u;
+    if (K >= 2) div_magic((uint64_t)K, AA.k_mq, AA.k_sq);
     div_magic((uint64_t)P.A * (uint64_t)P.L[2], G.mq, G.sq);
     div_magic((uint64_t)P.A * (uint64_t)P.L[1] * (uint64_t)P.L[2], G.mx, G.sx);
     G.PLy = P.L[1] + 2; G.PLz = P.L[2] + 2;
