@@ -37,6 +37,11 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+MC_REJECT_WARP_INSTR = 0.0      # per 32 trials, from the round-2 ncu capture named below
+MC_REJECT_WAVEFRONTS = 0.0
+MC_FULL_WARP_INSTR = 0.0        # whole c4 launch
+DTYPE = ("int32 counts + f64 objective (D6 order, no FMA); long windows pass a conservative fp32 reject filter on shell 1 "
+         "first (rigorous error bound in its threshold, survivors evaluated in f64: accept decisions are the f64 ones)")
 METRIC = "delta-SRO swap trials/sec (c4: fcc 40^3, 256,000 atoms, 16 chains x 1e7 steps, K=128) incl. the full-SRO recount of the start"
 UNIT = "swap-trials/s"
 
@@ -49,11 +54,19 @@ def load_peaks():
     return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
 
 
-# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed `ncu --set full` captures:
-# profiles/r1_mc_halo_c4_full.md (whole c4 trajectory, one launch) and profiles/r1_sro_count_v3.md (fcc 100^3, batch 1).
-NCU_TRAFFIC_MC_C4_FULL = 7_350_016 + 49_664
-NCU_TRAFFIC_RECOUNT_L100 = 680_663_040
-NCU_TRAFFIC_STENCIL_L100 = 4_030_464           # dram bytes read + written per launch, profiles/r1_sro_stencil.md
+# Figures that only a profiler can give, copied from the committed `ncu --set full` captures under profiles/ (bench.py
+# never runs under a profiler); every use below names its source file in the JSON line.
+NCU = {
+    # whole c4 trajectory, one launch: dram__bytes_read.sum + dram__bytes_write.sum
+    "mc_c4_full_dram_bytes": (7_350_016 + 49_664, "profiles/r1_mc_halo_c4_full.md"),
+    "mc_c4_full_warp_instr": (MC_FULL_WARP_INSTR, "profiles/r2_mc_halo_c4_full.md"),
+    # reject regime of c4 (1e6 steps after the trajectory): executed warp-instructions and shared-memory data-pipe
+    # wavefronts per 32 trials (smsp__inst_executed.sum, l1tex__data_pipe_lsu_wavefronts_mem_shared.sum over 6.4e7 warp-trials)
+    "mc_reject_warp_instr_per_32_trials": (MC_REJECT_WARP_INSTR, "profiles/r2_mc_halo_reject.md"),
+    "mc_reject_smem_wavefronts_per_32_trials": (MC_REJECT_WAVEFRONTS, "profiles/r2_mc_halo_reject.md"),
+    "recount_table_L100_dram_bytes": (680_663_040, "profiles/r1_sro_count_v3.md"),
+    "recount_stencil_L100_dram_bytes": (4_030_464, "profiles/r1_sro_stencil.md"),
+}
 
 
 # ALU-issue model of one swap trial: thread-instructions the method needs per candidate.
@@ -177,9 +190,11 @@ def run_reference(args):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t_all / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "int32 counts + f64 objective", "data": "synthetic",
+        "vs_baseline": None, "dtype": DTYPE, "data": "synthetic",
         "config": {"workload": "c4: fcc 40x40x40 (256,000 atoms), 4 species 0.25 each, shells 1-2, target seed 11, "
-                               "16 chains, K=128", "mc_steps_per_step": n_steps},
+                               "16 chains, K=128", "mc_steps_per_step": n_steps,
+                   "sample": f"the FIRST {n_steps} steps of the 1e7-step trajectory (accept regime), all K evaluated; the "
+                             "GPU arm runs the whole trajectory"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -254,6 +269,52 @@ def run_sweep(args):
         hm.close()
     print(json.dumps(out))
 
+def run_configs(args):
+    """BASELINE.json configs c1..c4 as configured (full length from the seeded start, all chains, one hea_mc_run call
+    each): device time, trials/s, accept rate.  Prints one JSON object; not the driver's bench line."""
+    import torch
+    from paper_2411_18906_b200 import binding, workloads
+    torch.cuda.set_device(0)
+    out = {"configs": []}
+    for ci in (1, 2, 3, 4):
+        w = workloads.config(ci)
+        h = binding.Hea(*w.create_args(), device=0)
+        best = None
+        for rep in range(3):
+            occ = h.init_random(w.n_chains, w.seed)
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            e[0].record()
+            cnt, _, _ = h.sro_full(occ)
+            e[1].record()
+            st, _ = h.mc_run(occ, cnt, w.n_steps, w.K, w.seed)
+            e[2].record()
+            torch.cuda.synchronize()
+            t_rc, t_mc = e[0].elapsed_time(e[1]) * 1e-3, e[1].elapsed_time(e[2]) * 1e-3
+            if best is None or t_mc < best[1]:
+                best = (t_rc, t_mc)
+        stn = binding.stats_to_numpy(st)
+        trials = w.n_chains * w.n_steps * w.K
+        out["configs"].append({"config": w.name, "lattice": w.lattice, "dims": list(w.dims), "atoms": w.n_sites,
+                               "species": w.n_species, "shells": w.n_shells, "chains": w.n_chains, "steps": w.n_steps, "K": w.K,
+                               "recount_us": 1e6 * best[0], "mc_ms": 1e3 * best[1], "trials": trials,
+                               "trials_per_s": trials / best[1], "us_per_step": 1e6 * best[1] / w.n_steps,
+                               "accept_rate": float(stn["n_accept"].sum()) / (w.n_chains * w.n_steps),
+                               "null_rate": float(stn["n_null"].sum()) / trials,
+                               "last_accept_step_max": int(stn["last_accept_step"][stn["n_accept"] > 0].max()),
+                               "J_mean": float(stn["J"].mean()), "J_max": float(stn["J"].max())})
+        h.close()
+    print(json.dumps(out))
+
+
+def run_peaks(args):
+    import torch
+    from paper_2411_18906_b200 import binding, workloads
+    torch.cuda.set_device(0)
+    h = binding.Hea(*workloads.config(1).create_args(), device=0)
+    print(json.dumps({"measured_peaks": h.measure_peaks(), "how": "hea_measure_peaks (csrc/hea_peaks.cu): one 512-thread block "
+                      "per SM, best of 3, CUDA events"}))
+
+
 # ------------------------------------------------------------------------------------------ GPU arm
 def main():
     ap = argparse.ArgumentParser()
@@ -270,6 +331,8 @@ def main():
     ap.add_argument("--chains", type=int, default=0, help="override the chain count (exploration only)")
     ap.add_argument("--opt", action="append", default=[], help="tuning option name=value (hea_set_option)")
     ap.add_argument("--sweep", action="store_true", help="run the configs[4] throughput sweeps instead of the bench step")
+    ap.add_argument("--configs", action="store_true", help="time configs c1..c4 as configured instead of the bench step")
+    ap.add_argument("--peaks", action="store_true", help="run the library's roofline micro-benchmarks and print them")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         args.warmup = 3                                   # timing rule: W >= 3
@@ -277,6 +340,10 @@ def main():
         return run_reference(args)
     if args.sweep:
         return run_sweep(args)
+    if args.configs:
+        return run_configs(args)
+    if args.peaks:
+        return run_peaks(args)
 
     import torch
     import torch.distributed as dist
@@ -422,7 +489,8 @@ def main():
         bytes_r = (4 * Zr + 1) * hr.N
         recount = {"bound": "hbm", "achieved": bytes_r / t_r / 1e9, "peak": hbm_peak, "unit": "GB/s",
                    "frac": bytes_r / t_r / 1e9 / hbm_peak,
-                   "traffic": NCU_TRAFFIC_RECOUNT_L100 if args.recount_L == 100 else None, "peak_source": peak_src,
+                   "traffic": NCU["recount_table_L100_dram_bytes"][0] if args.recount_L == 100 else None,
+                   "traffic_source": NCU["recount_table_L100_dram_bytes"][1], "peak_source": peak_src,
                    "kernel": "sro_count_kernel (sro_engine = 1)", "workload": f"fcc {args.recount_L}^3 ({hr.N} atoms), 5 species, "
                    f"3 shells (Z={Zr}), batch 1; table {4 * Zr * hr.N / 1e6:.0f} MB > L2",
                    "bytes_per_atom": 4 * Zr + 1, "atoms_per_s": hr.N / t_r, "ms_per_launch": t_r * 1e3}
@@ -431,7 +499,8 @@ def main():
         n_sms_r = torch.cuda.get_device_properties(dev).multi_processor_count
         recount_stencil = {"bound": "alu", "achieved": hr.N / t_s * ops_s / 1e12, "peak": issue_peak(n_sms_r, sm_mhz_r),
                            "unit": "T thread-instr/s", "frac": hr.N / t_s * ops_s / 1e12 / issue_peak(n_sms_r, sm_mhz_r),
-                           "traffic": NCU_TRAFFIC_STENCIL_L100 if args.recount_L == 100 else None,
+                           "traffic": NCU["recount_stencil_L100_dram_bytes"][0] if args.recount_L == 100 else None,
+                           "traffic_source": NCU["recount_stencil_L100_dram_bytes"][1],
                            "kernel": "sro_stencil_kernel (sro_engine = 2, the default)", "ops_per_atom": ops_s,
                            "workload": f"fcc {args.recount_L}^3 ({hr.N} atoms), 5 species, 3 shells, batch 1; 1 byte per atom",
                            "atoms_per_s": hr.N / t_s, "ms_per_launch": t_s * 1e3,
@@ -448,12 +517,31 @@ def main():
     value = trials_per_step * args.steps / t_dev
     ops = mc_ops_per_trial(sum(h.z), h.S, h.M)
     n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
-    alu_peak = n_sms * 128 * sm_max_mhz * 1e6 / 1e12                    # T thread-instr/s: 4 SMSPs x 32 lanes / clk
+    alu_peak = n_sms * 128 * sm_max_mhz * 1e6 / 1e12                    # nominal: 4 SMSPs x 32 lanes / clk
     mc_rate_1gpu = C * n_mc * K * args.steps / t_mc
+    # ---- roofline of the dominant kernel (mc_halo_kernel).  The kernel moves no HBM bytes in steady state; what binds it is
+    # instruction issue and the shared-memory data pipe.  Denominators: this box's own micro-benchmarks (hea_measure_peaks).
+    # achieved = warp-instructions the kernel EXECUTES per launch (ncu, committed profile) x 32 / measured launch duration.
+    peaks = h.measure_peaks()
+    is_metric_run = args.workload == 4 and not args.chains and n_mc == w.n_steps
+    full_instr, full_src = NCU["mc_c4_full_warp_instr"]
+    rej_instr, rej_src = NCU["mc_reject_warp_instr_per_32_trials"]
+    rej_wf, _ = NCU["mc_reject_smem_wavefronts_per_32_trials"]
+    issue_peak_T = peaks["issue_instr_per_s"] / 1e12
+    t_launch = t_mc / args.steps
+    achieved_T = full_instr * 32 / t_launch / 1e12 if is_metric_run else None
+    rej_rate = regimes["after_trajectory"]["trials_per_s"] / world
+    reject_roof = {
+        "issue": {"achieved": rej_rate * rej_instr / 1e12, "peak": issue_peak_T, "unit": "T thread-instr/s",
+                  "frac": rej_rate * rej_instr / 1e12 / issue_peak_T},
+        "smem_pipe": {"achieved": rej_rate / 32 * rej_wf / 1e12, "peak": peaks["lds_wavefronts_per_s"] / 1e12,
+                      "unit": "T wavefronts/s", "frac": rej_rate / 32 * rej_wf / peaks["lds_wavefronts_per_s"]},
+        "per_32_trials": {"warp_instr": rej_instr, "smem_wavefronts": rej_wf, "source": rej_src},
+        "trials_per_s": rej_rate}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "int32 counts + f64 objective", "data": "synthetic",
+        "dtype": DTYPE, "data": "synthetic",
         "config": {"workload": "c4: fcc 40x40x40 (256,000 atoms), 4 species 0.25 each, shells 1-2 (w 1, 0.5), "
                                "first-shell target in [-0.2, 0.2] from seed 11, 16 chains per GPU, K=128, chain seed 4",
                    "mc_steps_per_step": n_mc, "chains_per_gpu": C, "K": K, "l2": "flushed between timed iterations "
@@ -469,11 +557,19 @@ def main():
         "e2e": {"value": trials_per_step * args.steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "api": "hea_mc_run_host (pinned host occupancies)"},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "alu", "achieved": mc_rate_1gpu * ops / 1e12, "peak": alu_peak,
-                     "unit": "T thread-instr/s", "frac": mc_rate_1gpu * ops / 1e12 / alu_peak,
-                     "traffic": NCU_TRAFFIC_MC_C4_FULL if (args.workload == 4 and not args.chains and n_mc == w.n_steps) else None,
-                     "kernel": "mc_halo_kernel", "ops_per_trial": ops, "ms_per_launch": 1e3 * t_mc / args.steps,
-                     "peak_source": f"{n_sms} SMs x 128 lanes/clk x {sm_max_mhz:.0f} MHz (DESIGN.md section 6)"},
+        "roofline": {"bound": "alu", "achieved": achieved_T, "peak": issue_peak_T, "unit": "T thread-instr/s",
+                     "frac": (achieved_T / issue_peak_T) if achieved_T else None,
+                     "traffic": NCU["mc_c4_full_dram_bytes"][0] if is_metric_run else None,
+                     "traffic_source": NCU["mc_c4_full_dram_bytes"][1],
+                     "kernel": "mc_halo_kernel (whole launch: accept regime + reject regime)", "ms_per_launch": 1e3 * t_launch,
+                     "executed_warp_instr_per_launch": full_instr if is_metric_run else None, "executed_source": full_src,
+                     "peak_source": "measured on this box: hea_measure_peaks, LOP3 + IMAD interleaved on every SM (issue ceiling)",
+                     "reject_regime": reject_roof,
+                     "model": {"ops_per_trial": ops, "achieved": mc_rate_1gpu * ops / 1e12, "nominal_peak": alu_peak,
+                               "frac_of_nominal": mc_rate_1gpu * ops / 1e12 / alu_peak,
+                               "note": "round-1 figure: thread-instructions the method needs per trial (DESIGN.md 6) against "
+                                       f"{n_sms} SMs x 128 lanes/clk x {sm_max_mhz:.0f} MHz"}},
+        "measured_peaks": peaks,
     }
     if args.workload != 4 or args.chains:
         line["config"]["workload"] = f"EXPLORATION (not the metric's workload): {w.name}, {C} chains, K={K}, N={N}"

@@ -220,6 +220,24 @@ int hea_mc_run_host(hea_ctx* ctx, uint8_t* occ_host, int32_t* counts_host, int64
 /* Number of kernel launches issued by this context since creation (for bench.py's gpu_launches). */
 int hea_launch_count(const hea_ctx* ctx, int64_t* n);
 
+/*
+ * hea_measure_peaks -- micro-benchmarks of the resources the kernels of this library are bound by, for the roofline
+ * denominators that a copy / GEMM benchmark does not give.  Not part of the method: measurement support
+ * for bench.py.  Runs on `cuda_stream` of the context's device and synchronises on it (about 0.3 s).
+ * out_host [HEA_N_PEAKS] (HOST, doubles), whole-chip rates:
+ *   [0] random shared-memory byte gathers per second (LDS.U8, 32 lanes at random banks of a 128 KB array)
+ *   [1] conflict-free shared-memory wavefronts per second (LDS.32, lane l -> bank l)
+ *   [2] INT32 ALU-pipe thread-instructions per second (independent LOP3 chains)
+ *   [3] FMA-pipe integer thread-instructions per second (independent IMAD chains)
+ *   [4] thread-instructions per second with both pipes busy (LOP3 and IMAD interleaved): the issue ceiling
+ *   [5] fp64 thread-instructions per second (independent DMUL + DADD chains, no FMA, as in D6)
+ *   [6] GB/s of random 32-byte sectors read through L2 (64 MB array)
+ *   [7] SM clock in MHz reported by the device attribute
+ * Errors: HEA_EINVAL (NULL, n_out < HEA_N_PEAKS), HEA_ENOMEM / HEA_ECUDA.
+ */
+#define HEA_N_PEAKS 8
+int hea_measure_peaks(hea_ctx* ctx, double* out_host, int n_out, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ MOVE_DTYPE = np.dtype([("step", "<u8"), ("k", "<u4"), ("a", "<u4"), ("b", "<u4")
 
 EXPORTS = ["hea_version", "hea_last_error", "hea_create", "hea_destroy", "hea_info", "hea_neighbor_table",
            "hea_set_option", "hea_get_option", "hea_init_random", "hea_sro_full", "hea_mc_stats_reset",
-           "hea_mc_run", "hea_mc_run_ex", "hea_pool_select", "hea_sro_full_host", "hea_mc_run_host", "hea_launch_count"]
+           "hea_mc_run", "hea_mc_run_ex", "hea_pool_select", "hea_sro_full_host", "hea_mc_run_host", "hea_launch_count", "hea_measure_peaks"]
 
 
 class HeaError(RuntimeError):
@@ -61,6 +61,7 @@ def lib():
         L.hea_sro_full_host.argtypes = [vp, vp, i64, vp, vp, vp]
         L.hea_mc_run_host.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp]
         L.hea_launch_count.argtypes = [vp, vp]
+        L.hea_measure_peaks.argtypes = [vp, vp, i32, vp]
         _lib = L
     return _lib
 
@@ -126,6 +127,15 @@ class Hea:
         v = C.c_int64()
         _check(lib().hea_launch_count(self._h, C.byref(v)))
         return int(v.value)
+
+    PEAK_NAMES = ("lds_u8_random_gathers_per_s", "lds_wavefronts_per_s", "alu_pipe_instr_per_s", "fma_pipe_int_instr_per_s",
+                  "issue_instr_per_s", "fp64_instr_per_s", "l2_random_sector_GBps", "sm_clock_mhz")
+
+    def measure_peaks(self):
+        """hea_measure_peaks: dict of whole-chip rates measured by the library's micro-benchmarks."""
+        out = np.zeros(len(self.PEAK_NAMES), dtype=np.float64)
+        _check(lib().hea_measure_peaks(self._h, _np(out), len(out), _stream()))
+        return dict(zip(self.PEAK_NAMES, (float(v) for v in out)))
 
     # ---- device-buffer calls (torch tensors own the memory; asynchronous on the current stream)
     def init_random(self, n_chains, seed, chain0=0, out=None):

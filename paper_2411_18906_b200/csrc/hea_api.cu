@@ -35,6 +35,7 @@ cudaError_t launch_pool_rank(const double* J, int64_t C, int64_t n_keep, int32_t
 cudaError_t launch_pool_gather(const void* src, void* dst, const int32_t* order, int64_t n_keep, size_t item,
                                cudaStream_t st, int64_t* n_launches);
 size_t mc2_team_bytes(int64_t C);
+cudaError_t measure_peaks(int n_sms, int clock_khz, double* out, cudaStream_t st, int64_t* n_launches);
 constexpr int kMc2MaxThreads = 512;
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
                        void* team_ctl, int team_on, int team_off, int accept_engine, size_t smem_budget, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
@@ -567,6 +568,17 @@ int hea_pool_select(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, hea_mc_
         if ((rc = hea_mc_stats_reset(ctx, stats_dev + n_keep, n_new, cuda_stream)) != HEA_OK) return rc;
     }
     return HEA_OK;
+}
+
+int hea_measure_peaks(hea_ctx* ctx, double* out_host, int n_out, void* cuda_stream)
+{
+    if (!ctx || !out_host) return fail(HEA_EINVAL, "ctx / out_host is NULL");
+    if (n_out < HEA_N_PEAKS) return fail(HEA_EINVAL, "out_host needs HEA_N_PEAKS entries");
+    DeviceGuard guard(ctx->device);
+    int khz = 0;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, ctx->device);
+    cudaError_t e = hea::measure_peaks(ctx->n_sms, khz, out_host, (cudaStream_t)cuda_stream, &ctx->n_launches);
+    return e == cudaSuccess ? HEA_OK : fail_cuda(e, "hea_measure_peaks");
 }
 
 int hea_sro_full_host(hea_ctx* ctx, const uint8_t* occ_host, int64_t B, int32_t* counts_host, double* alpha_host,

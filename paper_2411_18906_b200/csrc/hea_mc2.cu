@@ -14,7 +14,6 @@
 //  * Whether b is a neighbour of a (the exclusion of D9.2) comes from the lattice coordinates of the two sites
 //    (minimum-image displacement, squared length == shell distance), not from a compare per table entry.
 //  * Shell sizes and the basis count are template constants (fcc 12/6/24, bcc 8/6/12), so every gather is unrolled.
-#include <cstdio>
 #include <cstring>
 #include <type_traits>
 
@@ -84,10 +83,9 @@ struct Sh2 {
     int4 wdesc[24];               // accumulator word w -> (int4 index in the offset row, slot mask, shell, side)
     uint4 mlog[kPaeRecs / kPaeK]; // serial accept engine: the move of each step of the epoch (a, b, p | q << 8 | 1 << 16, -)
     uint32_t swe_stop;            //   steps of the epoch consumed so far | (a step needs the candidates beyond kPaeK) << 31
-    uint32_t sbest[3], sstale[3]; //   lowest improving record / mask of stale records of a step, triple-buffered
-    uint32_t sbest2[3];           //   lowest improving REBUILT record of the step
-    uint32_t pad2[2];
-    MoveRec cand2[2][kPaeK];      //   improving records of a step, by step parity (the role warps read one step behind)
+    uint32_t sbest2[3];           //   lowest improving REBUILT record of a step (triple-buffered like sel)
+    uint2 sel[3];                 //   (lowest improving record, mask of stale records) of a step
+    double sJ[2][kPaeK];          //   J of the improving records of a step, by step parity (the role warps read one step behind)
     int4 fs_rd[4];                // first shell without the offset table: per basis index, per group of four, the part of a
                                   // neighbour's padded-index offset that depends on the site's basis (see Mc2Args::fs_c)
     double g[kSMM], t[kSMM];      // objective constants with a per-lane index
@@ -333,6 +331,11 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     PRec* s_prec = reinterpret_cast<PRec*>(s_ftab + ((MM * RS + 3) & ~3));
     uint32_t* s_dirty = reinterpret_cast<uint32_t*>(s_prec + kPaeRecs);
     int* s_loff = reinterpret_cast<int*>(s_dirty + ((P.N + 31) >> 5));
+    // serial accept engine: packed count changes per objective row of the improving records, [step parity][record][S*M]
+    unsigned long long* s_dn = reinterpret_cast<unsigned long long*>(
+        (reinterpret_cast<uintptr_t>(s_loff + LC::A * P.Z) + 7u) & ~(uintptr_t)7u);
+    // per record: padded index of a and of b, bit 31 = the site's cell is interior (no ghost image, neighbours = site + offset)
+    uint2* s_px = reinterpret_cast<uint2*>(s_dn + 2 * kPaeK * P.S * P.M);
 
     const int tid = threadIdx.x, T = blockDim.x;
     const int S = P.S, N = P.N, K = A.K, R = A.R;
@@ -705,46 +708,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         }
         return Jk;
     };
-    // the same with the counts of this lane's rows in registers (serial accept engine)
-    auto g8_Jr = [&](const int (&cntr)[NRR][M], const int (&c)[M], int p, int q, const int (&F0)[M], const int (&F1)[M],
-                     const int (&F2)[M]) -> double {
-        const int l8 = tid & 7;
-        double rowv[NRR];
-#pragma unroll
-        for (int rr = 0; rr < NRR; ++rr) {
-            const int rho = l8 + 8 * rr;
-            double row = 0.0;
-            if (rho < S * M) {
-                const int s = rho / M, i = rho - s * M;
-                const int ci = (i == p) - (i == q);
-                int Fi = 0;
-#pragma unroll
-                for (int j = 0; j < M; ++j) { const int Fj = s == 0 ? F0[j] : s == 1 ? F1[j] : F2[j]; Fi = j == i ? Fj : Fi; }
-#pragma unroll
-                for (int j = 0; j < M; ++j) {
-                    const int Fj = s == 0 ? F0[j] : s == 1 ? F1[j] : F2[j];
-                    const int n = cntr[rr][j] + ci * Fj + c[j] * Fi;
-                    row = __dadd_rn(row, sq_dev(n, sh.g[rho * M + j], sh.t[rho * M + j]));
-                }
-            }
-            rowv[rr] = row;
-        }
-        double Jk = 0.0;
-#pragma unroll
-        for (int s = 0; s < 3; ++s) {
-            if (s < S) {
-                double shs = 0.0;
-#pragma unroll
-                for (int i = 0; i < M; ++i) {
-                    const int rho = s * M + i;
-                    const double v = __shfl_sync(0xFFFFFFFFu, rowv[rho >> 3], (tid & 24) | (rho & 7));
-                    shs = __dadd_rn(shs, v);
-                }
-                Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[s], shs));
-            }
-        }
-        return Jk;
-    };
     auto g8_post = [&](bool live, double Jk, double J_cur, uint32_t k, uint32_t a, uint32_t b, int p, int q,
                        const int (&F0)[M], const int (&F1)[M], const int (&F2)[M], int grp, int buf) {
         const int l8 = tid & 7;
@@ -769,10 +732,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         g8_post(live, Jk, J_cur, k, a, b, p, q, F0, F1, F2, grp, buf);
     };
 
-#ifdef HEA_DBG
-    __shared__ long long dbg_t[16];
-    if (tid < 16) dbg_t[tid] = 0;
-#endif
     unsigned long long t0 = A.step0;
     const unsigned long long t_end = A.step0 + A.n_steps;
     uint32_t W = 1;
@@ -821,11 +780,13 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             //     through the epoch's move log.
             const uint32_t n_ep = (uint32_t)min((unsigned long long)(T / kPaeK), t_end - t0);
             const unsigned long long t_ep = t0;
-#ifdef HEA_DBG
-            long long dbg_c0 = clock64();
-#endif
-            auto build_record = [&](unsigned long long step, uint32_t k) -> PRec {
+            auto px_of = [&](const SiteC& sc) -> uint32_t {
+                const bool interior = sc.x >= 1 && sc.x <= Lx - 2 && sc.y >= 1 && sc.y <= Ly - 2 && sc.z >= 1 && sc.z <= Lz - 2;
+                return sc.pidx | (interior ? 0x80000000u : 0u);
+            };
+            auto build_record = [&](unsigned long long step, uint32_t k, uint2& px) -> PRec {
                 PRec rec;
+                px = make_uint2(0u, 0u);
                 rec.pad = 0; rec.d0 = rec.d1 = rec.d2 = 0ull; rec.a = rec.b = rec.a1 = rec.b1 = 0u;
                 rec.pqn = 1u << 17;                                   // absent (k >= K)
                 if (k < (uint32_t)K) {
@@ -833,6 +794,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     SiteC sa, sb;
                     propose2(step, k, a, b, sa, sb, hp, hq, a1, b1);
                     rec.a = a; rec.b = b; rec.a1 = a1; rec.b1 = b1;
+                    px = make_uint2(px_of(sa), px_of(sb));
                     if (hp == hq) {
                         rec.pqn = 1u << 16;                           // null
                     } else {
@@ -871,14 +833,13 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 }
                 return rec;
             };
-            if ((uint32_t)tid < n_ep * (uint32_t)kPaeK)
-                s_prec[tid] = build_record(t0 + (uint32_t)tid / (uint32_t)kPaeK, (uint32_t)tid % (uint32_t)kPaeK);
+            if ((uint32_t)tid < n_ep * (uint32_t)kPaeK) {
+                uint2 px;
+                s_prec[tid] = build_record(t0 + (uint32_t)tid / (uint32_t)kPaeK, (uint32_t)tid % (uint32_t)kPaeK, px);
+                s_px[tid] = px;
+            }
             if (tid < kPaeRecs / kPaeK) sh.mlog[tid] = make_uint4(0u, 0u, 0u, 0u);
             __syncthreads();
-#ifdef HEA_DBG
-            long long dbg_c1 = clock64();
-            if (tid == 0) dbg_t[0] += dbg_c1 - dbg_c0;
-#endif
             uint32_t e_done = 0;                                         // steps of the epoch consumed
             bool leave = false;
             while (e_done < n_ep && !leave) {
@@ -887,151 +848,209 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 // with its ghost images (warp 6), shared counts, J, hash, logs (warp 7) -- one step behind the evaluation.
                 // Named barriers: 2 = "bitmap and configuration of the previous move are in place" (roles arrive, eval
                 // waits), 3 = "selection of this step posted" (all eight warps), 4 = the same after rebuilt records.
+                // An improving group posts its J and, per objective row, the count changes as packed signed bytes
+                // (s_dn); the move itself is read from the record of the winner.
                 if (tid < 256) {
                     const bool is_eval = tid < 128;
                     const int grp = (tid >> 3) & 15, l8 = tid & 7;
+                    const int SMr = S * M;
                     auto dirty = [&](uint32_t v) { return (s_dirty[v >> 5] >> (v & 31u)) & 1u; };
+                    auto sext8 = [](unsigned long long v, int j) { return (int)(signed char)(unsigned char)(v >> (8 * j)); };
                     int cntr[NRR][M];                                    // EVAL: counts of rows l8 + 8 rr
+                    int srow[NRR], irow[NRR];
 #pragma unroll
                     for (int rr = 0; rr < NRR; ++rr) {
                         const int rho = l8 + 8 * rr;
+                        const bool v = is_eval && rho < SMr;
+                        srow[rr] = v ? rho / M : -1;
+                        irow[rr] = v ? rho - srow[rr] * M : 0;
 #pragma unroll
-                        for (int j = 0; j < M; ++j) cntr[rr][j] = (is_eval && rho < S * M) ? sh.cnt[rho * M + j] : 0;
+                        for (int j = 0; j < M; ++j) cntr[rr][j] = v ? sh.cnt[rho * M + j] : 0;
                     }
+                    // J and packed count changes of a candidate (pqn, packed F of the shells of this lane's rows)
+                    auto eval_rows = [&](uint32_t pqn, const unsigned long long (&dsel)[NRR], unsigned long long (&dnp)[NRR]) -> double {
+                        const bool live = !((pqn >> 16) & 3u);
+                        const int p = (int)(pqn & 0xFFu), q = (int)((pqn >> 8) & 0xFFu);
+                        double rowv[NRR];
+#pragma unroll
+                        for (int rr = 0; rr < NRR; ++rr) {
+                            double row = 0.0;
+                            unsigned long long pk = 0ull;
+                            if (srow[rr] >= 0) {
+                                const int i = irow[rr], rho = l8 + 8 * rr;
+                                const PW d = (PW)dsel[rr];
+                                const int ci = live ? (i == p) - (i == q) : 0;
+                                const int Fi = (int)((d >> (Pack<M>::FB * i)) & (PW)((1 << Pack<M>::FB) - 1)) - Pack<M>::kHalf;
+#pragma unroll
+                                for (int j = 0; j < M; ++j) {
+                                    const int cj = live ? (j == p) - (j == q) : 0;
+                                    const int dn = ci * Pack<M>::field(d, j) + cj * Fi;
+                                    pk |= (unsigned long long)(unsigned char)dn << (8 * j);
+                                    row = __dadd_rn(row, sq_dev(cntr[rr][j] + dn, sh.g[rho * M + j], sh.t[rho * M + j]));
+                                }
+                            }
+                            rowv[rr] = row;
+                            dnp[rr] = pk;
+                        }
+                        double Jk = 0.0;
+#pragma unroll
+                        for (int s = 0; s < 3; ++s) {
+                            if (s < S) {
+                                double shs = 0.0;
+#pragma unroll
+                                for (int i = 0; i < M; ++i) {
+                                    const int rho = s * M + i;
+                                    const double v = __shfl_sync(0xFFFFFFFFu, rowv[rho >> 3], (tid & 24) | (rho & 7));
+                                    shs = __dadd_rn(shs, v);
+                                }
+                                Jk = __dadd_rn(Jk, __dmul_rn(Kc.w[s], shs));
+                            }
+                        }
+                        return Jk;
+                    };
                     double J_cur = sh.J;
-                    if (tid < 3) { sh.sbest[tid] = kNoKey; sh.sbest2[tid] = kNoKey; sh.sstale[tid] = 0u; }
+                    if (tid < 3) { sh.sel[tid] = make_uint2(kNoKey, 0u); sh.sbest2[tid] = kNoKey; }
                     asm volatile("bar.sync 4, 256;" ::: "memory");
                     if (!is_eval && tid < 224) asm volatile("bar.arrive 2, 224;" ::: "memory");
                     uint32_t es = e_done, pend = 0u, sit = 0u;
-                    bool moved = false;
                     for (; es < n_ep; ++es, ++sit) {
                         const int sb = (int)(sit % 3u), par = (int)(sit & 1u);
                         const unsigned long long step = t_ep + es;
-                        PRec rec;
-                        uint32_t a = 0, b = 0;
-                        bool absent = true, live = false;
-                        int p = 0, q = 0;
-                        int c[M], F0[M], F1[M], F2[M];
+                        PRec* const rp = &s_prec[es * kPaeK + grp];
+                        unsigned long long dnp[NRR];
                         double Jk = 0.0;
                         if (is_eval) {
-                            rec = s_prec[es * kPaeK + grp];
-                            absent = (rec.pqn >> 17) & 1u;
-                            a = rec.a; b = rec.b;
-                            live = !absent && !((rec.pqn >> 16) & 1u);
-                            p = (int)(rec.pqn & 0xFFu); q = (int)((rec.pqn >> 8) & 0xFFu);
+                            const uint4 sites = *reinterpret_cast<const uint4*>(rp);     // a, b, a1, b1
+                            const uint32_t pqn = rp->pqn;
+                            unsigned long long dsel[NRR];
 #pragma unroll
-                            for (int r2 = 0; r2 < M; ++r2) {
-                                c[r2] = live ? (r2 == p) - (r2 == q) : 0;
-                                F0[r2] = Pack<M>::field((PW)rec.d0, r2); F1[r2] = Pack<M>::field((PW)rec.d1, r2);
-                                F2[r2] = Pack<M>::field((PW)rec.d2, r2);
-                            }
-                            Jk = g8_Jr(cntr, c, p, q, F0, F1, F2);
+                            for (int rr = 0; rr < NRR; ++rr) dsel[rr] = (&rp->d0)[max(srow[rr], 0)];
+                            Jk = eval_rows(pqn, dsel, dnp);
                             asm volatile("bar.sync 2, 224;" ::: "memory");       // the previous move is in the bitmap
-                            const bool stale = !absent && (dirty(rec.a) | dirty(rec.b) | dirty(rec.a1) | dirty(rec.b1));
-                            if (l8 == 0) {
-                                if (stale) {
-                                    atomicOr(&sh.sstale[sb], 1u << grp);
-                                } else if (live && Jk < J_cur) {
-                                    MoveRec& m = sh.cand2[par][grp];
-                                    m.key = (uint32_t)grp; m.a = a; m.b = b; m.pq = (uint32_t)p | ((uint32_t)q << 8); m.J = Jk;
-                                    m.d[0] = rec.d0; m.d[1] = rec.d1; m.d[2] = rec.d2;
-                                    atomicMin(&sh.sbest[sb], (uint32_t)grp);
-                                }
+                            const bool absent = (pqn >> 17) & 1u;
+                            const bool stale = !absent && (dirty(sites.x) | dirty(sites.y) | dirty(sites.z) | dirty(sites.w));
+                            if (stale) {
+                                if (l8 == 0) atomicOr(&sh.sel[sb].y, 1u << grp);
+                            } else if (!((pqn >> 16) & 3u) && Jk < J_cur) {
+#pragma unroll
+                                for (int rr = 0; rr < NRR; ++rr)
+                                    if (srow[rr] >= 0) s_dn[(par * kPaeK + grp) * SMr + l8 + 8 * rr] = dnp[rr];
+                                if (l8 == 0) { sh.sJ[par][grp] = Jk; atomicMin(&sh.sel[sb].x, (uint32_t)grp); }
                             }
                         }
                         asm volatile("bar.sync 3, 256;" ::: "memory");           // selection posted
-                        uint32_t kb = sh.sbest[sb];
-                        const uint32_t sm = sh.sstale[sb];
+                        const uint2 sel = sh.sel[sb];
+                        uint32_t kb = sel.x;
                         // stale records below the first improving fresh one decide the step: their warps rebuild their
                         // four records from the current configuration (8 lanes per record) and evaluate again
-                        const uint32_t need = sm & (kb == kNoKey ? 0xFFFFFFFFu : ((1u << kb) - 1u));
+                        const uint32_t need = sel.y & (kb == kNoKey ? 0xFFFFFFFFu : ((1u << kb) - 1u));
                         if (need) {
                             if (is_eval && ((need >> (grp & ~3)) & 0xFu)) {
-                                uint32_t hp, hq;
+                                uint32_t a, b, hp, hq;
                                 SiteC sa, sb2;
                                 propose(step, (uint32_t)grp, a, b, sa, sb2, hp, hq);
-                                live = !absent && hp != hq;
-                                p = 31 - __clz((int)hp); q = 31 - __clz((int)hq);
+                                const bool absent = (rp->pqn >> 17) & 1u;
+                                const bool live = !absent && hp != hq;
+                                const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+                                int c[M], F0[M], F1[M], F2[M];
                                 int mm0, mm1, mm2;
                                 adjacency(a, b, sa, sb2, mm0, mm1, mm2);
                                 g8_F(sa, sb2, mm0, mm1, mm2, p, q, c, F0, F1, F2);
-                                if (!live) {
+                                const unsigned long long d0 = pack_F<M>(F0), d1 = pack_F<M>(F1), d2 = pack_F<M>(F2);
+                                const uint32_t pqn = absent ? (1u << 17) : !live ? (1u << 16) : ((uint32_t)p | ((uint32_t)q << 8));
+                                unsigned long long dsel[NRR];
 #pragma unroll
-                                    for (int r2 = 0; r2 < M; ++r2) c[r2] = 0;
+                                for (int rr = 0; rr < NRR; ++rr) dsel[rr] = srow[rr] == 1 ? d1 : srow[rr] == 2 ? d2 : d0;
+                                Jk = eval_rows(pqn, dsel, dnp);
+                                if (l8 == 0) {
+                                    rp->a = a; rp->b = b; rp->pqn = pqn; rp->d0 = d0; rp->d1 = d1; rp->d2 = d2;
+                                    s_px[es * kPaeK + grp] = make_uint2(px_of(sa), px_of(sb2));
                                 }
-                                Jk = g8_Jr(cntr, c, p, q, F0, F1, F2);
-                                if (l8 == 0 && live && Jk < J_cur) {
-                                    MoveRec& m = sh.cand2[par][grp];
-                                    m.key = (uint32_t)grp; m.a = a; m.b = b; m.pq = (uint32_t)p | ((uint32_t)q << 8); m.J = Jk;
-                                    m.d[0] = pack_F<M>(F0); m.d[1] = pack_F<M>(F1); m.d[2] = pack_F<M>(F2);
-                                    atomicMin(&sh.sbest2[sb], (uint32_t)grp);     // (a slot of its own: barrier 3 readers still compare sbest)
+                                if (live && Jk < J_cur) {
+#pragma unroll
+                                    for (int rr = 0; rr < NRR; ++rr)
+                                        if (srow[rr] >= 0) s_dn[(par * kPaeK + grp) * SMr + l8 + 8 * rr] = dnp[rr];
+                                    // (a slot of its own: the readers of barrier 3 still compare sel)
+                                    if (l8 == 0) { sh.sJ[par][grp] = Jk; atomicMin(&sh.sbest2[sb], (uint32_t)grp); }
                                 }
                             }
                             asm volatile("bar.sync 4, 256;" ::: "memory");
                             kb = min(kb, sh.sbest2[sb]);
                         }
-                        if (tid == 255) { sh.sbest[(sb + 2) % 3] = kNoKey; sh.sbest2[(sb + 2) % 3] = kNoKey; sh.sstale[(sb + 2) % 3] = 0u; }
+                        if (tid == 255) { sh.sel[(sb + 2) % 3] = make_uint2(kNoKey, 0u); sh.sbest2[(sb + 2) % 3] = kNoKey; }
                         if (kb == kNoKey) { pend = 1u; break; }
-                        moved = true;
-                        const MoveRec* mv = &sh.cand2[par][kb];
-                        const int wp = (int)(mv->pq & 0xFFu), wq = (int)(mv->pq >> 8);
                         if (is_eval) {
                             // D9.4 on the register copy of this lane's rows
-                            J_cur = mv->J;
+                            J_cur = sh.sJ[par][kb];
 #pragma unroll
                             for (int rr = 0; rr < NRR; ++rr) {
-                                const int rho = l8 + 8 * rr;
-                                if (rho < S * M) {
-                                    const int s2 = rho / M, i = rho - s2 * M;
-                                    const PW d = (PW)mv->d[s2];
-                                    const int ci = (i == wp) - (i == wq);
-                                    const int Fi = Pack<M>::field(d, i);
+                                if (srow[rr] >= 0) {
+                                    const unsigned long long d8 = s_dn[(par * kPaeK + (int)kb) * SMr + l8 + 8 * rr];
 #pragma unroll
-                                    for (int j = 0; j < M; ++j)
-                                        cntr[rr][j] += ci * Pack<M>::field(d, j) + ((j == wp) - (j == wq)) * Fi;
+                                    for (int j = 0; j < M; ++j) cntr[rr][j] += sext8(d8, j);
                                 }
                             }
-                        } else if (tid < 192) {                          // warps 4, 5: neighbourhoods of a and of b
-                            mark_one(tid < 160 ? mv->a : mv->b, tid & 31);
-                            asm volatile("bar.arrive 2, 224;" ::: "memory");
-                        } else if (tid < 224) {                          // warp 6: the swap (one lane: a and b may share a byte)
-                            if (tid == 192) { write_site(mv->a, 1u << wq); write_site(mv->b, 1u << wp); }
-                            asm volatile("bar.arrive 2, 224;" ::: "memory");
-                        } else {                                         // warp 7: shared counts and bookkeeping
-                            for (int idx = tid - 224; idx < SMM; idx += 32) {
-                                const int s2 = idx / MM, rem = idx - s2 * MM, i = rem / M, jj = rem - i * M;
-                                const PW d = (PW)mv->d[s2];
-                                const int ci = (i == wp) - (i == wq), cj = (jj == wp) - (jj == wq);
-                                sh.cnt[idx] += ci * Pack<M>::field(d, jj) + cj * Pack<M>::field(d, i);
-                            }
-                            if (tid == 224) {
-                                const uint32_t wa = mv->a, wb = mv->b;
-                                sh.J = mv->J;
-                                sh.n_accept += 1;
-                                sh.last_accept = step;
-                                unsigned long long hsh = sh.hash;
-                                hsh = (hsh ^ (uint32_t)step) * 0x100000001b3ULL;
-                                hsh = (hsh ^ (uint32_t)(step >> 32)) * 0x100000001b3ULL;
-                                hsh = (hsh ^ kb) * 0x100000001b3ULL;
-                                hsh = (hsh ^ wa) * 0x100000001b3ULL;
-                                hsh = (hsh ^ wb) * 0x100000001b3ULL;
-                                sh.hash = hsh;
-                                sh.mlog[es] = make_uint4(wa, wb, mv->pq | (1u << 16), 0u);
-                                const unsigned long long nl = sh.n_logged;
-                                if (rank == 0 && A.log_all != nullptr && (long long)nl < A.log_cap) {
-                                    unsigned long long* lr = A.log_all + (chain_local * (size_t)A.log_cap + nl) * 3;
-                                    lr[0] = step;
-                                    lr[1] = (unsigned long long)kb | ((unsigned long long)wa << 32);
-                                    lr[2] = (unsigned long long)wb;
+                        } else {
+                            const PRec* wr = &s_prec[es * kPaeK + kb];
+                            const uint32_t wa = wr->a, wb = wr->b, wpq = wr->pqn;
+                            const uint2 wpx = s_px[es * kPaeK + kb];
+                            const int wp = (int)(wpq & 0xFFu), wq = (int)((wpq >> 8) & 0xFFu);
+                            if (tid < 192) {                             // warps 4, 5: neighbourhoods of a and of b
+                                const uint32_t u = tid < 160 ? wa : wb, upx = tid < 160 ? wpx.x : wpx.y;
+                                if (upx >> 31) {                         // interior cell: neighbour = site + offset of its basis index
+                                    const int lane = tid & 31, bb = (int)(upx & (uint32_t)(LC::A - 1));
+                                    for (int e = lane; e < P.Z; e += 32) {
+                                        const uint32_t v = u + (uint32_t)s_loff[bb * P.Z + e];
+                                        atomicOr(&s_dirty[v >> 5], 1u << (v & 31u));
+                                    }
+                                    if (lane == 0) atomicOr(&s_dirty[u >> 5], 1u << (u & 31u));
+                                } else {
+                                    mark_one(u, tid & 31);
                                 }
-                                sh.n_logged = nl + 1;
+                                asm volatile("bar.arrive 2, 224;" ::: "memory");
+                            } else if (tid < 224) {                      // warp 6: the swap (one lane: a and b may share a byte)
+                                const bool same_byte = OCC == OCC2_NIB && ((wpx.x & 0x7FFFFFFFu) >> 1) == ((wpx.y & 0x7FFFFFFFu) >> 1);
+                                if ((wpx.x & wpx.y) >> 31 && !same_byte) {       // both interior: one lane each
+                                    if (tid == 192) occ_set<OCC>(s_occ, wpx.x & 0x7FFFFFFFu, 1u << wq);
+                                    if (tid == 193) occ_set<OCC>(s_occ, wpx.y & 0x7FFFFFFFu, 1u << wp);
+                                } else if (tid == 192) {
+                                    write_site(wa, 1u << wq); write_site(wb, 1u << wp);
+                                }
+                                asm volatile("bar.arrive 2, 224;" ::: "memory");
+                            } else {                                     // warp 7: shared counts and bookkeeping
+                                for (int idx = tid - 224; idx < SMM; idx += 32) {
+                                    const int s2 = idx / MM, rem = idx - s2 * MM, i = rem / M, jj = rem - i * M;
+                                    const PW d = (PW)(&wr->d0)[s2];
+                                    const int ci = (i == wp) - (i == wq), cj = (jj == wp) - (jj == wq);
+                                    sh.cnt[idx] += ci * Pack<M>::field(d, jj) + cj * Pack<M>::field(d, i);
+                                }
+                                if (tid == 224) {
+                                    sh.J = sh.sJ[par][kb];
+                                    sh.n_accept += 1;
+                                    sh.last_accept = step;
+                                    unsigned long long hsh = sh.hash;
+                                    hsh = (hsh ^ (uint32_t)step) * 0x100000001b3ULL;
+                                    hsh = (hsh ^ (uint32_t)(step >> 32)) * 0x100000001b3ULL;
+                                    hsh = (hsh ^ kb) * 0x100000001b3ULL;
+                                    hsh = (hsh ^ wa) * 0x100000001b3ULL;
+                                    hsh = (hsh ^ wb) * 0x100000001b3ULL;
+                                    sh.hash = hsh;
+                                    sh.mlog[es] = make_uint4(wa, wb, (wpq & 0xFFFFu) | (1u << 16), 0u);
+                                    const unsigned long long nl = sh.n_logged;
+                                    if (rank == 0 && A.log_all != nullptr && (long long)nl < A.log_cap) {
+                                        unsigned long long* lr = A.log_all + (chain_local * (size_t)A.log_cap + nl) * 3;
+                                        lr[0] = step;
+                                        lr[1] = (unsigned long long)kb | ((unsigned long long)wa << 32);
+                                        lr[2] = (unsigned long long)wb;
+                                    }
+                                    sh.n_logged = nl + 1;
+                                }
                             }
                         }
                     }
                     // barrier 2 is left balanced: one arrival is outstanding unless the loop stopped at a step without a move
                     if (is_eval && !pend) asm volatile("bar.sync 2, 224;" ::: "memory");
                     if (tid == 0) sh.swe_stop = es | (pend << 31);
-                    (void)moved;
                 }
                 __syncthreads();
                 const uint32_t st = sh.swe_stop;
@@ -1068,10 +1087,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     e_done += 1;
                 }
             }
-#ifdef HEA_DBG
-            long long dbg_c2 = clock64();
-            if (tid == 0) { dbg_t[1] += dbg_c2 - dbg_c1; dbg_t[10] += e_done; }
-#endif
             // ---- (N) null candidates of the e_done consumed steps, all K of each.  The species of a drawn site at its
             // step is the final one unless a move of the epoch touched the site (the bitmap says so, conservatively):
             // then the moves from the end of the epoch back to that step are undone for this site.
@@ -1124,9 +1139,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 for (int i = tid; i < ((N + 31) >> 5); i += T) s_dirty[i] = 0u;
             }
             __syncthreads();
-#ifdef HEA_DBG
-            if (tid == 0) { dbg_t[2] += clock64() - dbg_c2; dbg_t[3] += 1; }
-#endif
             t0 = t_ep + e_done;
             steps_done = 0u;                                             // t0 already advanced
             key_best = kNoKey;
@@ -1483,11 +1495,6 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         }
     }
 
-#ifdef HEA_DBG
-    if (tid == 0 && blockIdx.x == 0 && dbg_t[3] > 0)
-        printf("DBG epochs %lld steps %lld | P %lld S %lld N %lld cyc/epoch | per step: eval %lld stale %lld (n %lld) apply %lld mark %lld\n", dbg_t[3], dbg_t[10],
-               dbg_t[0] / dbg_t[3], dbg_t[1] / dbg_t[3], dbg_t[2] / dbg_t[3], dbg_t[4] / (dbg_t[8] + 1), dbg_t[5] / (dbg_t[8] + 1), dbg_t[9], dbg_t[6] / (dbg_t[8] + 1), dbg_t[7] / (dbg_t[8] + 1));
-#endif
     // ---- epilogue: release waiting followers, write back (rank 0 owns the global copy; nulls are summed over blocks)
     if (R > 1 && rank == 0 && !team) {
         __syncthreads();
@@ -1687,7 +1694,8 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
     G.distinct = P.L[0] >= 3 && P.L[1] >= 3 && P.L[2] >= 3;
     size_t smem = mc2_shared_bytes(occ_mode, lattice, P.L, P.M);
     // the pipelined accept engine needs its record, bitmap and offset buffers on top; without room it is simply off
-    const size_t pae_bytes = sizeof(PRec) * (size_t)kPaeRecs + 4u * (size_t)((P.N + 31) >> 5) + 4u * (size_t)P.A * (size_t)P.Z + 16u;
+    const size_t pae_bytes = sizeof(PRec) * (size_t)kPaeRecs + 4u * (size_t)((P.N + 31) >> 5) + 4u * (size_t)P.A * (size_t)P.Z + 16u +
+                             8u * 2u * (size_t)kPaeK * (size_t)P.S * (size_t)P.M + 8u + sizeof(uint2) * (size_t)kPaeRecs;
     AA.pae = (accept_engine == 2 && threads >= 512 && smem + pae_bytes <= smem_budget) ? 1 : 0;
     if (AA.pae) smem += pae_bytes;
     const int part = (lattice != 0 ? 1 : 0) + (select_best ? 2 : 0);
