@@ -14,6 +14,8 @@
 //  * Whether b is a neighbour of a (the exclusion of D9.2) comes from the lattice coordinates of the two sites
 //    (minimum-image displacement, squared length == shell distance), not from a compare per table entry.
 //  * Shell sizes and the basis count are template constants (fcc 12/6/24, bcc 8/6/12), so every gather is unrolled.
+#include <algorithm>
+#include <cmath>
 #include <cstring>
 #include <type_traits>
 
@@ -292,6 +294,7 @@ struct Mc2Args {
     int team_on, team_off;        // enter TEAM when W*K >= team_on; leave it after a move with steps_done*K < team_off
     int accept_engine;            // 1: single-step windows run on the 8-lanes-per-candidate engine
     int pae;                      // 1: ... pipelined over epochs of steps (record, dirty-bitmap and offset buffers present)
+    double filt_floor;            // reject filter: absolute floor of its threshold
     uint32_t k_mq, k_sq;          // candidate index / K = umulhi(index, k_mq) >> k_sq (K >= 2)
     uint32_t rk[20];              // Philox round keys of the seed (D7): key + r * (0x9E3779B9, 0xBB67AE85), r = 0..9
     // First shell without the offset table.  A first-shell lattice vector v reaches, from basis offset beta (components
@@ -1198,7 +1201,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             // monotone), and in exact arithmetic it is a quadratic form of the first-shell count differences F:
             //   w_1 sh_1' = C + sum_r (L_r + Q_r F_r) F_r + X (F_q - F_p)^2,   coefficients per ordered species pair (p, q)
             // (DESIGN.md 6.2).  The form is evaluated in fp32 from a per-pair table row rebuilt after every move; the row's
-            // threshold = max(1.001 J_cur, 1e-18 w_1) - C + E rounded up, where E bounds (rigorously: coefficient
+            // threshold = max(1.001 J_cur, floor) - C + E rounded up (floor = 1e-18 w_1, scaled up for dilute species), where E bounds (rigorously: coefficient
             // rounding, the fp32 evaluation, the fp64 table arithmetic) the distance between the fp32 value and the exact
             // one for every admissible F, and the 0.1 % margin and the floor cover the rounding of the D6 evaluation itself.
             // A candidate above its threshold cannot improve and is dropped; the survivors are queued and evaluated exactly
@@ -1245,7 +1248,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     // E: 2^-19 A covers the fp32 coefficient roundings and the <= 16 roundings of the fp32 evaluation
                     // (gamma_16 < 2^-20) and the fp64 roundings of the table arithmetic; B and EC the cancellation in cnt - n*
                     const double E = 1.9073486328125e-6 * A + 1.000001 * (B + EC) + 1.0e-12 * fabs(Cq);
-                    const double thr = fmax(1.001 * J_cur, 1.0e-18 * Kc.w[0]) - Cq + E;
+                    const double thr = fmax(1.001 * J_cur, AA.filt_floor) - Cq + E;
                     const float thr_f = __double2float_ru(thr);
                     row[0] = (finite && isfinite(thr_f)) ? thr_f : __int_as_float(0x7f800000);   // +inf: nothing is dropped
                     row[MM] = Xf;
@@ -1650,6 +1653,17 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
         sft = (uint32_t)(l - 1);
         m = (uint32_t)(((1ull << (32 + sft)) + d - 1) / d);
     };
+    {
+        // the floor keeps the rounding of the D6 evaluation (absolute error ~ 2^-53 A per cell, A = |x| + |1-x| + |d|
+        // <= 2 / c_min + 2 + |t|) below 0.05 % of a first-shell term that reaches the threshold
+        double inv_c_max = 1.0, t_max = 0.0;
+        for (int i = 0; i < P.M; ++i) {
+            inv_c_max = std::max(inv_c_max, std::sqrt((double)P.N * (double)P.z[0] * host_tab.g[i * P.M + i]));
+            for (int j = 0; j < P.M; ++j) t_max = std::max(t_max, std::fabs(host_tab.t[i * P.M + j]));
+        }
+        const double Amax = 2.0 * inv_c_max + 2.0 + t_max;
+        AA.filt_floor = 1.0e-18 * host_tab.w[0] * std::max(1.0, (Amax / 100.0) * (Amax / 100.0));
+    }
     AA.k_mq = 0u; AA.k_sq = 0u;
     if (K >= 2) div_magic((uint64_t)K, AA.k_mq, AA.k_sq);
     div_magic((uint64_t)P.A * (uint64_t)P.L[2], G.mq, G.sq);

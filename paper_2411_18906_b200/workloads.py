@@ -120,6 +120,14 @@ def chain_sweep_workload(n_chains, n_steps=10_000):
                     shell_w=[1.0, 0.5, 0.25], n_chains=n_chains, n_steps=n_steps, K=32, seed=5)
 
 
+def large_m_workload(n_chains=16, n_steps=100_000):
+    """A cell the shared-memory (halo) MC engine cannot hold: fcc 40^3 with FIVE species (a byte per padded site does not
+    fit, nibbles hold at most four species) -- hea_mc_run falls back to the table-driven window engine with the
+    occupancy read through L2.  Shape of the paper's 5-species fcc rows (Table 1) at the c4 cell size."""
+    return Workload(name="x1-fcc40-M5", lattice="fcc", dims=(40, 40, 40), conc=[0.2] * 5, n_shells=2, shell_w=[1.0, 0.5],
+                    n_chains=n_chains, n_steps=n_steps, K=128, seed=8, target_seed=11, target_range=(-0.2, 0.2))
+
+
 RECOUNT_SWEEP_L = (10, 20, 40, 60, 80, 100)
 RECOUNT_SWEEP_B = (1, 4, 16, 64, 256, 1024)
 CHAIN_SWEEP_C = (1, 4, 16, 64, 256, 1024, 4096, 16384, 65536)

