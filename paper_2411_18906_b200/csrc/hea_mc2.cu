@@ -141,6 +141,17 @@ __device__ __forceinline__ void occ_set(uint8_t* s_occ, uint32_t pidx, uint32_t 
     }
 }
 
+// Four loaded bytes (zero-extended) into the byte slots of a word: three multiply-adds, i.e. FMA-pipe instructions (the ALU
+// pipe, which PRMT would use, is the busier one in the gather loops).
+__device__ __forceinline__ uint32_t merge4(uint32_t x0, uint32_t x1, uint32_t x2, uint32_t x3)
+{
+    uint32_t lo, hi, w;
+    asm("mad.lo.u32 %0, %1, 256, %2;" : "=r"(lo) : "r"(x1), "r"(x0));
+    asm("mad.lo.u32 %0, %1, 256, %2;" : "=r"(hi) : "r"(x3), "r"(x2));
+    asm("mad.lo.u32 %0, %1, 65536, %2;" : "=r"(w) : "r"(hi), "r"(lo));
+    return w;
+}
+
 // One-hot codes of the ZS neighbours of a site in one shell, four byte slots per accumulator word.
 // Table entries: OCC2_U8 -> padded index offset; OCC2_NIB -> 8 * byte offset + nibble shift, relative to the byte of the
 // site.  The entries of a shell are ordered by the basis index of the neighbour (see the table build), so the four
@@ -161,8 +172,7 @@ __device__ __forceinline__ void gather_shell(const uint8_t* __restrict__ s_occ, 
                 x[j] = base[OCC == OCC2_NIB ? (oj >> 3) : oj];
             }
         }
-        // bytes 1..3 of a loaded value are zero: selector 0x1140 = (x.b0, y.b0, 0, 0)
-        uint32_t w = __byte_perm(__byte_perm(x[0], x[1], 0x1140), __byte_perm(x[2], x[3], 0x1140), 0x5410);
+        uint32_t w = merge4(x[0], x[1], x[2], x[3]);
         if (OCC == OCC2_NIB) w = (w >> (o.x & 4)) & 0x0F0F0F0Fu;
         acc[g] = w;
     }
@@ -179,24 +189,43 @@ __device__ __forceinline__ void gather_first_direct(const uint8_t* __restrict__ 
         const uint32_t n = pidx + (uint32_t)(g == 0 ? rd.x : g == 1 ? rd.y : rd.z);
         const uint8_t* base = s_occ + (OCC == OCC2_NIB ? n >> 1 : n);
         const uint32_t x0 = base[fc[4 * g]], x1 = base[fc[4 * g + 1]], x2 = base[fc[4 * g + 2]], x3 = base[fc[4 * g + 3]];
-        uint32_t w = __byte_perm(__byte_perm(x0, x1, 0x1140), __byte_perm(x2, x3, 0x1140), 0x5410);
+        uint32_t w = merge4(x0, x1, x2, x3);
         if (OCC == OCC2_NIB) w = (w >> ((n & 1u) * 4u)) & 0x0F0F0F0Fu;
         acc[g] = w;
     }
 }
 
 // F[r] = #(neighbours of b of species r) - #(neighbours of a of species r) from the slot accumulators.
+// Up to three words per site (shells of at most 12 neighbours): the one-hot bits of a byte are split into even and odd
+// species, which leaves every species a 2-bit field, and the words of a site are ADDED before any per-species work.
 template <int M, int NA>
 __device__ __forceinline__ void hist_diff(const uint32_t (&accA)[NA], const uint32_t (&accB)[NA], int (&F)[M])
 {
     int last = 0;
+    if constexpr (NA <= 3) {
+        uint32_t ea = 0, oa = 0, eb = 0, ob = 0;
 #pragma unroll
-    for (int r = 0; r < M - 1; ++r) {
-        uint32_t x = (uint32_t)NA * 0x01010101u;             // per-byte bias: the byte sums stay in [0, 2 NA]
+        for (int g = 0; g < NA; ++g) {
+            ea += accA[g] & 0x55555555u; oa += (accA[g] >> 1) & 0x55555555u;
+            eb += accB[g] & 0x55555555u; ob += (accB[g] >> 1) & 0x55555555u;
+        }
 #pragma unroll
-        for (int g = 0; g < NA; ++g) x += ((accB[g] >> r) & 0x01010101u) - ((accA[g] >> r) & 0x01010101u);
-        F[r] = (int)((x * 0x01010101u) >> 24) - 4 * NA;
-        last -= F[r];
+        for (int r = 0; r < M - 1; ++r) {
+            const int sh = r & ~1;
+            const uint32_t xa = ((r & 1 ? oa : ea) >> sh) & 0x03030303u, xb = ((r & 1 ? ob : eb) >> sh) & 0x03030303u;
+            const uint32_t x = xb + (uint32_t)NA * 0x01010101u - xa;          // per byte in [0, 2 NA]
+            F[r] = (int)((x * 0x01010101u) >> 24) - 4 * NA;
+            last -= F[r];
+        }
+    } else {
+#pragma unroll
+        for (int r = 0; r < M - 1; ++r) {
+            uint32_t x = (uint32_t)NA * 0x01010101u;             // per-byte bias: the byte sums stay in [0, 2 NA]
+#pragma unroll
+            for (int g = 0; g < NA; ++g) x += ((accB[g] >> r) & 0x01010101u) - ((accA[g] >> r) & 0x01010101u);
+            F[r] = (int)((x * 0x01010101u) >> 24) - 4 * NA;
+            last -= F[r];
+        }
     }
     F[M - 1] = last;                                          // both sites have z_s entries: the differences sum to 0
 }
