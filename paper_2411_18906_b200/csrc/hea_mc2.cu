@@ -1149,21 +1149,31 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     }
                     return code;
                 };
-                const uint32_t n_iter = (n_cand + (uint32_t)T - 1u) / (uint32_t)T;
+                // two candidates per thread and pass: two independent Philox chains and eight site look-ups in flight
+                const uint32_t n_iter = (n_cand + 2u * (uint32_t)T - 1u) / (2u * (uint32_t)T);
                 for (uint32_t i2 = 0; i2 < n_iter; ++i2) {
-                    const uint32_t cnd0 = i2 * (uint32_t)T + (uint32_t)tid;
-                    const bool valid = cnd0 < n_cand;
-                    const uint32_t cnd = valid ? cnd0 : 0u;
-                    const uint32_t e_at = K == 1 ? cnd : __umulhi(cnd, AA.k_mq) >> AA.k_sq, k = cnd - e_at * (uint32_t)K;
-                    const unsigned long long step = t_ep + e_at;
-                    const uint4 r = philox4x32_10_rk((uint32_t)step, (uint32_t)(step >> 32), k, chain, AA.rk);
-                    uint32_t a1 = __umulhi(r.x, (uint32_t)N), b1 = __umulhi(r.y, (uint32_t)N - 1u);
-                    b1 += (b1 >= a1);
-                    uint32_t a2 = __umulhi(r.z, (uint32_t)N), b2 = __umulhi(r.w, (uint32_t)N - 1u);
-                    b2 += (b2 >= a2);
-                    const uint32_t h1 = species_at(a1, e_at), h2 = species_at(b1, e_at);
-                    const uint32_t h3 = species_at(a2, e_at), h4 = species_at(b2, e_at);
-                    my_null += (valid && h1 == h2 && h3 == h4) ? 1u : 0u;
+                    bool valid[2];
+                    uint32_t e_at[2], sa1[2], sb1[2], sa2[2], sb2[2];
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const uint32_t cnd0 = (2u * i2 + (uint32_t)u) * (uint32_t)T + (uint32_t)tid;
+                        valid[u] = cnd0 < n_cand;
+                        const uint32_t cnd = valid[u] ? cnd0 : 0u;
+                        e_at[u] = K == 1 ? cnd : __umulhi(cnd, AA.k_mq) >> AA.k_sq;
+                        const uint32_t k = cnd - e_at[u] * (uint32_t)K;
+                        const unsigned long long step = t_ep + e_at[u];
+                        const uint4 r = philox4x32_10_rk((uint32_t)step, (uint32_t)(step >> 32), k, chain, AA.rk);
+                        sa1[u] = __umulhi(r.x, (uint32_t)N); sb1[u] = __umulhi(r.y, (uint32_t)N - 1u);
+                        sb1[u] += (sb1[u] >= sa1[u]);
+                        sa2[u] = __umulhi(r.z, (uint32_t)N); sb2[u] = __umulhi(r.w, (uint32_t)N - 1u);
+                        sb2[u] += (sb2[u] >= sa2[u]);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const uint32_t h1 = species_at(sa1[u], e_at[u]), h2 = species_at(sb1[u], e_at[u]);
+                        const uint32_t h3 = species_at(sa2[u], e_at[u]), h4 = species_at(sb2[u], e_at[u]);
+                        my_null += (valid[u] && h1 == h2 && h3 == h4) ? 1u : 0u;
+                    }
                 }
             }
             __syncthreads();
