@@ -37,9 +37,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-MC_REJECT_WARP_INSTR = 0.0      # per 32 trials, from the round-2 ncu capture named below
-MC_REJECT_WAVEFRONTS = 0.0
-MC_FULL_WARP_INSTR = 0.0        # whole c4 launch
+MC_REJECT_WARP_INSTR = 26_472_988_180 / 6.4e7     # per 32 trials: smsp__inst_executed.sum of the 1e6-step reject launch
+MC_REJECT_WAVEFRONTS = 7_457_908_721 / 6.4e7       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum of the same launch
+MC_FULL_WARP_INSTR = 265_620_284_000.0             # whole c4 launch (16 chains x 1e7 steps)
 DTYPE = ("int32 counts + f64 objective (D6 order, no FMA); long windows pass a conservative fp32 reject filter on shell 1 "
          "first (rigorous error bound in its threshold, survivors evaluated in f64: accept decisions are the f64 ones)")
 METRIC = "delta-SRO swap trials/sec (c4: fcc 40^3, 256,000 atoms, 16 chains x 1e7 steps, K=128) incl. the full-SRO recount of the start"
@@ -58,14 +58,14 @@ def load_peaks():
 # never runs under a profiler); every use below names its source file in the JSON line.
 NCU = {
     # whole c4 trajectory, one launch: dram__bytes_read.sum + dram__bytes_write.sum
-    "mc_c4_full_dram_bytes": (7_350_016 + 49_664, "profiles/r1_mc_halo_c4_full.md"),
+    "mc_c4_full_dram_bytes": (7_293_696 + 18_432, "profiles/r2_mc_halo_c4_full.md"),
     "mc_c4_full_warp_instr": (MC_FULL_WARP_INSTR, "profiles/r2_mc_halo_c4_full.md"),
     # reject regime of c4 (1e6 steps after the trajectory): executed warp-instructions and shared-memory data-pipe
     # wavefronts per 32 trials (smsp__inst_executed.sum, l1tex__data_pipe_lsu_wavefronts_mem_shared.sum over 6.4e7 warp-trials)
     "mc_reject_warp_instr_per_32_trials": (MC_REJECT_WARP_INSTR, "profiles/r2_mc_halo_reject.md"),
     "mc_reject_smem_wavefronts_per_32_trials": (MC_REJECT_WAVEFRONTS, "profiles/r2_mc_halo_reject.md"),
-    "recount_table_L100_dram_bytes": (680_663_040, "profiles/r1_sro_count_v3.md"),
-    "recount_stencil_L100_dram_bytes": (4_030_464, "profiles/r1_sro_stencil.md"),
+    "recount_table_L100_dram_bytes": (680_581_888 + 4_061_184, "profiles/r2_recount.md"),
+    "recount_stencil_L100_dram_bytes": (4_028_928, "profiles/r2_recount.md"),
 }
 
 

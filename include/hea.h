@@ -109,6 +109,13 @@ int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host);
  *   "mc_window"       cap on the speculative step window (steps evaluated against one configuration before the
  *                     lowest improving (step, k) is applied): 0 = auto, 1 = strictly step by step, up to 2^20
  *   "mc_neighbors"    0 = auto, 1 = always the neighbour table, 2 = interior sites use site + offset (no table load)
+ *   "mc_engine"       0 = auto (2 when the padded one-hot configuration fits in shared memory), 1 = table-driven
+ *                     window engine (hea_mc.cu), 2 = shared-memory "halo" engine (hea_mc2.cu; HEA_EINVAL if it does not fit)
+ *   "mc_team"         halo engine: blocks per chain (replicas synchronised through global memory, cooperative launch),
+ *                     0 = auto (min(32, SMs / C)), 1..32;  "mc_team_on" / "mc_team_off": window sizes (candidates) at which
+ *                     a team starts / stops sharing a window, 0 = auto
+ *   "mc_accept"       halo engine, single-step windows: 0 = auto (3), 1 = thread per candidate, 2 = eight lanes per
+ *                     candidate, 3 = the warp-specialised serial engine over epochs of records computed ahead
  *   "sro_engine"      recount: 0 = auto (the table-free stencil kernel when occ_dev is aligned to the basis size,
  *                     else the table-driven kernel), 1 = table-driven (HBM-bound, 4 Z + 1 bytes per atom),
  *                     2 = stencil (1 byte per atom; HEA_EINVAL when occ_dev is not aligned)

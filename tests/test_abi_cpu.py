@@ -48,6 +48,15 @@ def test_argument_validation_precedes_device_use(L):
     assert L.hea_create(None, 0, 2, 2, 2, 2, p(conc), 1, p(w), p(t), 0) == 1
     assert L.hea_info(None, None, None, None) == 1
     assert L.hea_destroy(None) == 0
+    # the ordered pair counts are int32: max_s(z_s) * N must stay below 2^31 (fcc 283^3 with three shells: 24 * 90.6e6)
+    w3 = np.array([1.0, 0.5, 0.25]); t3 = np.zeros(12)
+    assert L.hea_create(C.byref(h), 0, 283, 283, 283, 2, p(conc), 3, p(w3), p(t3), 0) == 2
+    assert b"2^31" in L.hea_last_error()
+    # non-finite weights and targets are argument errors
+    assert L.hea_create(C.byref(h), 0, 2, 2, 2, 2, p(conc), 1, p(np.array([np.nan])), p(t), 0) == 1
+    tinf = np.zeros(4); tinf[1] = np.inf
+    assert L.hea_create(C.byref(h), 0, 2, 2, 2, 2, p(conc), 1, p(w), p(tinf), 0) == 1
+    assert L.hea_measure_peaks(None, None, 0, None) == 1
 
 
 def test_no_cpu_fallback_without_a_device(L):
