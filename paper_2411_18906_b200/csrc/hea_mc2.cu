@@ -14,6 +14,10 @@
 //  * Whether b is a neighbour of a (the exclusion of D9.2) comes from the lattice coordinates of the two sites
 //    (minimum-image displacement, squared length == shell distance), not from a compare per table entry.
 //  * Shell sizes and the basis count are template constants (fcc 12/6/24, bcc 8/6/12), so every gather is unrolled.
+//
+// Round 2: site decode by two exact multiply-high divisions, no coordinates; Philox round keys in
+// kernel-parameter space; the first shell gathered without the offset table; the reject filter of long windows as an fp32
+// quadratic form with a proven error bound in its threshold; the accept regime as a warp-specialised serial engine.
 #include <algorithm>
 #include <cmath>
 #include <cstring>
