@@ -190,7 +190,7 @@ def run_reference(args):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t_all / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": DTYPE, "data": "synthetic",
+        "vs_baseline": None, "dtype": "int32 counts + f64 objective (the oracle: D6 order, no FMA, no filter)", "data": "synthetic",
         "config": {"workload": "c4: fcc 40x40x40 (256,000 atoms), 4 species 0.25 each, shells 1-2, target seed 11, "
                                "16 chains, K=128", "mc_steps_per_step": n_steps,
                    "sample": f"the FIRST {n_steps} steps of the 1e7-step trajectory (accept regime), all K evaluated; the "
