@@ -356,7 +356,10 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: libhea_b200 has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
+    # under torchrun (RANK / WORLD_SIZE / MASTER_* in the environment) the process group is created even for one rank, so
+    # that `torchrun --nproc-per-node 1 bench.py` exercises the NCCL plumbing (barrier, MAX all-reduce of the times) on one GPU
+    use_dist = world > 1 or ("RANK" in os.environ and "MASTER_ADDR" in os.environ)
+    if use_dist:
         dist.init_process_group("nccl", device_id=dev)
     hbm_peak, sm_max_mhz, peak_src = load_peaks()
 
@@ -388,7 +391,7 @@ def main():
 
     def barrier():
         torch.cuda.synchronize()
-        if world > 1:
+        if use_dist:
             dist.barrier()
             torch.cuda.synchronize()
 
@@ -510,7 +513,7 @@ def main():
 
     # ---- reduce over ranks: max time
     times = torch.tensor([t_dev, t_rc, t_mc, t_e2e, t_wall], dtype=torch.float64, device=dev)
-    if world > 1:
+    if use_dist:
         dist.all_reduce(times, op=dist.ReduceOp.MAX)
     t_dev, t_rc, t_mc, t_e2e, t_wall = [float(x) for x in times.cpu()]
     trials_per_step = world * C * n_mc * K
@@ -580,7 +583,7 @@ def main():
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(w)
         print(json.dumps(line))
-    if world > 1:
+    if use_dist:
         dist.destroy_process_group()
 
 
