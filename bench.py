@@ -66,6 +66,8 @@ NCU = {
     "mc_reject_smem_wavefronts_per_32_trials": (MC_REJECT_WAVEFRONTS, "profiles/r2_mc_halo_reject.md"),
     "recount_table_L100_dram_bytes": (680_581_888 + 4_061_184, "profiles/r2_recount.md"),
     "recount_stencil_L100_dram_bytes": (4_028_928, "profiles/r2_recount.md"),
+    # table-free recount on fcc 100^3, batch 1: smsp__inst_executed.sum of one launch
+    "recount_stencil_L100_warp_instr": (17_792_245, "profiles/r2_recount.md"),
 }
 
 
@@ -508,7 +510,9 @@ def main():
                            "workload": f"fcc {args.recount_L}^3 ({hr.N} atoms), 5 species, 3 shells, batch 1; 1 byte per atom",
                            "atoms_per_s": hr.N / t_s, "ms_per_launch": t_s * 1e3,
                            "hbm_GBps": hr.N / t_s / 1e9, "speedup_vs_table_kernel": t_r / t_s,
-                           "peak_source": "SMs x 128 lanes/clk x max SM clock (DESIGN.md section 6)"}
+                           "peak_source": "SMs x 128 lanes/clk x max SM clock (DESIGN.md section 6)",
+                           "executed_warp_instr_per_launch": NCU["recount_stencil_L100_warp_instr"][0] if args.recount_L == 100 else None,
+                           "executed_source": NCU["recount_stencil_L100_warp_instr"][1]}
         hr.close()
 
     # ---- reduce over ranks: max time
@@ -577,6 +581,10 @@ def main():
     if args.workload != 4 or args.chains:
         line["config"]["workload"] = f"EXPLORATION (not the metric's workload): {w.name}, {C} chains, K={K}, N={N}"
     if recount:
+        if recount_stencil.get("executed_warp_instr_per_launch"):
+            ex_T = recount_stencil["executed_warp_instr_per_launch"] * 32 / (recount_stencil["ms_per_launch"] * 1e-3) / 1e12
+            recount_stencil["executed"] = {"achieved": ex_T, "peak": issue_peak_T, "unit": "T thread-instr/s",
+                                           "frac": ex_T / issue_peak_T, "peak_source": "measured issue ceiling (hea_measure_peaks)"}
         line["recount_roofline"] = recount
         line["recount_stencil"] = recount_stencil
     if rank == 0:

@@ -336,3 +336,16 @@ def test_product_sharding_union_equals_single_call(hb, world):
         part = hb.stats_to_numpy(s_r)
         for f in ("n_accept", "n_null", "hash", "last_accept_step", "J"):
             np.testing.assert_array_equal(part[f], whole[f][c0:c0 + cnt])
+
+
+def test_measure_peaks_reports_sane_rates(hb):
+    # hea_measure_peaks (roofline denominators): whole-chip rates of a B200-class part, internally consistent
+    h, _ = pair(hb, small("bcc", (3, 3, 3), [0.5, 0.5], 1))
+    pk = h.measure_peaks()
+    assert set(pk) == set(h.PEAK_NAMES)
+    assert 1e11 < pk["lds_wavefronts_per_s"] < 1e12 and 1e12 < pk["lds_u8_random_gathers_per_s"] < 32 * pk["lds_wavefronts_per_s"]
+    assert 5e12 < pk["alu_pipe_instr_per_s"] < 5e13 and 5e12 < pk["fma_pipe_int_instr_per_s"] < 5e13
+    assert max(pk["alu_pipe_instr_per_s"], pk["fma_pipe_int_instr_per_s"]) < pk["issue_instr_per_s"] < 1e14
+    assert 1e12 < pk["fp64_instr_per_s"] < 1e14 and 1e3 < pk["l2_random_sector_GBps"] < 1e5
+    with pytest.raises(hb.HeaError):
+        hb._check(hb.lib().hea_measure_peaks(h._h, None, 8, None))
