@@ -171,6 +171,10 @@ int hea_mc_stats_reset(hea_ctx* ctx, hea_mc_stats* stats_dev, int64_t C, void* c
  *   log_dev    [C][log_cap] accepted moves of THIS call in order (first log_cap of them), or NULL with log_cap 0
  *   K in [1, HEA_MAX_K].  Results depend only on (seed, chain id, step), never on C, batching or tuning options:
  *   run(S1) followed by run(S2, step0 = S1) equals run(S1 + S2).
+ *   Arithmetic: int32 counts, fp64 objective in the D6 order.  With a bit-symmetric target and weights >= 0, long windows
+ *   first pass a conservative fp32 reject filter on the first shell (the paper's own reduced precision: P:297); its
+ *   threshold carries a proven error bound and every survivor is evaluated in fp64, so the accept decisions are exactly
+ *   those of the fp64 rule.
  */
 int hea_mc_run(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C, uint64_t n_steps, int K,
                uint64_t seed, uint64_t chain0, uint64_t step0,
