@@ -13,6 +13,7 @@
  *   hea_mc_run_ex     the same with the paper's own selection and termination: best-of-K (Eq. 6) and the
  *                     search-depth counter (Alg. 3)  (A23)
  *   hea_pool_select   selection step of the global search (Alg. 1)  (A24)
+ *   hea_pool_rank_static  its ranking step with no device allocation (static scratch of a fixed size)
  *
  * Conventions for every call
  *   - All functions return HEA_OK (0) or an error code; hea_last_error() gives a thread-local message.
@@ -214,6 +215,24 @@ int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C
  */
 int hea_pool_select(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, hea_mc_stats* stats_dev, int64_t C,
                     int64_t n_keep, uint64_t seed, uint64_t new_chain0, int32_t* order_dev, void* cuda_stream);
+
+/*
+ * hea_pool_rank_static -- the ranking step of hea_pool_select (Alg. 1; A24) for callers that cannot allocate
+ * device memory (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): this call allocates
+ * nothing, on the host side of the device or on the device -- no cudaMalloc, cudaFree or allocating library routine.
+ *   counts_dev [C][S][M][M] in: the recount of each chain;  order_dev [n_keep] int32 out: order_dev[r] = index of the chain
+ *   of rank r by J (D6) ascending, ties -> lower index -- what hea_pool_select(n_keep) reports in its order_dev.
+ * Its scratch (J of every chain) is a static device array inside the library of HEA_POOL_RANK_STATIC_MAX doubles
+ * (512 KB) that every GPU loading the library holds until the process exits.  C > HEA_POOL_RANK_STATIC_MAX -> HEA_EINVAL
+ * with a message naming the limit (hea_pool_select has no such limit below 65,536 but allocates).
+ * The array is shared by EVERY call in the process, whatever the context, and keeps the last call's contents; this
+ * call overwrites the entries it reads, so nothing needs clearing.  Calls that overlap on one GPU (different streams,
+ * contexts or threads) race on it: order them on one stream or synchronise between them.  The first call on a device
+ * resolves the array's device address (cudaGetSymbolAddress; not an allocation).  Asynchronous on cuda_stream.
+ */
+#define HEA_POOL_RANK_STATIC_MAX 65536
+int hea_pool_rank_static(hea_ctx* ctx, const int32_t* counts_dev, int64_t C, int64_t n_keep, int32_t* order_dev,
+                         void* cuda_stream);
 
 /*
  * Host-buffer (end-to-end) forms: the same kernels, with host<->device copies done by the library on an internal

@@ -23,7 +23,8 @@ MOVE_DTYPE = np.dtype([("step", "<u8"), ("k", "<u4"), ("a", "<u4"), ("b", "<u4")
 
 EXPORTS = ["hea_version", "hea_last_error", "hea_create", "hea_destroy", "hea_info", "hea_neighbor_table",
            "hea_set_option", "hea_get_option", "hea_init_random", "hea_sro_full", "hea_mc_stats_reset",
-           "hea_mc_run", "hea_mc_run_ex", "hea_pool_select", "hea_sro_full_host", "hea_mc_run_host", "hea_launch_count", "hea_measure_peaks"]
+           "hea_mc_run", "hea_mc_run_ex", "hea_pool_select", "hea_sro_full_host", "hea_mc_run_host", "hea_launch_count", "hea_measure_peaks",
+           "hea_pool_rank_static"]
 
 
 class HeaError(RuntimeError):
@@ -62,6 +63,7 @@ def lib():
         L.hea_mc_run_host.argtypes = [vp, vp, vp, i64, u64, i32, u64, u64, u64, vp]
         L.hea_launch_count.argtypes = [vp, vp]
         L.hea_measure_peaks.argtypes = [vp, vp, i32, vp]
+        L.hea_pool_rank_static.argtypes = [vp, vp, i64, i64, vp, vp]
         _lib = L
     return _lib
 
@@ -201,6 +203,14 @@ class Hea:
         _check(lib().hea_pool_select(self._h, C.c_void_p(occ.data_ptr()), C.c_void_p(counts.data_ptr()),
                                      C.c_void_p(stats.data_ptr()), n, n_keep, seed, new_chain0,
                                      C.c_void_p(order.data_ptr()), _stream()))
+        return order[:n_keep]
+
+    POOL_RANK_STATIC_MAX = 65536
+
+    def pool_rank_static(self, counts, n_keep, order):
+        """hea_pool_rank_static: order[:n_keep] = chain indices by ascending J; allocates nothing (order is the caller's)."""
+        _check(lib().hea_pool_rank_static(self._h, C.c_void_p(counts.data_ptr()), counts.shape[0], n_keep,
+                                          C.c_void_p(order.data_ptr()), _stream()))
         return order[:n_keep]
 
     # ---- host-buffer (end-to-end) calls: numpy arrays in, synchronous

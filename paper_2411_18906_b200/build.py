@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhea_b200.so")
-SOURCES = ["hea_api.cu", "hea_sro.cu", "hea_sro2.cu", "hea_mc.cu", "hea_mc2.cu", "hea_mc2_p1.cu", "hea_mc2_p2.cu", "hea_mc2_p3.cu", "hea_pool.cu", "hea_peaks.cu", "hea_lattice.cpp"]
+SOURCES = ["hea_api.cu", "hea_sro.cu", "hea_sro2.cu", "hea_mc.cu", "hea_mc2.cu", "hea_mc2_p1.cu", "hea_mc2_p2.cu", "hea_mc2_p3.cu", "hea_pool.cu", "hea_peaks.cu", "hea_noalloc.cu", "hea_lattice.cpp"]
 HEADERS = ["hea_mc2.cu", "hea_device.cuh", "hea_mc_common.cuh", "hea_lattice.hpp", os.path.join("..", "..", "include", "hea.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread"]

@@ -36,6 +36,8 @@ cudaError_t launch_pool_gather(const void* src, void* dst, const int32_t* order,
                                cudaStream_t st, int64_t* n_launches);
 size_t mc2_team_bytes(int64_t C);
 cudaError_t measure_peaks(int n_sms, int clock_khz, double* out, cudaStream_t st, int64_t* n_launches);
+cudaError_t pool_rank_static(const KParams& P, int device, const int32_t* counts, int64_t C, int64_t n_keep, int32_t* order,
+                             cudaStream_t st, int64_t* n_launches, std::string* err);
 constexpr int kMc2MaxThreads = 512;
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
                        void* team_ctl, int team_on, int team_off, int accept_engine, size_t smem_budget, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
@@ -567,6 +569,25 @@ int hea_pool_select(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, hea_mc_
         if ((rc = hea_sro_full(ctx, occ_dev + N * (size_t)n_keep, n_new, counts_dev + SMM * (size_t)n_keep, nullptr, nullptr, cuda_stream)) != HEA_OK) return rc;
         if ((rc = hea_mc_stats_reset(ctx, stats_dev + n_keep, n_new, cuda_stream)) != HEA_OK) return rc;
     }
+    return HEA_OK;
+}
+
+int hea_pool_rank_static(hea_ctx* ctx, const int32_t* counts_dev, int64_t C, int64_t n_keep, int32_t* order_dev, void* cuda_stream)
+{
+    // allocation-free: no ensure_scratch, no cudaMalloc / cudaFree on this path (the scratch is the static array of hea_noalloc.cu)
+    if (!ctx) return fail(HEA_EINVAL, "ctx is NULL");
+    if (C < 0 || n_keep < 0 || n_keep > C) return fail(HEA_EINVAL, "need 0 <= n_keep <= C");
+    if (C > HEA_POOL_RANK_STATIC_MAX)
+        return fail(HEA_EINVAL, "hea_pool_rank_static: C = " + std::to_string(C) + " chains exceed the static scratch of HEA_POOL_RANK_STATIC_MAX = " +
+                                    std::to_string(HEA_POOL_RANK_STATIC_MAX) + " (use hea_pool_select, which allocates)");
+    if (C == 0 || n_keep == 0) return HEA_OK;
+    if (!counts_dev || !order_dev) return fail(HEA_EINVAL, "counts_dev / order_dev is NULL");
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return fail(HEA_ECUDA, "cannot make the context's device current");
+    std::string err;
+    cudaError_t e = hea::pool_rank_static(ctx->P, ctx->device, counts_dev, C, n_keep, order_dev, (cudaStream_t)cuda_stream,
+                                          &ctx->n_launches, &err);
+    if (e != cudaSuccess) return fail(HEA_ECUDA, "hea_pool_rank_static: " + err);
     return HEA_OK;
 }
 
