@@ -42,7 +42,7 @@ constexpr int kMc2MaxThreads = 512;
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
                        void* team_ctl, int team_on, int team_off, int accept_engine, size_t smem_budget, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
                        uint64_t step0, void* stats, void* log, int64_t log_cap, int select_best, uint64_t depth_limit,
-                       uint64_t* depth, uint64_t* steps_done, cudaStream_t st, int64_t* n_launches);
+                       uint64_t* depth, uint64_t* steps_done, uint32_t* hist, cudaStream_t st, int64_t* n_launches);
 }  // namespace hea
 
 struct hea_ctx {
@@ -58,12 +58,12 @@ struct hea_ctx {
     int64_t* d_nps = nullptr;
     hea::KParams P{};
     // tuning options (0 = auto)
-    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0, opt_neighbors = 0, opt_engine = 0, opt_team = 0, opt_team_on = 0, opt_team_off = 0, opt_accept = 0, opt_sro_stages = 0, opt_sro_bps = 0, opt_sro_warps = 0, opt_sro_engine = 0, opt_sro_tile_xy = 0, opt_sro_tile_z = 0, opt_sro_flush = 0, opt_sro_threads = 0, opt_sro_lanes = 0;
+    int64_t opt_occ_mode = 0, opt_threads = 0, opt_cluster = 0, opt_window = 0, opt_neighbors = 0, opt_engine = 0, opt_team = 0, opt_team_on = 0, opt_team_off = 0, opt_accept = 0, opt_hist = 0, opt_sro_stages = 0, opt_sro_bps = 0, opt_sro_warps = 0, opt_sro_engine = 0, opt_sro_tile_xy = 0, opt_sro_tile_z = 0, opt_sro_flush = 0, opt_sro_threads = 0, opt_sro_lanes = 0;
     int64_t n_launches = 0;
     // internal stream and scratch for the *_host entry points
     cudaStream_t stream = nullptr;
-    void* scratch[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    size_t scratch_cap[6] = {0, 0, 0, 0, 0, 0};
+    void* scratch[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    size_t scratch_cap[7] = {0, 0, 0, 0, 0, 0, 0};
 };
 
 namespace {
@@ -119,6 +119,7 @@ int64_t* option_slot(hea_ctx* ctx, const char* name)
     if (!strcmp(name, "mc_engine")) return &ctx->opt_engine;
     if (!strcmp(name, "mc_team")) return &ctx->opt_team;
     if (!strcmp(name, "mc_accept")) return &ctx->opt_accept;
+    if (!strcmp(name, "mc_hist")) return &ctx->opt_hist;
     if (!strcmp(name, "mc_team_on")) return &ctx->opt_team_on;
     if (!strcmp(name, "mc_team_off")) return &ctx->opt_team_off;
     if (!strcmp(name, "sro_stages")) return &ctx->opt_sro_stages;
@@ -144,6 +145,7 @@ bool option_value_ok(const char* name, int64_t v)
     if (!strcmp(name, "mc_engine")) return v == 1 || v == 2;
     if (!strcmp(name, "mc_team")) return v >= 1 && v <= 32;
     if (!strcmp(name, "mc_accept")) return v >= 1 && v <= 3;      // 1 off, 2 single-step engine, 3 (= default) pipelined
+    if (!strcmp(name, "mc_hist")) return v == 1 || v == 2;        // 1 off, 2 on wherever the kernel can use it
     if (!strcmp(name, "mc_team_on") || !strcmp(name, "mc_team_off")) return v >= 1 && v <= (1 << 30);
     if (!strcmp(name, "sro_stages")) return v >= 1 && v <= 8;
     if (!strcmp(name, "sro_blocks_per_sm")) return v >= 1 && v <= 4;
@@ -483,12 +485,20 @@ int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C
             if (rc != HEA_OK) return rc;
             team_ctl = ctx->scratch[5];
         }
+        // site-histogram table of the reject filter: 4 bytes per site and chain, kept in L2.  Default: for
+        // teams (few chains, large cells); mc_hist = 2 also for one block per chain, mc_hist = 1 never.
+        uint32_t* hist = nullptr;
+        if (ctx->M >= 2 && ctx->M <= 5 && ctx->opt_hist != 1 && (team > 1 || ctx->opt_hist == 2)) {
+            int rc = ensure_scratch(ctx, 6, sizeof(uint32_t) * (size_t)N * (size_t)C);
+            if (rc != HEA_OK) return rc;
+            hist = (uint32_t*)ctx->scratch[6];
+        }
         const int w_max2 = ctx->opt_window ? (int)ctx->opt_window : (1 << 20);
         cudaError_t e2 = hea::launch_mc2(ctx->P, ctx->tab_host, ctx->lat.type, om, threads, team, team_ctl,
                                          (int)ctx->opt_team_on, (int)ctx->opt_team_off,
                                          ctx->opt_accept == 1 ? 0 : ctx->opt_accept == 2 ? 1 : 2, budget, w_max2, occ_dev, counts_dev, C,
                                          n_steps, K, seed, chain0, step0, stats_dev, log_dev, log_cap, select_best,
-                                         depth_limit, depth_dev, steps_done_dev, (cudaStream_t)cuda_stream,
+                                         depth_limit, depth_dev, steps_done_dev, hist, (cudaStream_t)cuda_stream,
                                          &ctx->n_launches);
         return e2 == cudaSuccess ? HEA_OK : fail_cuda(e2, "hea_mc_run launch (halo engine)");
     }

@@ -59,7 +59,7 @@ struct Geo {
     int distinct;                 // every L >= 3: a site pair is joined by at most one lattice vector of a shell
 };
 
-constexpr int kQueueCap = 2048;
+constexpr int kQueueCap = 1024;
 constexpr int kPaeK = 16;                   // pipelined accept engine: candidates per step evaluated ahead
 constexpr int kPaeRecs = 512;               // records per epoch (= block threads): kPaeRecs / kPaeK steps
 
@@ -304,7 +304,8 @@ struct TeamCtl {
     unsigned long long t0;        // next step
     double J;
     unsigned long long depth;     // search-depth counter (hea_mc_run_ex)
-    uint32_t pad[8];
+    uint32_t hist_bar;            // arrivals at the team barrier that ends a site-histogram build (monotone)
+    uint32_t pad[7];
     TeamSlot slot[2][kMaxTeam];   // [team-window parity][rank]
 };
 
@@ -327,7 +328,11 @@ struct Mc2Args {
     int team_on, team_off;        // enter TEAM when W*K >= team_on; leave it after a move with steps_done*K < team_off
     int accept_engine;            // 1: single-step windows run on the 8-lanes-per-candidate engine
     int pae;                      // 1: ... pipelined over epochs of steps (record, dirty-bitmap and offset buffers present)
+    int dshift;                   //    log2 of the sites per bit of its touched-site bitmap
     double filt_floor;            // reject filter: absolute floor of its threshold
+    uint32_t* hist;               // [C][N] site-histogram table of the reject filter, or nullptr: per site
+                                  // species << 24 | first-shell neighbour counts of species 0..M-2 in fields of 8 (M <= 4) or
+                                  // 6 (M = 5) bits; read and written through L2 only
     uint32_t k_mq, k_sq;          // candidate index / K = umulhi(index, k_mq) >> k_sq (K >= 2)
     uint32_t rk[20];              // Philox round keys of the seed (D7): key + r * (0x9E3779B9, 0xBB67AE85), r = 0..9
     // First shell without the offset table.  A first-shell lattice vector v reaches, from basis offset beta (components
@@ -343,6 +348,165 @@ struct Mc2Args {
     unsigned long long* depth_all;         // [C] in/out, or nullptr
     unsigned long long* steps_done_all;    // [C] out, or nullptr
 };
+
+// ---- stage 1 of a long window from the site-histogram table
+struct HistArgs {                 // the same in every thread of the block
+    const uint32_t* H;            // the chain's table: species << 24 | first-shell neighbour counts of species 0..M-2
+    const uint32_t* rk;           // Philox round keys (Mc2Args::rk)
+    // shared-memory objects as 32-bit shared-space addresses (a generic pointer would make every access a generic LD / ATOM)
+    uint32_t best_slot;           // lowest improving key found so far in this window
+    uint32_t ftab;                // reject-filter table, element-major
+    uint32_t queue;               // keys of the survivors
+    uint32_t q_n;
+    unsigned long long t0;        // first step of the window
+    uint32_t Wc, ts_inc, k_inc, K, N, chain;
+    int Lx, Ly, Lz;
+    uint32_t mx, sx, mq, sq;      // site / (A Ly Lz), site / (A Lz) by multiply-high (Geo)
+    uint32_t basis;
+    int d2_0;                     // squared first-shell distance, doubled units
+};
+
+struct HistScan {                 // one thread's scan of its candidates of the window
+    uint32_t ts, k;               // next candidate (window step, k)
+    uint32_t ncur;                // null bits of the current group of 32 candidates
+    int j;                        // candidates scanned
+    uint32_t nullw[kNullWords];
+    uint32_t ovf[4];              // survivors that found the queue full: the caller evaluates them
+    int n_ovf;
+    int done;
+};
+
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t lds_volatile_u32(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ float lds_f32(uint32_t a)
+{
+    float v;
+    asm("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t atoms_inc(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+
+// Scans this thread's candidates in batches of four: Philox, the two table words (two more after a redraw, D9.1), null bit,
+// first-shell adjacency (D9.2), F = difference of the neighbour counts, the fp32 form of the reject filter; survivors go
+// to the queue.  Not inlined on purpose: inside the kernel body the loop would share 128 registers with everything else
+// that is live there, and the allocator then reuses load destinations, which serialises the L2 round trips.
+template <int M, int LAT, bool BEST>
+__device__ __noinline__ void hist_scan(HistScan& st, const HistArgs& A)
+{
+    constexpr int U = 4;
+    static_assert(32 % U == 0, "null words are closed on batch boundaries");
+    constexpr int MM = M * M;
+    constexpr int HFB = M <= 4 ? 8 : 6;
+    constexpr uint32_t HFM = (1u << HFB) - 1u;
+    constexpr uint32_t kBias = (M > 1 ? 16u : 0u) | (M > 2 ? 16u << HFB : 0u) | (M > 3 ? 16u << (2 * HFB) : 0u) |
+                               (M > 4 ? 16u << (3 * HFB) : 0u);
+    using LC = LatC<LAT>;
+    uint32_t rk[20];
+#pragma unroll
+    for (int i = 0; i < 20; ++i) rk[i] = A.rk[i];
+    const uint32_t* __restrict__ H = A.H;
+    const uint32_t N = A.N, K = A.K, Wc = A.Wc, ts_inc = A.ts_inc, k_inc = A.k_inc, chain = A.chain;
+    const unsigned long long t0 = A.t0;
+    const int Lx = A.Lx, Ly = A.Ly, Lz = A.Lz;
+    const uint32_t Lxy = (uint32_t)(Lx * Ly);
+    uint32_t ts = st.ts, k = st.k, ncur = st.ncur;
+    int j = st.j;
+    int n_ovf = 0;
+    bool done = true;
+    while (ts < Wc) {
+        const uint32_t hint = lds_volatile_u32(A.best_slot);
+        if ((hint >> 10) < ts) break;                               // a move at an earlier step exists
+        if (n_ovf != 0) { done = false; break; }                    // hand the overflow to the caller first
+        uint32_t key[U], a[U], b[U], ha[U], hb[U], rx[U], rz[U], rw[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            key[u] = ts < Wc ? ((ts << 10) | k) : kNoKey;
+            const unsigned long long step = t0 + ts;
+            const uint4 r = philox4x32_10_rk((uint32_t)step, (uint32_t)(step >> 32), k, chain, rk);
+            a[u] = __umulhi(r.x, N); b[u] = __umulhi(r.y, N - 1u);
+            b[u] += (b[u] >= a[u]);
+            rx[u] = r.x; rz[u] = r.z; rw[u] = r.w;
+            ha[u] = __ldcg(H + a[u]); hb[u] = __ldcg(H + b[u]);
+            k += k_inc; ts += ts_inc;
+            if (k >= K) { k -= K; ++ts; }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (((ha[u] ^ hb[u]) >> 24) == 0u) {                    // like species: redraw once (D9.1)
+                rx[u] = rz[u];
+                a[u] = __umulhi(rz[u], N); b[u] = __umulhi(rw[u], N - 1u);
+                b[u] += (b[u] >= a[u]);
+                ha[u] = __ldcg(H + a[u]); hb[u] = __ldcg(H + b[u]);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int p = (int)(ha[u] >> 24), q = (int)(hb[u] >> 24);
+            ncur = __funnelshift_r(ncur, p == q ? 1u : 0u, 1);
+            if (p != q && key[u] != kNoKey && (BEST || key[u] < hint)) {
+                // D9.2: are a and b first-shell neighbours?  The cell coordinates of a come straight from its random word
+                // (floor(floor(r N / 2^32) / d) = floor(r (N / d) / 2^32)); almost every pair fails on x or y
+                const uint32_t xa = __umulhi(rx[u], (uint32_t)Lx), qa = __umulhi(rx[u], Lxy);
+                const uint32_t xb = __umulhi(b[u], A.mx) >> A.sx, qb = __umulhi(b[u], A.mq) >> A.sq;
+                const int cx = (int)xb - (int)xa, cy = (int)(qb - qa) - cx * Ly;
+                const int ax = abs(cx), ay = abs(cy);
+                int mm0 = 0;
+                if ((ax <= 1 || ax == Lx - 1) && (ay <= 1 || ay == Ly - 1)) {
+                    const int za = (int)((a[u] >> LC::lgA) - qa * (uint32_t)Lz), zb = (int)((b[u] >> LC::lgA) - qb * (uint32_t)Lz);
+                    const int ba = (int)(a[u] & (uint32_t)(LC::A - 1)), bb = (int)(b[u] & (uint32_t)(LC::A - 1));
+                    const int dx = 2 * cx + (int)((A.basis >> (3 * bb)) & 1u) - (int)((A.basis >> (3 * ba)) & 1u);
+                    const int dy = 2 * cy + (int)((A.basis >> (3 * bb + 1)) & 1u) - (int)((A.basis >> (3 * ba + 1)) & 1u);
+                    const int dz = 2 * (zb - za) + (int)((A.basis >> (3 * bb + 2)) & 1u) - (int)((A.basis >> (3 * ba + 2)) & 1u);
+                    const int wx = dx > Lx ? dx - 2 * Lx : dx < -Lx ? dx + 2 * Lx : dx;
+                    const int wy = dy > Ly ? dy - 2 * Ly : dy < -Ly ? dy + 2 * Ly : dy;
+                    const int wz = dz > Lz ? dz - 2 * Lz : dz < -Lz ? dz + 2 * Lz : dz;
+                    mm0 = (wx * wx + wy * wy + wz * wz) == A.d2_0;
+                }
+                const uint32_t X = (hb[u] & 0xFFFFFFu) + kBias - (ha[u] & 0xFFFFFFu);      // fields in [4, 28]: no borrow
+                int F0[M];
+                int last = 0;
+#pragma unroll
+                for (int r2 = 0; r2 < M - 1; ++r2) {
+                    F0[r2] = (int)((X >> (HFB * r2)) & HFM) - 16;
+                    last -= F0[r2];
+                }
+                F0[M - 1] = last;
+                if (mm0 != 0) {
+#pragma unroll
+                    for (int r2 = 0; r2 < M; ++r2) F0[r2] -= (r2 == p) - (r2 == q);
+                }
+                const uint32_t row = A.ftab + 4u * (uint32_t)(p * M + q);       // element e at row + 4 e MM
+                float acc = 0.0f, D = 0.0f;
+#pragma unroll
+                for (int r2 = 0; r2 < M; ++r2) {
+                    const float f = (float)F0[r2];
+                    acc = fmaf(fmaf(lds_f32(row + 4u * (2 + M + r2) * MM), f, lds_f32(row + 4u * (2 + r2) * MM)), f, acc);
+                    D = fmaf(lds_f32(row + 4u * (2 + 2 * M + r2) * MM), f, D);
+                }
+                acc = fmaf(lds_f32(row + 4u * MM) * D, D, acc);
+                if (!(acc > lds_f32(row))) {
+                    const uint32_t slot = atoms_inc(A.q_n);
+                    if (slot < (uint32_t)kQueueCap) sts_u32(A.queue + 4u * slot, key[u]);
+                    else st.ovf[n_ovf++] = key[u];
+                }
+            }
+        }
+        j += U;
+        if ((j & 31) == 0) st.nullw[(j >> 5) - 1] = ncur;
+    }
+    st.ts = ts; st.k = k; st.ncur = ncur; st.j = j; st.n_ovf = n_ovf; st.done = done ? 1 : 0;
+}
 
 // Shared memory: occupancy (offset 0, so a gather address is the loaded offset itself) | Sh2 | offset table [A][ZP].
 template <int M, int OCC, bool SYM, int LAT, bool BEST>
@@ -366,7 +530,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     float* s_ftab = reinterpret_cast<float*>(s_tab + LC::A * ZP);       // [RS][M*M] reject-filter table, element-major
     PRec* s_prec = reinterpret_cast<PRec*>(s_ftab + ((MM * RS + 3) & ~3));
     uint32_t* s_dirty = reinterpret_cast<uint32_t*>(s_prec + kPaeRecs);
-    int* s_loff = reinterpret_cast<int*>(s_dirty + ((P.N + 31) >> 5));
+    // one bit per group of 2^dshift consecutive sites (coarser = conservative: more records count as stale)
+    const uint32_t dshift = (uint32_t)AA.dshift;
+    const int dwords = (int)(((((uint32_t)P.N + (1u << dshift) - 1u) >> dshift) + 31u) >> 5);
+    int* s_loff = reinterpret_cast<int*>(s_dirty + dwords);
     // serial accept engine: packed count changes per objective row of the improving records, [step parity][record][S*M]
     unsigned long long* s_dn = reinterpret_cast<unsigned long long*>(
         (reinterpret_cast<uintptr_t>(s_loff + LC::A * P.Z) + 7u) & ~(uintptr_t)7u);
@@ -450,7 +617,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         sh.W1[i] = Kc.w[0] * gi * gi;
     }
     if (AA.pae) {
-        for (int i = tid; i < ((P.N + 31) >> 5); i += T) s_dirty[i] = 0u;
+        for (int i = tid; i < dwords; i += T) s_dirty[i] = 0u;
         for (int i = tid; i < LC::A * P.Z; i += T) {      // neighbour e of a site of basis b without periodic wrap
             const int8_t* st = P.tab->stencil + i * 4;
             const int b = i / P.Z;
@@ -533,9 +700,9 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         const bool interior = sc.x >= 1 && sc.x <= Lx - 2 && sc.y >= 1 && sc.y <= Ly - 2 && sc.z >= 1 && sc.z <= Lz - 2;
         for (int e = lane; e < P.Z; e += 32) {
             const uint32_t v = interior ? u + (uint32_t)s_loff[sc.b * P.Z + e] : (uint32_t)__ldg(P.nbr_site + (size_t)u * P.Z + e);
-            atomicOr(&s_dirty[v >> 5], 1u << (v & 31u));
+            atomicOr(&s_dirty[v >> (5u + dshift)], 1u << ((v >> dshift) & 31u));
         }
-        if (lane == 0) atomicOr(&s_dirty[u >> 5], 1u << (u & 31u));
+        if (lane == 0) atomicOr(&s_dirty[u >> (5u + dshift)], 1u << ((u >> dshift) & 31u));
     };
     auto mark_touched = [&](uint32_t ma, uint32_t mb, int lane) {
         mark_one(ma, lane);
@@ -627,6 +794,62 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 if (e < P.zoff[1]) mm0 += hit; else if (e < P.zoff[2]) mm1 += hit; else mm2 += hit;
             }
             mm0 -= P.m_self[0]; mm1 -= P.m_self[1]; mm2 -= P.m_self[2];
+        }
+    };
+
+    // ---- site-histogram table of the reject filter.  The filter needs, per candidate, only the species
+    // of the two sites and the difference of their first-shell neighbour counts.  Both are kept PER SITE in a 32-bit word
+    // (species << 24 | counts of species 0..M-2) in global memory, read through L2: a candidate of a long window is then
+    // Philox, two loads and the fp32 form -- no site decode, no gathers.  Moves are rare where long windows run, and a move
+    // changes the words of its two sites and of their 2 z_1 neighbours, which are recomputed from the configuration.
+    // Every block of a team writes the same values (its replica of the configuration is the same), so no block waits
+    // for another: its own stores are fenced before its next window, and the window exchange orders the stores of
+    // consecutive moves.  The table is built when a phase of long windows starts (each block a slice, then a team barrier).
+    constexpr int HFB = M <= 4 ? 8 : 6;
+    constexpr uint32_t HFM = (1u << HFB) - 1u;
+    uint32_t* const g_hist = (M >= 2 && M <= 5 && AA.hist != nullptr && G.distinct) ? AA.hist + chain_local * (size_t)N : nullptr;
+    bool hist_valid = false, hist_pending = false;
+    uint32_t hist_a = 0u, hist_b = 0u, hist_epoch = 0u;
+    auto hist_word = [&](uint32_t site) -> uint32_t {
+        const SiteC sc = decode_site<LAT>(G, site);
+        uint32_t acc[NA0];
+        gather_first_direct<OCC, NA0>(s_occ, sh.fs_rd[sc.b], sc.pidx, AA.fs_c, acc);
+        uint32_t h = (uint32_t)(31 - __clz((int)occ_get<OCC>(s_occ, sc.pidx))) << 24;
+#pragma unroll
+        for (int r = 0; r < M - 1; ++r) {
+            uint32_t x = 0u;
+#pragma unroll
+            for (int g = 0; g < NA0; ++g) x += (acc[g] >> r) & 0x01010101u;
+            h |= ((x * 0x01010101u) >> 24) << (HFB * r);
+        }
+        return h;
+    };
+    auto hist_build = [&]() {
+        const uint32_t per = ((uint32_t)N + (uint32_t)R - 1u) / (uint32_t)R;
+        const uint32_t lo = rank * per, hi = min((uint32_t)N, lo + per);
+        for (uint32_t i = lo + (uint32_t)tid; i < hi; i += (uint32_t)T) __stcg(g_hist + i, hist_word(i));
+        __threadfence();
+        __syncthreads();
+        if (R > 1) {
+            ++hist_epoch;
+            if (tid == 0) {
+                __threadfence();
+                atomicAdd(&ctl->hist_bar, 1u);
+                while (ld_acquire_u32(&ctl->hist_bar) < hist_epoch * (uint32_t)R) { }
+            }
+            __syncthreads();
+        }
+    };
+    // the words of the two sites of a move and of their first-shell neighbours, by the last warp of the block
+    auto hist_update = [&](uint32_t ma, uint32_t mb) {
+        if (tid >= T - 32) {
+            for (int e = tid - (T - 32); e < 2 * LC::z0 + 2; e += 32) {
+                const uint32_t v = e < LC::z0       ? (uint32_t)__ldg(nbr + (size_t)ma * P.Z + e)
+                                 : e < 2 * LC::z0   ? (uint32_t)__ldg(nbr + (size_t)mb * P.Z + (e - LC::z0))
+                                 : e == 2 * LC::z0  ? ma : mb;
+                __stcg(g_hist + v, hist_word(v));
+            }
+            __threadfence();
         }
     };
 
@@ -800,6 +1023,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         }
         uint32_t key_best = kNoKey, steps_done = 1u;
         if (accept_ok && !team && W == 1u && AA.pae) {
+            hist_valid = false; hist_pending = false;            // moves of this engine do not maintain the site histograms
             // ---- serial accept engine.  In the accept regime nearly every step applies a move found among its first few
             // candidates, so a chain advances one dependent move at a time and what counts is the latency of a step.
             // (P) What depends only on the configuration (proposal, adjacency, the 2Z gathers) is computed AHEAD for an
@@ -890,7 +1114,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     const bool is_eval = tid < 128;
                     const int grp = (tid >> 3) & 15, l8 = tid & 7;
                     const int SMr = S * M;
-                    auto dirty = [&](uint32_t v) { return (s_dirty[v >> 5] >> (v & 31u)) & 1u; };
+                    auto dirty = [&](uint32_t v) { return (s_dirty[v >> (5u + dshift)] >> ((v >> dshift) & 31u)) & 1u; };
                     auto sext8 = [](unsigned long long v, int j) { return (int)(signed char)(unsigned char)(v >> (8 * j)); };
                     int cntr[NRR][M];                                    // EVAL: counts of rows l8 + 8 rr
                     int srow[NRR], irow[NRR];
@@ -1037,9 +1261,9 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                                     const int lane = tid & 31, bb = (int)(upx & (uint32_t)(LC::A - 1));
                                     for (int e = lane; e < P.Z; e += 32) {
                                         const uint32_t v = u + (uint32_t)s_loff[bb * P.Z + e];
-                                        atomicOr(&s_dirty[v >> 5], 1u << (v & 31u));
+                                        atomicOr(&s_dirty[v >> (5u + dshift)], 1u << ((v >> dshift) & 31u));
                                     }
-                                    if (lane == 0) atomicOr(&s_dirty[u >> 5], 1u << (u & 31u));
+                                    if (lane == 0) atomicOr(&s_dirty[u >> (5u + dshift)], 1u << ((u >> dshift) & 31u));
                                 } else {
                                     mark_one(u, tid & 31);
                                 }
@@ -1135,7 +1359,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 // species code of `site` as step e_at saw it; every lane of the warp takes part
                 auto species_at = [&](uint32_t site, uint32_t e_at) -> uint32_t {
                     uint32_t code = occ_get<OCC>(s_occ, decode_site<LAT>(G, site).pidx);
-                    uint32_t todo = __ballot_sync(0xFFFFFFFFu, ((s_dirty[site >> 5] >> (site & 31u)) & 1u) != 0u);
+                    uint32_t todo = __ballot_sync(0xFFFFFFFFu, ((s_dirty[site >> (5u + dshift)] >> ((site >> dshift) & 31u)) & 1u) != 0u);
                     while (todo) {                                   // flagged lanes, one at a time: 32 lanes x 32 log entries
                         const int src = __ffs((int)todo) - 1;
                         todo &= todo - 1u;
@@ -1182,13 +1406,14 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             }
             __syncthreads();
             if (e_done > 0u) {                                           // new epoch, clean bitmap
-                for (int i = tid; i < ((N + 31) >> 5); i += T) s_dirty[i] = 0u;
+                for (int i = tid; i < dwords; i += T) s_dirty[i] = 0u;
             }
             __syncthreads();
             t0 = t_ep + e_done;
             steps_done = 0u;                                             // t0 already advanced
             key_best = kNoKey;
         } else if (accept_ok && !team && W == 1u) {
+            hist_valid = false; hist_pending = false;
             // ---- accept engine: this one step, 32 candidates per round on the first 8 warps; the other warps settle
             // which candidates of the step are null (all K count, D9.1)
             const double J_cur = sh.J;
@@ -1250,7 +1475,14 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             // A candidate above its threshold cannot improve and is dropped; the survivors are queued and evaluated exactly
             // (stage 2), so every accept decision is the fp64 one.  Needs a bit-symmetric target and w >= 0, w_1 > 0.
             const bool use_filter = SYM && prune && Kc.w[0] > 0.0 && (unsigned long long)Wc * (unsigned)K >= 2ull * GT;
+            // site histograms: the filter of this window reads them when the whole team is here (a leader
+            // running long windows alone must not wait for followers that wait for it)
+            const bool use_hist = use_filter && g_hist != nullptr && (R == 1 || team);
+            bool need_sync = false;
+            if (hist_pending) { hist_update(hist_a, hist_b); hist_pending = false; need_sync = true; }
+            if (use_hist && !hist_valid) { hist_build(); hist_valid = true; }
             if (use_filter && !(slack_J == J_cur)) {
+                need_sync = true;
                 for (int idx = tid; idx < MM; idx += T) {
                     const int p = idx / M, q = idx - p * M;
                     float* row = s_ftab + idx;                           // element e at row[e * MM]
@@ -1297,8 +1529,8 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     row[MM] = Xf;
                 }
                 slack_J = J_cur;
-                __syncthreads();
             }
+            if (need_sync) __syncthreads();
             // the part of an evaluation after the first shell's F: D6 objective shell by shell with the exact pruning
             auto eval_rest = [&](uint32_t key, uint32_t a, uint32_t b, const SiteC& sa, const SiteC& sb, int p, int q,
                                  int mm1, int mm2, const int (&F0)[M]) {
@@ -1357,9 +1589,41 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 }
             };
 
+            // a queued (or overflowing) candidate, evaluated exactly from the configuration
+            auto eval_key = [&](uint32_t key) {
+                uint32_t a, b, hp, hq;
+                SiteC sa, sb;
+                propose(t0 + (key >> 10), key & 1023u, a, b, sa, sb, hp, hq);
+                const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
+                int F0[M];
+                int mm0, mm1, mm2;
+                adjacency(a, b, sa, sb, mm0, mm1, mm2);
+                first_shell(sa, sb, mm0, p, q, F0);
+                eval_rest(key, a, b, sa, sb, p, q, mm1, mm2, F0);
+            };
+
             uint32_t ts = ts_first, k = k_first;
             uint32_t ncur = 0u;                                     // null bits of the current group of 32 candidates
             int j = 0;
+            if (use_hist) {
+                // ---- stage 1 from the site-histogram table: hist_scan (its own register allocation) runs this thread's
+                // candidates; what it cannot settle itself (queue overflow) comes back to be evaluated here
+                HistScan hs;
+                hs.ts = ts_first; hs.k = k_first; hs.ncur = 0u; hs.j = 0; hs.n_ovf = 0; hs.done = 0;
+#pragma unroll
+                for (int wd = 0; wd < kNullWords; ++wd) hs.nullw[wd] = 0u;
+                HistArgs ha;
+                ha.H = g_hist; ha.rk = AA.rk; ha.best_slot = smem_addr(&sh.best[buf]); ha.ftab = smem_addr(s_ftab); ha.queue = smem_addr(sh.queue); ha.q_n = smem_addr(&sh.q_n[buf]);
+                ha.t0 = t0; ha.Wc = Wc; ha.ts_inc = ts_inc; ha.k_inc = k_inc; ha.K = (uint32_t)K; ha.N = (uint32_t)N; ha.chain = chain;
+                ha.Lx = Lx; ha.Ly = Ly; ha.Lz = Lz; ha.mx = G.mx; ha.sx = G.sx; ha.mq = G.mq; ha.sq = G.sq; ha.basis = G.basis; ha.d2_0 = G.d2[0];
+                do {
+                    hist_scan<M, LAT, BEST>(hs, ha);
+                    for (int i = 0; i < hs.n_ovf; ++i) eval_key(hs.ovf[i]);
+                } while (!hs.done);
+                j = hs.j; ncur = hs.ncur;
+#pragma unroll
+                for (int wd = 0; wd < kNullWords; ++wd) nullw[wd] = hs.nullw[wd];
+            } else
             for (; ts < Wc; ++j) {
                 const uint32_t hint = *best_slot;
                 if ((hint >> 10) < ts) break;                       // a move at an earlier step exists: this step is void
@@ -1412,15 +1676,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     const uint32_t key = sh.queue[i];
                     const uint32_t hint = *best_slot;
                     if (best_mode ? (hint >> 10) < (key >> 10) : !(key < hint)) continue;
-                    uint32_t a, b, hp, hq;
-                    SiteC sa, sb;
-                    propose(t0 + (key >> 10), key & 1023u, a, b, sa, sb, hp, hq);
-                    const int p = 31 - __clz((int)hp), q = 31 - __clz((int)hq);
-                    int F0[M];
-                    int mm0, mm1, mm2;
-                    adjacency(a, b, sa, sb, mm0, mm1, mm2);
-                    first_shell(sa, sb, mm0, p, q, F0);
-                    eval_rest(key, a, b, sa, sb, p, q, mm1, mm2, F0);
+                    eval_key(key);
                 }
             }
             __syncthreads();                                        // B1: window evaluated, local minimum posted
@@ -1506,6 +1762,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             }
             if (key_best != kNoKey) {
                 apply_move(mv, key_best & 1023u, t0 + (key_best >> 10));
+                if (hist_valid) { hist_pending = true; hist_a = mv->a; hist_b = mv->b; }
                 W = min(steps_done, w_cap);                         // the observed gap (a quarter of the gap between moves
                                                                     // was tried: no gain on c4, 3-6 % slower on the chain sweep)
                 depth = 0;
@@ -1524,6 +1781,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             if (team) {
                 if (key_best != kNoKey && (unsigned long long)steps_done * (unsigned)K < (unsigned long long)AA.team_off) {
                     set_mode(false);                            // followers go and wait at the top of the loop
+                    hist_valid = false; hist_pending = false;
                     W = min(W, w_cap);
                 }
             } else if ((unsigned long long)W * (unsigned)K >= (unsigned long long)AA.team_on) {
@@ -1653,7 +1911,7 @@ size_t mc2_team_bytes(int64_t C) { return sizeof(TeamCtl) * (size_t)C; }
 cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice, int occ_mode, int threads, int team,
                        void* team_ctl, int team_on, int team_off, int accept_engine, size_t smem_budget, int w_max, uint8_t* occ, int32_t* counts, int64_t C, uint64_t n_steps, int K, uint64_t seed, uint64_t chain0,
                        uint64_t step0, void* stats, void* log, int64_t log_cap, int select_best, uint64_t depth_limit,
-                       uint64_t* depth, uint64_t* steps_done, cudaStream_t st, int64_t* n_launches)
+                       uint64_t* depth, uint64_t* steps_done, uint32_t* hist, cudaStream_t st, int64_t* n_launches)
 {
     Mc2Args AA;
     McArgs& A = AA.a;
@@ -1666,6 +1924,7 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
     AA.team_on = team_on > 0 ? team_on : 4 * threads;
     AA.team_off = team_off > 0 ? team_off : threads;
     AA.accept_engine = accept_engine;
+    AA.hist = hist;
     AA.select_best = select_best ? 1 : 0;
     AA.depth_limit = depth_limit;
     AA.depth_all = reinterpret_cast<unsigned long long*>(depth);
@@ -1751,8 +2010,22 @@ cudaError_t launch_mc2(const KParams& P, const DevTables& host_tab, int lattice,
     G.distinct = P.L[0] >= 3 && P.L[1] >= 3 && P.L[2] >= 3;
     size_t smem = mc2_shared_bytes(occ_mode, lattice, P.L, P.M);
     // the pipelined accept engine needs its record, bitmap and offset buffers on top; without room it is simply off
-    const size_t pae_bytes = sizeof(PRec) * (size_t)kPaeRecs + 4u * (size_t)((P.N + 31) >> 5) + 4u * (size_t)P.A * (size_t)P.Z + 16u +
-                             8u * 2u * (size_t)kPaeK * (size_t)P.S * (size_t)P.M + 8u + sizeof(uint2) * (size_t)kPaeRecs;
+    auto pae_bytes_of = [&](int ds) {
+        const size_t dwords = ((((size_t)P.N + ((size_t)1 << ds) - 1) >> ds) + 31) >> 5;
+        return sizeof(PRec) * (size_t)kPaeRecs + 4u * dwords + 4u * (size_t)P.A * (size_t)P.Z + 16u +
+               8u * 2u * (size_t)kPaeK * (size_t)P.S * (size_t)P.M + 8u + sizeof(uint2) * (size_t)kPaeRecs;
+    };
+    // The site-histogram filter is bound by the random L2 loads an SM can keep in flight, and those need L1 lines: with the
+    // 228 KB shared-memory carve-out (28 KB of L1) an SM sustains ~0.5 random sectors per clock, with 196 KB ~0.9.  When the
+    // table is in use, the touched-site bitmap of the accept engine is made coarser (conservative) if that brings the block
+    // under the 196 KB carve-out (1 KB of it is reserved by the system).
+    AA.dshift = 0;
+    if (hist != nullptr && accept_engine == 2 && threads >= 512) {
+        const size_t target = 196u * 1024u - 1024u;
+        for (int ds = 0; ds <= 4; ++ds)
+            if (smem + pae_bytes_of(ds) <= target) { AA.dshift = ds; break; }
+    }
+    const size_t pae_bytes = pae_bytes_of(AA.dshift);
     AA.pae = (accept_engine == 2 && threads >= 512 && smem + pae_bytes <= smem_budget) ? 1 : 0;
     if (AA.pae) smem += pae_bytes;
     const int part = (lattice != 0 ? 1 : 0) + (select_best ? 2 : 0);
