@@ -350,6 +350,7 @@ struct Mc2Args {
 };
 
 // ---- stage 1 of a long window from the site-histogram table
+constexpr int kHistBatch = 4;     // candidates a thread keeps in flight
 struct HistArgs {                 // the same in every thread of the block
     const uint32_t* H;            // the chain's table: species << 24 | first-shell neighbour counts of species 0..M-2
     const uint32_t* rk;           // Philox round keys (Mc2Args::rk)
@@ -362,6 +363,8 @@ struct HistArgs {                 // the same in every thread of the block
     uint32_t Wc, ts_inc, k_inc, K, N, chain;
     int Lx, Ly, Lz;
     uint32_t mx, sx, mq, sq;      // site / (A Ly Lz), site / (A Lz) by multiply-high (Geo)
+    uint32_t cx, cc;              // padded index = site + 2 A q + cx x + cc (Geo)
+    uint32_t occ;                 // shared-space address of the padded one-hot configuration
     uint32_t basis;
     int d2_0;                     // squared first-shell distance, doubled units
 };
@@ -371,7 +374,7 @@ struct HistScan {                 // one thread's scan of its candidates of the 
     uint32_t ncur;                // null bits of the current group of 32 candidates
     int j;                        // candidates scanned
     uint32_t nullw[kNullWords];
-    uint32_t ovf[4];              // survivors that found the queue full: the caller evaluates them
+    uint32_t ovf[kTeamRounds];    // survivors that found the queue full: the caller evaluates them
     int n_ovf;
     int done;
 };
@@ -381,6 +384,12 @@ __device__ __forceinline__ uint32_t lds_volatile_u32(uint32_t a)
 {
     uint32_t v;
     asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u8(uint32_t a)
+{
+    uint32_t v;
+    asm("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a));
     return v;
 }
 __device__ __forceinline__ float lds_f32(uint32_t a)
@@ -397,14 +406,16 @@ __device__ __forceinline__ uint32_t atoms_inc(uint32_t a)
 }
 __device__ __forceinline__ void sts_u32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 
-// Scans this thread's candidates in batches of four: Philox, the two table words (two more after a redraw, D9.1), null bit,
+// Scans this thread's candidates in batches of four: Philox, the species of the drawn sites from the configuration in shared
+// memory (which settles redraw and nullness, D9.1), the two table words of a live candidate (its only L2 round trip),
 // first-shell adjacency (D9.2), F = difference of the neighbour counts, the fp32 form of the reject filter; survivors go
-// to the queue.  Not inlined on purpose: inside the kernel body the loop would share 128 registers with everything else
+// to the queue.  What bounds it is the rate at which an SM takes random 32-byte sectors from L2 (~0.75 per clock with the
+// 196 KB carve-out, measured), hence as few loads per candidate as possible.  Not inlined on purpose: inside the kernel body the loop would share 128 registers with everything else
 // that is live there, and the allocator then reuses load destinations, which serialises the L2 round trips.
-template <int M, int LAT, bool BEST>
+template <int M, int LAT, bool BEST, int OCC>
 __device__ __noinline__ void hist_scan(HistScan& st, const HistArgs& A)
 {
-    constexpr int U = 4;
+    constexpr int U = kHistBatch;
     static_assert(32 % U == 0, "null words are closed on batch boundaries");
     constexpr int MM = M * M;
     constexpr int HFB = M <= 4 ? 8 : 6;
@@ -420,52 +431,61 @@ __device__ __noinline__ void hist_scan(HistScan& st, const HistArgs& A)
     const unsigned long long t0 = A.t0;
     const int Lx = A.Lx, Ly = A.Ly, Lz = A.Lz;
     const uint32_t Lxy = (uint32_t)(Lx * Ly);
-    uint32_t ts = st.ts, k = st.k, ncur = st.ncur;
-    int j = st.j;
-    int n_ovf = 0;
-    bool done = true;
+    const uint32_t mx = A.mx, sx = A.sx, mq = A.mq, sq = A.sq, gcx = A.cx, gcc = A.cc, occ_s = A.occ;
+    // one-hot species code of the site with cell-row index q = x Ly + y and x, from the padded configuration in shared memory
+    auto code_at = [&](uint32_t site, uint32_t q, uint32_t x) -> uint32_t {
+        const uint32_t pidx = site + (uint32_t)(2 * LC::A) * q + gcx * x + gcc;
+        if (OCC == OCC2_NIB) return (lds_u8(occ_s + (pidx >> 1)) >> ((pidx & 1u) * 4u)) & 0xFu;
+        return lds_u8(occ_s + pidx);
+    };
+    uint32_t ts = st.ts, k = st.k, ncur = 0u;
+    int j = 0, n_ovf = 0;
     while (ts < Wc) {
         const uint32_t hint = lds_volatile_u32(A.best_slot);
         if ((hint >> 10) < ts) break;                               // a move at an earlier step exists
-        if (n_ovf != 0) { done = false; break; }                    // hand the overflow to the caller first
-        uint32_t key[U], a[U], b[U], ha[U], hb[U], rx[U], rz[U], rw[U];
+        uint32_t key[U], a[U], b[U], ha[U], hb[U], qa[U], qb[U];
+        int cx[U];
+        bool live[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             key[u] = ts < Wc ? ((ts << 10) | k) : kNoKey;
             const unsigned long long step = t0 + ts;
             const uint4 r = philox4x32_10_rk((uint32_t)step, (uint32_t)(step >> 32), k, chain, rk);
-            a[u] = __umulhi(r.x, N); b[u] = __umulhi(r.y, N - 1u);
-            b[u] += (b[u] >= a[u]);
-            rx[u] = r.x; rz[u] = r.z; rw[u] = r.w;
-            ha[u] = __ldcg(H + a[u]); hb[u] = __ldcg(H + b[u]);
+            // D9.1.  The cell coordinates of a come straight from its random word: floor(floor(r N / 2^32) / d) =
+            // floor(r (N / d) / 2^32); those of b by the exact multiply-high divisions of Geo.
+            uint32_t sa = __umulhi(r.x, N), sb = __umulhi(r.y, N - 1u);
+            sb += (sb >= sa);
+            uint32_t xa = __umulhi(r.x, (uint32_t)Lx), ya = __umulhi(r.x, Lxy);
+            uint32_t xb = __umulhi(sb, mx) >> sx, yb = __umulhi(sb, mq) >> sq;
+            uint32_t ca = code_at(sa, ya, xa), cb = code_at(sb, yb, xb);
+            if (ca == cb) {                                         // like species: redraw once
+                sa = __umulhi(r.z, N); sb = __umulhi(r.w, N - 1u);
+                sb += (sb >= sa);
+                xa = __umulhi(r.z, (uint32_t)Lx); ya = __umulhi(r.z, Lxy);
+                xb = __umulhi(sb, mx) >> sx; yb = __umulhi(sb, mq) >> sq;
+                ca = code_at(sa, ya, xa); cb = code_at(sb, yb, xb);
+            }
+            live[u] = ca != cb;
+            a[u] = sa; b[u] = sb; qa[u] = ya; qb[u] = yb; cx[u] = (int)xb - (int)xa;
+            ha[u] = 0u; hb[u] = 0u;
+            if (live[u]) { ha[u] = __ldcg(H + sa); hb[u] = __ldcg(H + sb); }     // the only L2 round trip of a candidate
             k += k_inc; ts += ts_inc;
             if (k >= K) { k -= K; ++ts; }
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            if (((ha[u] ^ hb[u]) >> 24) == 0u) {                    // like species: redraw once (D9.1)
-                rx[u] = rz[u];
-                a[u] = __umulhi(rz[u], N); b[u] = __umulhi(rw[u], N - 1u);
-                b[u] += (b[u] >= a[u]);
-                ha[u] = __ldcg(H + a[u]); hb[u] = __ldcg(H + b[u]);
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int p = (int)(ha[u] >> 24), q = (int)(hb[u] >> 24);
-            ncur = __funnelshift_r(ncur, p == q ? 1u : 0u, 1);
-            if (p != q && key[u] != kNoKey && (BEST || key[u] < hint)) {
-                // D9.2: are a and b first-shell neighbours?  The cell coordinates of a come straight from its random word
-                // (floor(floor(r N / 2^32) / d) = floor(r (N / d) / 2^32)); almost every pair fails on x or y
-                const uint32_t xa = __umulhi(rx[u], (uint32_t)Lx), qa = __umulhi(rx[u], Lxy);
-                const uint32_t xb = __umulhi(b[u], A.mx) >> A.sx, qb = __umulhi(b[u], A.mq) >> A.sq;
-                const int cx = (int)xb - (int)xa, cy = (int)(qb - qa) - cx * Ly;
-                const int ax = abs(cx), ay = abs(cy);
+            ncur = __funnelshift_r(ncur, live[u] ? 0u : 1u, 1);
+            if (live[u] && key[u] != kNoKey && (BEST || key[u] < hint)) {
+                const int p = (int)(ha[u] >> 24), q = (int)(hb[u] >> 24);
+                // D9.2: are a and b first-shell neighbours?  Almost every pair fails on x or y.
+                const int cy = (int)(qb[u] - qa[u]) - cx[u] * Ly;
+                const int ax = abs(cx[u]), ay = abs(cy);
                 int mm0 = 0;
                 if ((ax <= 1 || ax == Lx - 1) && (ay <= 1 || ay == Ly - 1)) {
-                    const int za = (int)((a[u] >> LC::lgA) - qa * (uint32_t)Lz), zb = (int)((b[u] >> LC::lgA) - qb * (uint32_t)Lz);
-                    const int ba = (int)(a[u] & (uint32_t)(LC::A - 1)), bb = (int)(b[u] & (uint32_t)(LC::A - 1));
-                    const int dx = 2 * cx + (int)((A.basis >> (3 * bb)) & 1u) - (int)((A.basis >> (3 * ba)) & 1u);
+                    const uint32_t sa = a[u], sb = b[u];
+                    const int za = (int)((sa >> LC::lgA) - qa[u] * (uint32_t)Lz), zb = (int)((sb >> LC::lgA) - qb[u] * (uint32_t)Lz);
+                    const int ba = (int)(sa & (uint32_t)(LC::A - 1)), bb = (int)(sb & (uint32_t)(LC::A - 1));
+                    const int dx = 2 * cx[u] + (int)((A.basis >> (3 * bb)) & 1u) - (int)((A.basis >> (3 * ba)) & 1u);
                     const int dy = 2 * cy + (int)((A.basis >> (3 * bb + 1)) & 1u) - (int)((A.basis >> (3 * ba + 1)) & 1u);
                     const int dz = 2 * (zb - za) + (int)((A.basis >> (3 * bb + 2)) & 1u) - (int)((A.basis >> (3 * ba + 2)) & 1u);
                     const int wx = dx > Lx ? dx - 2 * Lx : dx < -Lx ? dx + 2 * Lx : dx;
@@ -498,14 +518,14 @@ __device__ __noinline__ void hist_scan(HistScan& st, const HistArgs& A)
                 if (!(acc > lds_f32(row))) {
                     const uint32_t slot = atoms_inc(A.q_n);
                     if (slot < (uint32_t)kQueueCap) sts_u32(A.queue + 4u * slot, key[u]);
-                    else st.ovf[n_ovf++] = key[u];
+                    else st.ovf[n_ovf++] = key[u];                 // at most kTeamRounds candidates per thread and window
                 }
             }
         }
         j += U;
         if ((j & 31) == 0) st.nullw[(j >> 5) - 1] = ncur;
     }
-    st.ts = ts; st.k = k; st.ncur = ncur; st.j = j; st.n_ovf = n_ovf; st.done = done ? 1 : 0;
+    st.ts = ts; st.k = k; st.ncur = ncur; st.j = j; st.n_ovf = n_ovf; st.done = 1;
 }
 
 // Shared memory: occupancy (offset 0, so a gather address is the loaded offset itself) | Sh2 | offset table [A][ZP].
@@ -1615,9 +1635,9 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 HistArgs ha;
                 ha.H = g_hist; ha.rk = AA.rk; ha.best_slot = smem_addr(&sh.best[buf]); ha.ftab = smem_addr(s_ftab); ha.queue = smem_addr(sh.queue); ha.q_n = smem_addr(&sh.q_n[buf]);
                 ha.t0 = t0; ha.Wc = Wc; ha.ts_inc = ts_inc; ha.k_inc = k_inc; ha.K = (uint32_t)K; ha.N = (uint32_t)N; ha.chain = chain;
-                ha.Lx = Lx; ha.Ly = Ly; ha.Lz = Lz; ha.mx = G.mx; ha.sx = G.sx; ha.mq = G.mq; ha.sq = G.sq; ha.basis = G.basis; ha.d2_0 = G.d2[0];
+                ha.Lx = Lx; ha.Ly = Ly; ha.Lz = Lz; ha.mx = G.mx; ha.sx = G.sx; ha.mq = G.mq; ha.sq = G.sq; ha.cx = G.cx; ha.cc = G.cc; ha.occ = smem_addr(s_occ); ha.basis = G.basis; ha.d2_0 = G.d2[0];
                 do {
-                    hist_scan<M, LAT, BEST>(hs, ha);
+                    hist_scan<M, LAT, BEST, OCC>(hs, ha);
                     for (int i = 0; i < hs.n_ovf; ++i) eval_key(hs.ovf[i]);
                 } while (!hs.done);
                 j = hs.j; ncur = hs.ncur;
