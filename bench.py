@@ -281,6 +281,9 @@ def run_configs(args):
     for ci in (1, 2, 3, 4, 0):
         w = workloads.config(ci) if ci else workloads.large_m_workload()     # 0: the cell only the window engine holds
         h = binding.Hea(*w.create_args(), device=0)
+        for kv in args.opt:
+            name, val = kv.split("=")
+            h.set_option(name, int(val))
         best = None
         for rep in range(3):
             occ = h.init_random(w.n_chains, w.seed)

@@ -485,11 +485,12 @@ int hea_mc_run_ex(hea_ctx* ctx, uint8_t* occ_dev, int32_t* counts_dev, int64_t C
             if (rc != HEA_OK) return rc;
             team_ctl = ctx->scratch[5];
         }
-        // site-histogram table of the reject filter: 4 bytes per site and chain, kept in L2.  Default: for
-        // teams (few chains, large cells); mc_hist = 2 also for one block per chain, mc_hist = 1 never.
+        // site-histogram table of the reject filter: 4 bytes per site and chain, read through L2.  Default: on
+        // while the tables of all chains stay well inside L2 (64 MB); mc_hist = 2 always, mc_hist = 1 never.
         uint32_t* hist = nullptr;
-        if (ctx->M >= 2 && ctx->M <= 5 && ctx->opt_hist != 1 && (team > 1 || ctx->opt_hist == 2)) {
-            int rc = ensure_scratch(ctx, 6, sizeof(uint32_t) * (size_t)N * (size_t)C);
+        const size_t hist_bytes = sizeof(uint32_t) * (size_t)N * (size_t)C;
+        if (ctx->M >= 2 && ctx->M <= 5 && ctx->opt_hist != 1 && (hist_bytes <= ((size_t)64 << 20) || ctx->opt_hist == 2)) {
+            int rc = ensure_scratch(ctx, 6, hist_bytes);
             if (rc != HEA_OK) return rc;
             hist = (uint32_t*)ctx->scratch[6];
         }

@@ -315,6 +315,38 @@ def test_reject_filter_at_the_accept_threshold(hb, shift, gamma, lattice, dims, 
         np.testing.assert_array_equal(got[0][:n][f], o_log[0][:n][f])
 
 
+# ---- the site-histogram table of the reject filter: on (2), off (1), SOLO and TEAM windows, both layouts
+HIST_CASES = [("fcc", (6, 6, 6), (0.25,) * 4, 2, 7, (-0.1, 0.1), 32, 2500, 200),
+              ("bcc", (7, 7, 7), (0.2,) * 5, 2, 3, (-0.1, 0.1), 16, 2500, 200),
+              ("fcc", (5, 6, 7), (0.5, 0.3, 0.2), 3, 5, (-0.05, 0.05), 64, 1500, 200),
+              ("bcc", (9, 8, 7), (0.5, 0.5), 3, 9, (-0.2, 0.2), 8, 3000, 200),
+              # a target out of reach: J stays large, most candidates pass the filter and the queue overflows
+              ("fcc", (4, 4, 4), (0.25,) * 4, 3, 11, (-0.6, 0.6), 128, 3000, 0)]
+
+
+@pytest.mark.parametrize("lattice,dims,conc,S,tseed,rng,K,n_steps,tail", HIST_CASES)
+@pytest.mark.parametrize("shape", [{"mc_team": 1, "mc_threads": 64}, {"mc_team": 1, "mc_threads": 512},
+                                   {"mc_team": 4, "mc_threads": 128}, {"mc_team": 9, "mc_threads": 512},
+                                   {"mc_team": 3, "mc_threads": 512, "mc_occ_mode": 2}])
+@pytest.mark.parametrize("hist", [1, 2])
+def test_site_histogram_filter_on_and_off(hb, lattice, dims, conc, S, tseed, rng, K, n_steps, tail, shape, hist):
+    if shape.get("mc_occ_mode") == 2 and len(conc) > 4:
+        pytest.skip("nibble layout holds at most 4 species")
+    w = small(lattice, dims, conc, S, target_seed=tseed, rng=rng, K=K)
+    st = run_both(hb, w, 3, n_steps, log_cap=32, opts={"mc_engine": 2, "mc_hist": hist, **shape})
+    assert int(st["n_accept"].min()) > 20
+    assert int((n_steps - 1 - st["last_accept_step"]).max()) >= tail    # long windows were reached
+
+
+@pytest.mark.parametrize("hist", [1, 2])
+@pytest.mark.parametrize("shape", [{"mc_team": 1, "mc_threads": 256}, {"mc_team": 5, "mc_threads": 512}])
+def test_site_histogram_filter_best_of_K_and_split_runs(hb, shape, hist):
+    w = small("fcc", (6, 6, 6), (0.25,) * 4, 2, target_seed=7, K=32)
+    run_both_ex(hb, w, 3, 2500, 1, 0, opts={"mc_engine": 2, "mc_hist": hist, **shape})
+    run_both_ex(hb, w, 3, 2500, 1, 300, opts={"mc_engine": 2, "mc_hist": hist, **shape}, split=1700)
+    run_both_ex(hb, w, 3, 2500, 0, 500, opts={"mc_engine": 2, "mc_hist": hist, **shape})
+
+
 # ---- the product's own chain sharding: two (chain0, count) shards on one device == one call
 @pytest.mark.parametrize("world", [2, 3])
 def test_product_sharding_union_equals_single_call(hb, world):
