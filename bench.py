@@ -37,11 +37,13 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-MC_REJECT_WARP_INSTR = 26_472_988_180 / 6.4e7     # per 32 trials: smsp__inst_executed.sum of the 1e6-step reject launch
-MC_REJECT_WAVEFRONTS = 7_457_908_721 / 6.4e7       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum of the same launch
-MC_FULL_WARP_INSTR = 265_620_284_000.0             # whole c4 launch (16 chains x 1e7 steps)
+MC_REJECT_WARP_INSTR = 15_102_426_293 / 6.4e7     # per 32 trials: smsp__inst_executed.sum of the 1e6-step reject launch
+MC_REJECT_WAVEFRONTS = 1_707_546_932 / 6.4e7       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum of the same launch
+MC_REJECT_L2_SECTORS = 3_860_524_676 / 6.4e7       # l1tex__t_sectors_pipe_lsu_mem_global_op_ld.sum (site-histogram table words, via L2)
+MC_FULL_WARP_INSTR = 152_684_466_856.0             # whole c4 launch (16 chains x 1e7 steps)
 DTYPE = ("int32 counts + f64 objective (D6 order, no FMA); long windows pass a conservative fp32 reject filter on shell 1 "
-         "first (rigorous error bound in its threshold, survivors evaluated in f64: accept decisions are the f64 ones)")
+         "first (rigorous error bound in its threshold, survivors evaluated in f64: accept decisions are the f64 ones); its "
+         "inputs are per-site integer neighbour counts kept in a table")
 METRIC = "delta-SRO swap trials/sec (c4: fcc 40^3, 256,000 atoms, 16 chains x 1e7 steps, K=128) incl. the full-SRO recount of the start"
 UNIT = "swap-trials/s"
 
@@ -58,12 +60,13 @@ def load_peaks():
 # never runs under a profiler); every use below names its source file in the JSON line.
 NCU = {
     # whole c4 trajectory, one launch: dram__bytes_read.sum + dram__bytes_write.sum
-    "mc_c4_full_dram_bytes": (7_293_696 + 18_432, "profiles/r2_mc_halo_c4_full.md"),
+    "mc_c4_full_dram_bytes": (8_034_048 + 91_675_136, "profiles/r2_mc_halo_c4_full.md"),
     "mc_c4_full_warp_instr": (MC_FULL_WARP_INSTR, "profiles/r2_mc_halo_c4_full.md"),
     # reject regime of c4 (1e6 steps after the trajectory): executed warp-instructions and shared-memory data-pipe
     # wavefronts per 32 trials (smsp__inst_executed.sum, l1tex__data_pipe_lsu_wavefronts_mem_shared.sum over 6.4e7 warp-trials)
     "mc_reject_warp_instr_per_32_trials": (MC_REJECT_WARP_INSTR, "profiles/r2_mc_halo_reject.md"),
     "mc_reject_smem_wavefronts_per_32_trials": (MC_REJECT_WAVEFRONTS, "profiles/r2_mc_halo_reject.md"),
+    "mc_reject_l2_sectors_per_32_trials": (MC_REJECT_L2_SECTORS, "profiles/r2_mc_halo_reject.md"),
     "recount_table_L100_dram_bytes": (680_581_888 + 4_061_184, "profiles/r2_recount.md"),
     "recount_stencil_L100_dram_bytes": (4_028_928, "profiles/r2_recount.md"),
     # table-free recount on fcc 100^3, batch 1: smsp__inst_executed.sum of one launch
@@ -530,13 +533,14 @@ def main():
     alu_peak = n_sms * 128 * sm_max_mhz * 1e6 / 1e12                    # nominal: 4 SMSPs x 32 lanes / clk
     mc_rate_1gpu = C * n_mc * K * args.steps / t_mc
     # ---- roofline of the dominant kernel (mc_halo_kernel).  The kernel moves no HBM bytes in steady state; what binds it is
-    # instruction issue and the shared-memory data pipe.  Denominators: this box's own micro-benchmarks (hea_measure_peaks).
+    # instruction issue, the shared-memory data pipe and (long windows) the random L2 sectors of the site-histogram table.  Denominators: this box's own micro-benchmarks (hea_measure_peaks).
     # achieved = warp-instructions the kernel EXECUTES per launch (ncu, committed profile) x 32 / measured launch duration.
     peaks = h.measure_peaks()
     is_metric_run = args.workload == 4 and not args.chains and n_mc == w.n_steps
     full_instr, full_src = NCU["mc_c4_full_warp_instr"]
     rej_instr, rej_src = NCU["mc_reject_warp_instr_per_32_trials"]
     rej_wf, _ = NCU["mc_reject_smem_wavefronts_per_32_trials"]
+    rej_l2, _ = NCU["mc_reject_l2_sectors_per_32_trials"]
     issue_peak_T = peaks["issue_instr_per_s"] / 1e12
     t_launch = t_mc / args.steps
     achieved_T = full_instr * 32 / t_launch / 1e12 if is_metric_run else None
@@ -546,7 +550,13 @@ def main():
                   "frac": rej_rate * rej_instr / 1e12 / issue_peak_T},
         "smem_pipe": {"achieved": rej_rate / 32 * rej_wf / 1e12, "peak": peaks["lds_wavefronts_per_s"] / 1e12,
                       "unit": "T wavefronts/s", "frac": rej_rate / 32 * rej_wf / peaks["lds_wavefronts_per_s"]},
-        "per_32_trials": {"warp_instr": rej_instr, "smem_wavefronts": rej_wf, "source": rej_src},
+        # random 32-byte sectors of the site-histogram table against the measured random-sector rate
+        "l2_sectors": {"achieved": rej_rate / 32 * rej_l2 / 1e12, "peak": peaks["l2_random_sector_GBps"] * 1e9 / 32 / 1e12,
+                       "unit": "T sectors/s", "frac": rej_rate / 32 * rej_l2 / (peaks["l2_random_sector_GBps"] * 1e9 / 32)},
+        "per_32_trials": {"warp_instr": rej_instr, "smem_wavefronts": rej_wf, "l2_sectors": rej_l2, "source": rej_src},
+        # what the measured denominators allow for this formulation: the lowest of the three per-resource limits
+        "trials_per_s_bound": min(peaks["issue_instr_per_s"] / rej_instr, peaks["lds_wavefronts_per_s"] * 32 / rej_wf,
+                                  peaks["l2_random_sector_GBps"] * 1e9 / 32 * 32 / rej_l2),
         "trials_per_s": rej_rate}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

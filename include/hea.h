@@ -117,6 +117,10 @@ int hea_neighbor_table(const hea_ctx* ctx, int shell, int32_t* out_host);
  *                     a team starts / stops sharing a window, 0 = auto
  *   "mc_accept"       halo engine, single-step windows: 0 = auto (3), 1 = thread per candidate, 2 = eight lanes per
  *                     candidate, 3 = the warp-specialised serial engine over epochs of records computed ahead
+ *   "mc_hist"         halo engine, long windows: the reject filter reads a per-site table (species and first-shell
+ *                     neighbour counts, 4 bytes per site and chain, library-owned, kept in L2) instead of gathering the
+ *                     neighbours; 0 = auto (on for 2..5 species on cells of at least 3 cells per side while the tables of
+ *                     all chains take at most 64 MB), 1 = off, 2 = on whatever the size
  *   "sro_engine"      recount: 0 = auto (the table-free stencil kernel when occ_dev is aligned to the basis size,
  *                     else the table-driven kernel), 1 = table-driven (HBM-bound, 4 Z + 1 bytes per atom),
  *                     2 = stencil (1 byte per atom; HEA_EINVAL when occ_dev is not aligned)
