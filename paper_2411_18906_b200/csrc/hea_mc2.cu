@@ -554,6 +554,18 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     const uint32_t dshift = (uint32_t)AA.dshift;
     const int dwords = (int)(((((uint32_t)P.N + (1u << dshift) - 1u) >> dshift) + 31u) >> 5);
     int* s_loff = reinterpret_cast<int*>(s_dirty + dwords);
+    // second, hashed view of the same touched set: bit (site mod 32 kQueueCap), in the words of the survivor queue (which is
+    // idle while the serial accept engine runs).  A site counts as touched only when BOTH bitmaps say so: the coarse one
+    // flags whole groups of 2^dshift neighbouring sites, this one separates them again (conservative: no false negative).
+    uint32_t* const s_dirty2 = sh.queue;
+    bool mark2 = false;                                      // inside a serial-engine epoch (block-uniform)
+    auto mark_bits = [&](uint32_t v) {
+        atomicOr(&s_dirty[v >> (5u + dshift)], 1u << ((v >> dshift) & 31u));
+        if (mark2) atomicOr(&s_dirty2[(v >> 5) & (uint32_t)(kQueueCap - 1)], 1u << (v & 31u));
+    };
+    auto touched = [&](uint32_t v) -> uint32_t {
+        return (s_dirty[v >> (5u + dshift)] >> ((v >> dshift) & 31u)) & (s_dirty2[(v >> 5) & (uint32_t)(kQueueCap - 1)] >> (v & 31u)) & 1u;
+    };
     // serial accept engine: packed count changes per objective row of the improving records, [step parity][record][S*M]
     unsigned long long* s_dn = reinterpret_cast<unsigned long long*>(
         (reinterpret_cast<uintptr_t>(s_loff + LC::A * P.Z) + 7u) & ~(uintptr_t)7u);
@@ -720,9 +732,9 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         const bool interior = sc.x >= 1 && sc.x <= Lx - 2 && sc.y >= 1 && sc.y <= Ly - 2 && sc.z >= 1 && sc.z <= Lz - 2;
         for (int e = lane; e < P.Z; e += 32) {
             const uint32_t v = interior ? u + (uint32_t)s_loff[sc.b * P.Z + e] : (uint32_t)__ldg(P.nbr_site + (size_t)u * P.Z + e);
-            atomicOr(&s_dirty[v >> (5u + dshift)], 1u << ((v >> dshift) & 31u));
+            mark_bits(v);
         }
-        if (lane == 0) atomicOr(&s_dirty[u >> (5u + dshift)], 1u << ((u >> dshift) & 31u));
+        if (lane == 0) mark_bits(u);
     };
     auto mark_touched = [&](uint32_t ma, uint32_t mb, int lane) {
         mark_one(ma, lane);
@@ -1119,6 +1131,8 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 s_px[tid] = px;
             }
             if (tid < kPaeRecs / kPaeK) sh.mlog[tid] = make_uint4(0u, 0u, 0u, 0u);
+            for (int i = tid; i < kQueueCap; i += T) s_dirty2[i] = 0u;   // the queue's words: dead between windows
+            mark2 = true;
             __syncthreads();
             uint32_t e_done = 0;                                         // steps of the epoch consumed
             bool leave = false;
@@ -1134,7 +1148,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                     const bool is_eval = tid < 128;
                     const int grp = (tid >> 3) & 15, l8 = tid & 7;
                     const int SMr = S * M;
-                    auto dirty = [&](uint32_t v) { return (s_dirty[v >> (5u + dshift)] >> ((v >> dshift) & 31u)) & 1u; };
+                    auto dirty = [&](uint32_t v) { return touched(v); };
                     auto sext8 = [](unsigned long long v, int j) { return (int)(signed char)(unsigned char)(v >> (8 * j)); };
                     int cntr[NRR][M];                                    // EVAL: counts of rows l8 + 8 rr
                     int srow[NRR], irow[NRR];
@@ -1281,9 +1295,9 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                                     const int lane = tid & 31, bb = (int)(upx & (uint32_t)(LC::A - 1));
                                     for (int e = lane; e < P.Z; e += 32) {
                                         const uint32_t v = u + (uint32_t)s_loff[bb * P.Z + e];
-                                        atomicOr(&s_dirty[v >> (5u + dshift)], 1u << ((v >> dshift) & 31u));
+                                        mark_bits(v);
                                     }
-                                    if (lane == 0) atomicOr(&s_dirty[u >> (5u + dshift)], 1u << ((u >> dshift) & 31u));
+                                    if (lane == 0) mark_bits(u);
                                 } else {
                                     mark_one(u, tid & 31);
                                 }
@@ -1379,7 +1393,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 // species code of `site` as step e_at saw it; every lane of the warp takes part
                 auto species_at = [&](uint32_t site, uint32_t e_at) -> uint32_t {
                     uint32_t code = occ_get<OCC>(s_occ, decode_site<LAT>(G, site).pidx);
-                    uint32_t todo = __ballot_sync(0xFFFFFFFFu, ((s_dirty[site >> (5u + dshift)] >> ((site >> dshift) & 31u)) & 1u) != 0u);
+                    uint32_t todo = __ballot_sync(0xFFFFFFFFu, touched(site) != 0u);
                     while (todo) {                                   // flagged lanes, one at a time: 32 lanes x 32 log entries
                         const int src = __ffs((int)todo) - 1;
                         todo &= todo - 1u;
@@ -1428,6 +1442,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
             if (e_done > 0u) {                                           // new epoch, clean bitmap
                 for (int i = tid; i < dwords; i += T) s_dirty[i] = 0u;
             }
+            mark2 = false;
             __syncthreads();
             t0 = t_ep + e_done;
             steps_done = 0u;                                             // t0 already advanced
