@@ -567,8 +567,10 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
         return (s_dirty[v >> (5u + dshift)] >> ((v >> dshift) & 31u)) & (s_dirty2[(v >> 5) & (uint32_t)(kQueueCap - 1)] >> (v & 31u)) & 1u;
     };
     // serial accept engine: packed count changes per objective row of the improving records, [step parity][record][S*M]
+    // (8-byte aligned through its byte offset from s_raw, not through an integer cast of the pointer: the compiler then
+    // keeps the shared address space and emits LDS / STS instead of generic loads and stores for s_dn and s_px)
     unsigned long long* s_dn = reinterpret_cast<unsigned long long*>(
-        (reinterpret_cast<uintptr_t>(s_loff + LC::A * P.Z) + 7u) & ~(uintptr_t)7u);
+        s_raw + (((size_t)(reinterpret_cast<uint8_t*>(s_loff + LC::A * P.Z) - s_raw) + 7u) & ~(size_t)7u));
     // per record: padded index of a and of b, bit 31 = the site's cell is interior (no ghost image, neighbours = site + offset)
     uint2* s_px = reinterpret_cast<uint2*>(s_dn + 2 * kPaeK * P.S * P.M);
 
