@@ -283,9 +283,11 @@ __device__ __forceinline__ typename Pack<M>::W pack_F(const int (&F)[M])
 //         leader writes the state back, posts a phase record, and the followers reload and join.
 constexpr int kMaxTeam = 32;
 constexpr int kHaloThreads = 512;            // block size cap: 128 registers per thread, no spills in the hot paths
-constexpr int kTeamRounds = 128;            // candidates per thread per window: longer windows amortise the imbalance between
-                                            // warps and blocks at the window barrier (c4 reject regime, trials/s: 32 rounds 3.9e10,
-                                            // 64 4.1e10, 128 4.25e10, 256 4.15e10 -- two more mask registers cost more than they save)
+constexpr int kTeamRounds = 192;            // candidates per thread per window: longer windows amortise the imbalance between
+                                            // warps and blocks at the window barrier, stage 2 and the team exchange (c4 reject regime,
+                                            // trials/s, round 1: 32 rounds 3.9e10, 64 4.1e10, 128 4.25e10, 256 4.15e10; with the
+                                            // site-histogram scan: 128 7.28e10, 192 7.55e10).  Bounded by the survivor queue: 0.78 % of
+                                            // 192 x 512 candidates = 767 of its 1,024 entries
 constexpr int kNullWords = kTeamRounds / 32; // 32-bit words of the per-thread null mask
 // Reject-filter table: per ordered species pair (p, q) the elements threshold, X, L[M], Q[M], c'[M] (floats), stored
 // element-major (element e of pair i at [e * M*M + i]) so that lanes with different pairs read different banks.
