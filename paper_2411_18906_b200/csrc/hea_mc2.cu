@@ -59,7 +59,8 @@ struct Geo {
     int distinct;                 // every L >= 3: a site pair is joined by at most one lattice vector of a shell
 };
 
-constexpr int kQueueCap = 1024;
+constexpr int kQueueCap = 1536;
+constexpr int kDirty2Words = 1024;           // words of the hashed touched-site bitmap that lives in the queue
 constexpr int kPaeK = 16;                   // pipelined accept engine: candidates per step evaluated ahead
 constexpr int kPaeRecs = 512;               // records per epoch (= block threads): kPaeRecs / kPaeK steps
 
@@ -283,11 +284,11 @@ __device__ __forceinline__ typename Pack<M>::W pack_F(const int (&F)[M])
 //         leader writes the state back, posts a phase record, and the followers reload and join.
 constexpr int kMaxTeam = 32;
 constexpr int kHaloThreads = 512;            // block size cap: 128 registers per thread, no spills in the hot paths
-constexpr int kTeamRounds = 192;            // candidates per thread per window: longer windows amortise the imbalance between
+constexpr int kTeamRounds = 256;            // candidates per thread per window: longer windows amortise the imbalance between
                                             // warps and blocks at the window barrier, stage 2 and the team exchange (c4 reject regime,
                                             // trials/s, round 1: 32 rounds 3.9e10, 64 4.1e10, 128 4.25e10, 256 4.15e10; with the
-                                            // site-histogram scan: 128 7.28e10, 192 7.55e10).  Bounded by the survivor queue: 0.78 % of
-                                            // 192 x 512 candidates = 767 of its 1,024 entries
+                                            // site-histogram scan: 128 7.28e10, 192 7.55e10, 256 7.65e10).  Bounded by the survivor queue:
+                                            // 0.78 % of 256 x 512 candidates = 1,022 of its 1,536 entries (overflow: evaluated in place)
 constexpr int kNullWords = kTeamRounds / 32; // 32-bit words of the per-thread null mask
 // Reject-filter table: per ordered species pair (p, q) the elements threshold, X, L[M], Q[M], c'[M] (floats), stored
 // element-major (element e of pair i at [e * M*M + i]) so that lanes with different pairs read different banks.
@@ -556,17 +557,17 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
     const uint32_t dshift = (uint32_t)AA.dshift;
     const int dwords = (int)(((((uint32_t)P.N + (1u << dshift) - 1u) >> dshift) + 31u) >> 5);
     int* s_loff = reinterpret_cast<int*>(s_dirty + dwords);
-    // second, hashed view of the same touched set: bit (site mod 32 kQueueCap), in the words of the survivor queue (which is
+    // second, hashed view of the same touched set: bit (site mod 32 kDirty2Words), in the first words of the survivor queue (which is
     // idle while the serial accept engine runs).  A site counts as touched only when BOTH bitmaps say so: the coarse one
     // flags whole groups of 2^dshift neighbouring sites, this one separates them again (conservative: no false negative).
     uint32_t* const s_dirty2 = sh.queue;
     bool mark2 = false;                                      // inside a serial-engine epoch (block-uniform)
     auto mark_bits = [&](uint32_t v) {
         atomicOr(&s_dirty[v >> (5u + dshift)], 1u << ((v >> dshift) & 31u));
-        if (mark2) atomicOr(&s_dirty2[(v >> 5) & (uint32_t)(kQueueCap - 1)], 1u << (v & 31u));
+        if (mark2) atomicOr(&s_dirty2[(v >> 5) & (uint32_t)(kDirty2Words - 1)], 1u << (v & 31u));
     };
     auto touched = [&](uint32_t v) -> uint32_t {
-        return (s_dirty[v >> (5u + dshift)] >> ((v >> dshift) & 31u)) & (s_dirty2[(v >> 5) & (uint32_t)(kQueueCap - 1)] >> (v & 31u)) & 1u;
+        return (s_dirty[v >> (5u + dshift)] >> ((v >> dshift) & 31u)) & (s_dirty2[(v >> 5) & (uint32_t)(kDirty2Words - 1)] >> (v & 31u)) & 1u;
     };
     // serial accept engine: packed count changes per objective row of the improving records, [step parity][record][S*M]
     // (8-byte aligned through its byte offset from s_raw, not through an integer cast of the pointer: the compiler then
@@ -1135,7 +1136,7 @@ mc_halo_kernel(const KParams P, const __grid_constant__ McConst<M> Kc, const __g
                 s_px[tid] = px;
             }
             if (tid < kPaeRecs / kPaeK) sh.mlog[tid] = make_uint4(0u, 0u, 0u, 0u);
-            for (int i = tid; i < kQueueCap; i += T) s_dirty2[i] = 0u;   // the queue's words: dead between windows
+            for (int i = tid; i < kDirty2Words; i += T) s_dirty2[i] = 0u;   // the queue's words: dead between windows
             mark2 = true;
             __syncthreads();
             uint32_t e_done = 0;                                         // steps of the epoch consumed
