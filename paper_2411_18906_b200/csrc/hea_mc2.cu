@@ -284,11 +284,11 @@ __device__ __forceinline__ typename Pack<M>::W pack_F(const int (&F)[M])
 //         leader writes the state back, posts a phase record, and the followers reload and join.
 constexpr int kMaxTeam = 32;
 constexpr int kHaloThreads = 512;            // block size cap: 128 registers per thread, no spills in the hot paths
-constexpr int kTeamRounds = 256;            // candidates per thread per window: longer windows amortise the imbalance between
+constexpr int kTeamRounds = 320;            // candidates per thread per window: longer windows amortise the imbalance between
                                             // warps and blocks at the window barrier, stage 2 and the team exchange (c4 reject regime,
                                             // trials/s, round 1: 32 rounds 3.9e10, 64 4.1e10, 128 4.25e10, 256 4.15e10; with the
-                                            // site-histogram scan: 128 7.28e10, 192 7.55e10, 256 7.65e10).  Bounded by the survivor queue:
-                                            // 0.78 % of 256 x 512 candidates = 1,022 of its 1,536 entries (overflow: evaluated in place)
+                                            // site-histogram scan: 128 7.28e10, 192 7.55e10, 256 7.65e10, 320 7.74e10).  Bounded by the survivor
+                                            // queue: 0.78 % of 320 x 512 candidates = 1,278 of its 1,536 entries (overflow: evaluated in place)
 constexpr int kNullWords = kTeamRounds / 32; // 32-bit words of the per-thread null mask
 // Reject-filter table: per ordered species pair (p, q) the elements threshold, X, L[M], Q[M], c'[M] (floats), stored
 // element-major (element e of pair i at [e * M*M + i]) so that lanes with different pairs read different banks.
