@@ -37,10 +37,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-MC_REJECT_WARP_INSTR = 15_101_645_777 / 6.4e7     # per 32 trials: smsp__inst_executed.sum of the 1e6-step reject launch
-MC_REJECT_WAVEFRONTS = 1_707_580_922 / 6.4e7       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum of the same launch
-MC_REJECT_L2_SECTORS = 3_860_600_303 / 6.4e7       # l1tex__t_sectors_pipe_lsu_mem_global_op_ld.sum (site-histogram table words, via L2)
-MC_FULL_WARP_INSTR = 152_661_721_246.0             # whole c4 launch (16 chains x 1e7 steps)
+MC_REJECT_WARP_INSTR = 14_961_870_598 / 6.4e7     # per 32 trials: smsp__inst_executed.sum of the 1e6-step reject launch
+MC_REJECT_WAVEFRONTS = 1_703_546_922 / 6.4e7       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum of the same launch
+MC_REJECT_L2_SECTORS = 3_854_036_651 / 6.4e7       # l1tex__t_sectors_pipe_lsu_mem_global_op_ld.sum (site-histogram table words, via L2)
+MC_FULL_WARP_INSTR = 151_253_341_748.0             # whole c4 launch (16 chains x 1e7 steps)
 DTYPE = ("int32 counts + f64 objective (D6 order, no FMA); long windows pass a conservative fp32 reject filter on shell 1 "
          "first (rigorous error bound in its threshold, survivors evaluated in f64: accept decisions are the f64 ones); its "
          "inputs are per-site integer neighbour counts kept in a table")
@@ -60,7 +60,7 @@ def load_peaks():
 # never runs under a profiler); every use below names its source file in the JSON line.
 NCU = {
     # whole c4 trajectory, one launch: dram__bytes_read.sum + dram__bytes_write.sum
-    "mc_c4_full_dram_bytes": (7_963_904 + 110_200_576, "profiles/r2_mc_halo_c4_full.md"),
+    "mc_c4_full_dram_bytes": (8_003_584 + 69_541_120, "profiles/r2_mc_halo_c4_full.md"),
     "mc_c4_full_warp_instr": (MC_FULL_WARP_INSTR, "profiles/r2_mc_halo_c4_full.md"),
     # reject regime of c4 (1e6 steps after the trajectory): executed warp-instructions and shared-memory data-pipe
     # wavefronts per 32 trials (smsp__inst_executed.sum, l1tex__data_pipe_lsu_wavefronts_mem_shared.sum over 6.4e7 warp-trials)
