@@ -287,7 +287,7 @@ constexpr int kHaloThreads = 512;            // block size cap: 128 registers pe
 constexpr int kTeamRounds = 320;            // candidates per thread per window: longer windows amortise the imbalance between
                                             // warps and blocks at the window barrier, stage 2 and the team exchange (c4 reject regime,
                                             // trials/s, round 1: 32 rounds 3.9e10, 64 4.1e10, 128 4.25e10, 256 4.15e10; with the
-                                            // site-histogram scan: 128 7.28e10, 192 7.55e10, 256 7.65e10, 320 7.74e10).  Bounded by the survivor
+                                            // site-histogram scan: 128 7.28e10, 192 7.55e10, 256 7.65e10, 320 7.74e10; 384 with 1,752 entries 7.80e10).  Bounded by the survivor
                                             // queue: 0.78 % of 320 x 512 candidates = 1,278 of its 1,536 entries (overflow: evaluated in place)
 constexpr int kNullWords = kTeamRounds / 32; // 32-bit words of the per-thread null mask
 // Reject-filter table: per ordered species pair (p, q) the elements threshold, X, L[M], Q[M], c'[M] (floats), stored
